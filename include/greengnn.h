@@ -1,0 +1,221 @@
+/* greengnn.h -- C ABI of the B200-native hot path of GreenGNN's runtime phase
+ * (arxiv/paper_2606_02916): per-window hot-set staging for sampling-based GNN training.
+ *
+ * Citations are /root/reference/PAPER.md line numbers (section / algorithm in brackets)
+ * and DESIGN.md readings S1..S21 where the paper is silent.
+ *
+ * For each window k of W consecutive mini-batches (PAPER.md:130 [Sec. IV-A]: "partitions
+ * the epoch into ceil(B/W) windows") the library
+ *   a-1/a-2  samples every batch's multi-layer blocks with a deterministic keyed
+ *            selection ("deterministic neighbor sampling ... seeds are
+ *            fixed"); N_b = the outermost frontier ("N_b is the set of nodes
+ *            whose features batch b requires");
+ *   a-3      takes the window's unique union U_k with access counts c_k(u) over the trace
+ *            T = {(b,u) : u in N_b};
+ *   a-4      selects the hot set H_k = the n_hot most frequently accessed REMOTE nodes
+ *            (PAPER.md:130);
+ *   a-5      forms per owner m the rebuild delta Delta_{k,m} = (H_k n N_m) \ (C_{k-1} n N_m)
+ *             as one packed, ascending ID list per owner;
+ *   a-6      stages those rows with ONE bulk transfer per owner (PAPER.md:34,192 [Sec. IV-C]
+ *            "one bulk RPC per partition owner") from the owner's pinned host store into an
+ *            HBM cache, on the library's side stream, overlapped with window k-1's batches
+ *            (Alg. 1 l.8: PREFETCHER.WARMCACHE(H_{k+1} \ C), "parallel with
+ *            training"); C_k = H_k;
+ *   a-7/a-8  serves each batch: cached features for N_b n H_k, residual misses
+ *            M_b = N_b \ H_k fetched on demand (Alg. 1 l.11-14), assembling
+ *            the dense feature tensor X_b;
+ *   a-9      exports the event counts the W-selection simulator consumes (Eqs. 1-2,
+ *            per-owner |Delta_{k,m}|, |M_{b,m}| and their indicators).
+ *
+ * Conventions
+ *  - Node IDs are int32 (N < 2^31); CSR offsets int64.  Row v of the CSR lists the nodes v
+ *    aggregates from.  Owner m owns the contiguous ID range [part_offsets[m],
+ *    part_offsets[m+1]) (reading S18).  Feature rows are opaque bytes: nothing here
+ *    computes in floating point.
+ *  - "device" = memory the GPU of the current CUDA context addresses directly (cudaMalloc /
+ *    torch CUDA tensor); "host" = ordinary host memory; "pinned" = page-locked host memory
+ *    registered with CUDA (cudaHostAlloc / torch pin_memory) -- the stand-in for a remote
+ *    owner's store.
+ *  - blocks[0] is the hop out of the seeds (n_dst = batch size); blocks[L-1] is the outermost
+ *    hop whose n_src = n_input.  fanouts[h] belongs to hop h counted outward (reading S2).
+ *  - Every function returns a gg_status; none aborts or throws; on error no output is
+ *    partially valid.  gg_last_error() gives the text for the calling thread's last failure.
+ *  - One caller thread per gg_graph.  At most two windows are live (k being served, k+1
+ *    being staged).
+ */
+#ifndef GREENGNN_H_
+#define GREENGNN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GG_MAX_LAYERS 8
+#define GG_MAX_PARTS 16
+#define GG_MAX_FANOUT 96   /* selection candidate buffer is 256 entries; see DESIGN.md a-1 */
+#define GG_MAX_WINDOW 255  /* access counts are 8-bit lanes of a packed counter; W in {1..64} in PAPER.md:130 */
+
+typedef struct gg_graph gg_graph; /* opaque */
+
+typedef enum {
+  GG_OK = 0,
+  GG_ERR_INVALID_ARG = 1, /* null pointer, out-of-range value, wrong memory kind */
+  GG_ERR_STATE = 2,       /* window never staged / already released / third live window */
+  GG_ERR_CAPACITY = 3,    /* a caller buffer or a create-time cap is too small; nothing truncated */
+  GG_ERR_OOM = 4,
+  GG_ERR_CUDA = 5
+} gg_status;
+
+typedef enum { GG_F32 = 0, GG_BF16 = 1 } gg_dtype;
+
+typedef struct {
+  int64_t num_nodes, num_edges;
+  const int64_t* indptr;  /* device, [num_nodes+1] */
+  const int32_t* indices; /* device, [num_edges] */
+} gg_csr;
+
+typedef struct {
+  int32_t num_parts, local_part;
+  const int64_t* part_offsets; /* host, [num_parts+1], 0 = p[0] <= ... <= p[P] = num_nodes; copied */
+} gg_owner_map;
+
+typedef struct {
+  int32_t dim;
+  gg_dtype dtype;
+  int64_t row_stride_bytes;    /* >= dim*sizeof(elt), multiple of 4 */
+  const void* const* part_base; /* host array [P]: [local_part] = device pointer, others = pinned
+                                   host pointers; row of node u of part m at
+                                   part_base[m] + (u - part_offsets[m]) * row_stride_bytes */
+} gg_feature_store;
+
+typedef struct {
+  uint64_t seed;          /* sampling seed (first argument of the key, reading S1) */
+  int64_t n_hot;          /* hot-set budget n_hot; < 0 = unlimited */
+  int32_t carry_over;     /* 1 = stage only Delta against C_{k-1}; 0 = full restage */
+  int32_t max_layers;     /* <= GG_MAX_LAYERS */
+  int32_t max_window;     /* <= GG_MAX_WINDOW */
+  int32_t max_batch;      /* seeds per mini-batch */
+  int64_t max_cache_rows; /* rows per cache buffer; <= 0 = every remote node.  The effective
+                             budget is min(n_hot, max_cache_rows): an over-full hot set spills
+                             to the miss path, it is never an error (reading S9) */
+  int64_t max_input_nodes; /* cap on |N_b|; <= 0 = derived from the fanouts, capped at N */
+  int32_t staging_mode;   /* 0 = owner-service pack on host threads + one cudaMemcpyAsync per
+                             owner (BASELINE.json:north_star (d));
+                             1 = one GPU-initiated pull kernel per owner reading the pinned store */
+  int32_t host_threads;   /* owner-service pack threads; <= 0 = min(16, hardware threads) */
+} gg_config;
+
+/* Builds the handle.  Borrows indptr / indices / part_base pointers (caller keeps them alive
+ * and unmodified until gg_graph_destroy); copies part_offsets.  Verifies memory kinds with
+ * cudaPointerGetAttributes (GG_ERR_INVALID_ARG otherwise).  Allocates slot maps, cache
+ * buffers, the side stream and the prefetch thread.  Uses the current CUDA device. */
+gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners,
+                          const gg_feature_store* store, const gg_config* cfg, gg_graph** out);
+gg_status gg_graph_destroy(gg_graph* g);
+
+/* Alg. 1 l.7-9: hands window `window_id` to the prefetcher.  Asynchronous:
+ * returns after copying the arguments; the prefetch thread samples the W batches (a-1, a-2),
+ * builds U_k / H_k / Delta (a-3..a-5) and stages (a-6) on the library's side stream.
+ *   seeds          host int32, concatenated seed IDs of the W batches (distinct inside a batch)
+ *   batch_offsets  host int64 [W+1], batch i = seeds[batch_offsets[i] .. batch_offsets[i+1])
+ *   first_batch_index  global index of the window's first batch inside the epoch; batch i is
+ *                  keyed with first_batch_index+i (reading S7: epoch is not hashed)
+ *   fanouts        host int32 [num_layers], hop order outward from the seeds, 1..GG_MAX_FANOUT
+ * Errors: INVALID_ARG (nulls, W<1 or >max_window, L<1 or >max_layers, a batch larger than
+ * max_batch or empty window, seed outside [0,N)), STATE (two windows already live, or
+ * window_id already live), CAPACITY (caps derived from fanouts exceed int32 indexing). */
+gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_index,
+                          const int32_t* seeds, const int64_t* batch_offsets, int32_t W,
+                          const int32_t* fanouts, int32_t num_layers);
+
+typedef struct {
+  int32_t n_dst, n_src, n_edge;
+  const int32_t* indptr;    /* device [n_dst+1], 0-based inside the block */
+  const int32_t* src_local; /* device [n_edge], index into the batch's node list */
+  const int32_t* src_global; /* device [n_edge], global IDs in ascending edge position */
+} gg_block;
+
+typedef struct {
+  int32_t num_layers;
+  gg_block blocks[GG_MAX_LAYERS]; /* hop order */
+  int32_t n_input;
+  const int32_t* input_nodes; /* device [n_input] = N_b; feature row i belongs to input_nodes[i] */
+  void* features;             /* IN: caller-owned device buffer, row-major, row pitch = dim*elt */
+  int64_t features_capacity_rows; /* IN */
+  /* miss list M_b in ascending position (valid after the gather's stream work completes) */
+  const int32_t* miss_pos;  /* device [n_input] capacity */
+  const int32_t* miss_id;   /* device */
+  const int32_t* n_miss;    /* device scalar */
+} gg_batch_out;
+
+/* Blocks until the prefetcher has finished ENQUEUING window_id (the brief wait of Alg. 1 l.5,
+ * PAPER.md:194), then fills sizes and device pointers of batch `batch_in_window`.  Pointers
+ * stay valid until gg_window_release.  Does not touch `features*`. */
+gg_status gg_batch_info(gg_graph* g, int64_t window_id, int32_t batch_in_window, gg_batch_out* out);
+
+/* Alg. 1 l.11-14.  Asynchronous on `cuda_stream` (a cudaStream_t; NULL = default stream): makes
+ * the stream wait for the window's cache-ready event, gathers X_b (local rows from the HBM
+ * store, hot rows through the ID->slot map from the cache, a-7), compacts the misses and fills
+ * them from the owners' pinned stores (a-8).  Fills `out` like gg_batch_info.
+ * Errors: STATE, CAPACITY (features_capacity_rows < n_input), INVALID_ARG (features null or
+ * not 4-byte aligned). */
+gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t batch_in_window,
+                          gg_batch_out* out, void* cuda_stream);
+
+/* Frees the window's blocks; its cache buffer becomes reusable once the gathers already
+ * enqueued have run (the library orders this with events, the call does not block on the GPU). */
+gg_status gg_window_release(gg_graph* g, int64_t window_id);
+
+typedef struct {
+  int32_t W, num_parts;
+  int64_t n_access;        /* sum_b |N_b| = |T restricted to the window| */
+  int64_t n_unique;        /* |U_k| */
+  int64_t n_unique_remote; /* |R_k| */
+  int64_t n_hot;           /* |H_k| */
+  int64_t carried_rows;    /* |H_k n C_{k-1}| (0 when carry_over = 0) */
+  int64_t staged_rows[GG_MAX_PARTS]; /* |H_k n N_m| */
+  int64_t bulk_rows[GG_MAX_PARTS];   /* |Delta_{k,m}|; 0 => no transfer issued (Eq. 1 indicator) */
+  int64_t bulk_bytes[GG_MAX_PARTS];
+  int32_t bulk_copies;     /* transfers issued = #owners with Delta != empty */
+  /* per batch, caller-provided host arrays (may be NULL to skip) */
+  int32_t* n_input;   /* [W] */
+  int32_t* hit_local; /* [W] */
+  int32_t* hit_cache; /* [W] */
+  int32_t* miss;      /* [W*num_parts], miss[b*num_parts+m] = |M_{b,m}| (Eq. 2) */
+  /* timings in ms, informational (not parity-checked) */
+  float ms_sample, ms_unique, ms_select, ms_pack_host, ms_h2d, ms_carry, ms_stage_total;
+  float ms_boundary_wait; /* host time gg_batch_info/gather spent waiting for this window */
+} gg_window_trace;
+
+/* Synchronises the window's staging and every gather enqueued so far for it, then fills `out`.
+ * Per-batch hit/miss counters of batches not gathered yet are 0. */
+gg_status gg_trace(gg_graph* g, int64_t window_id, gg_window_trace* out);
+
+/* Parity / simulator export of the window's lists to HOST buffers (synchronises staging).
+ * what: 0 = uniq (U_k ascending), 1 = cnt (c_k aligned with uniq), 2 = hot (H_k ascending),
+ *       3 = request IDs (Delta_{k,m} ascending, owners ascending, concatenated),
+ *       4 = carried IDs (ascending).
+ * Writes min(n, capacity) int32 values and stores n in *n_out; CAPACITY if capacity < n. */
+gg_status gg_window_export(gg_graph* g, int64_t window_id, int32_t what, int32_t* out,
+                           int64_t capacity, int64_t* n_out);
+
+/* Parity helper: reads back cache rows of the given global IDs for a staged window
+ * (row at slot_of[u]); ids absent from H_k give GG_ERR_INVALID_ARG.  out: host, n*row_bytes. */
+gg_status gg_cache_read(gg_graph* g, int64_t window_id, const int32_t* ids, int64_t n, void* out);
+
+/* C <- empty (Alg. 1 l.1); requires no live window. */
+gg_status gg_cache_reset(gg_graph* g);
+
+/* The sampling key of reading S1, evaluated by the library's own hash (host function; parity
+ * pin against tests/golden/keys.txt). */
+uint64_t gg_key(uint64_t seed, uint64_t batch, uint64_t layer, uint64_t dst, uint64_t edge_pos);
+
+const char* gg_last_error(void);
+const char* gg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GREENGNN_H_ */

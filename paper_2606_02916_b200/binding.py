@@ -1,0 +1,268 @@
+"""Thin ctypes binding of include/greengnn.h: argument marshalling only.
+
+Every step of the path runs inside libgreengnn.so's CUDA kernels; torch is used here for
+device memory (`data_ptr()`), streams and zero-copy views of the library's device arrays.
+There is NO CPU fallback: if the library has not been built or cannot be loaded this module
+raises (build with `python -m paper_2606_02916_b200.build`).
+"""
+from __future__ import annotations
+
+import contextlib
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+GG_MAX_LAYERS, GG_MAX_PARTS, GG_MAX_FANOUT, GG_MAX_WINDOW = 8, 16, 96, 255
+GG_OK, GG_ERR_INVALID_ARG, GG_ERR_STATE, GG_ERR_CAPACITY, GG_ERR_OOM, GG_ERR_CUDA = range(6)
+_STATUS = {0: "GG_OK", 1: "GG_ERR_INVALID_ARG", 2: "GG_ERR_STATE", 3: "GG_ERR_CAPACITY",
+           4: "GG_ERR_OOM", 5: "GG_ERR_CUDA"}
+
+i32, i64, u64, vp, f32 = C.c_int32, C.c_int64, C.c_uint64, C.c_void_p, C.c_float
+
+
+class gg_csr(C.Structure):
+    _fields_ = [("num_nodes", i64), ("num_edges", i64), ("indptr", vp), ("indices", vp)]
+
+
+class gg_owner_map(C.Structure):
+    _fields_ = [("num_parts", i32), ("local_part", i32), ("part_offsets", vp)]
+
+
+class gg_feature_store(C.Structure):
+    _fields_ = [("dim", i32), ("dtype", i32), ("row_stride_bytes", i64), ("part_base", vp)]
+
+
+class gg_config(C.Structure):
+    _fields_ = [("seed", u64), ("n_hot", i64), ("carry_over", i32), ("max_layers", i32),
+                ("max_window", i32), ("max_batch", i32), ("max_cache_rows", i64),
+                ("max_input_nodes", i64), ("staging_mode", i32), ("host_threads", i32)]
+
+
+class gg_block(C.Structure):
+    _fields_ = [("n_dst", i32), ("n_src", i32), ("n_edge", i32), ("indptr", vp), ("src_local", vp),
+                ("src_global", vp)]
+
+
+class gg_batch_out(C.Structure):
+    _fields_ = [("num_layers", i32), ("blocks", gg_block * GG_MAX_LAYERS), ("n_input", i32),
+                ("input_nodes", vp), ("features", vp), ("features_capacity_rows", i64),
+                ("miss_pos", vp), ("miss_id", vp), ("n_miss", vp)]
+
+
+class gg_window_trace(C.Structure):
+    _fields_ = [("W", i32), ("num_parts", i32), ("n_access", i64), ("n_unique", i64),
+                ("n_unique_remote", i64), ("n_hot", i64), ("carried_rows", i64),
+                ("staged_rows", i64 * GG_MAX_PARTS), ("bulk_rows", i64 * GG_MAX_PARTS),
+                ("bulk_bytes", i64 * GG_MAX_PARTS), ("bulk_copies", i32),
+                ("n_input", vp), ("hit_local", vp), ("hit_cache", vp), ("miss", vp),
+                ("ms_sample", f32), ("ms_unique", f32), ("ms_select", f32), ("ms_pack_host", f32),
+                ("ms_h2d", f32), ("ms_carry", f32), ("ms_stage_total", f32), ("ms_boundary_wait", f32)]
+
+
+SYMBOLS = ["gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
+           "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
+           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version"]
+
+_lib = None
+
+
+class GreenGNNError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__("%s: %s" % (_STATUS.get(status, status), text))
+        self.status = status
+
+
+def load_library(path: Optional[str] = None):
+    """Loads libgreengnn.so; raises if it is missing (no fallback of any kind)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _build.LIB
+    if not os.path.exists(path):
+        raise ImportError("libgreengnn.so is not built (%s); run `python -m paper_2606_02916_b200.build`"
+                          % path)
+    lib = C.CDLL(path)
+    P = C.POINTER
+    lib.gg_graph_create.argtypes = [P(gg_csr), P(gg_owner_map), P(gg_feature_store), P(gg_config), P(vp)]
+    lib.gg_graph_destroy.argtypes = [vp]
+    lib.gg_window_stage.argtypes = [vp, i64, u64, vp, vp, i32, vp, i32]
+    lib.gg_batch_info.argtypes = [vp, i64, i32, P(gg_batch_out)]
+    lib.gg_batch_gather.argtypes = [vp, i64, i32, P(gg_batch_out), vp]
+    lib.gg_window_release.argtypes = [vp, i64]
+    lib.gg_trace.argtypes = [vp, i64, P(gg_window_trace)]
+    lib.gg_window_export.argtypes = [vp, i64, i32, vp, i64, P(i64)]
+    lib.gg_cache_read.argtypes = [vp, i64, vp, i64, vp]
+    lib.gg_cache_reset.argtypes = [vp]
+    lib.gg_key.argtypes = [u64] * 5
+    lib.gg_key.restype = u64
+    lib.gg_last_error.restype = C.c_char_p
+    lib.gg_version.restype = C.c_char_p
+    for s in SYMBOLS:
+        getattr(lib, s)
+        if s not in ("gg_key", "gg_last_error", "gg_version"):
+            getattr(lib, s).restype = i32
+    _lib = lib
+    return lib
+
+
+def gg_key(seed: int, batch: int, layer: int, dst: int, edge_pos: int) -> int:
+    return load_library().gg_key(seed, batch, layer, dst, edge_pos)
+
+
+class _DevView:
+    """Zero-copy torch view of `n` elements of library-owned device memory."""
+
+    def __init__(self, ptr: int, n: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, False),
+                                         "version": 2, "strides": None}
+
+
+def _view_i32(ptr, n: int, device) -> torch.Tensor:
+    if n == 0 or not ptr:
+        return torch.empty(0, dtype=torch.int32, device=device)
+    return torch.as_tensor(_DevView(int(ptr), int(n), "<i4"), device=device)
+
+
+class Graph:
+    """gg_graph handle.  Tensors passed in are borrowed and kept referenced here."""
+
+    def __init__(self, indptr: torch.Tensor, indices: torch.Tensor, part_offsets: Sequence[int],
+                 local_part: int, feat_parts: List[torch.Tensor], seed: int, n_hot: int = -1,
+                 carry_over: int = 1, max_layers: int = 3, max_window: int = 32, max_batch: int = 1024,
+                 max_cache_rows: int = 0, max_input_nodes: int = 0, staging_mode: int = 0,
+                 host_threads: int = 0):
+        self.lib = load_library()
+        assert indptr.dtype == torch.int64 and indices.dtype == torch.int32
+        self._keep = (indptr, indices, feat_parts)
+        self.device = indptr.device
+        self.P = len(part_offsets) - 1
+        self.po = np.ascontiguousarray(part_offsets, dtype=np.int64)
+        self.dim = int(feat_parts[local_part].shape[1])
+        self.feat_dtype = feat_parts[local_part].dtype
+        esz = feat_parts[local_part].element_size()
+        self.rb = self.dim * esz
+        csr = gg_csr(indptr.numel() - 1, indices.numel(), indptr.data_ptr(), indices.data_ptr())
+        om = gg_owner_map(self.P, local_part, self.po.ctypes.data)
+        bases = (vp * self.P)(*[p.data_ptr() if p.numel() else None for p in feat_parts])
+        strides = {int(p.stride(0)) * esz for p in feat_parts if p.numel()}
+        assert len(strides) == 1, "all parts must share one row stride"
+        fs = gg_feature_store(self.dim, {torch.float32: 0, torch.bfloat16: 1}[self.feat_dtype],
+                              strides.pop(), C.cast(bases, vp))
+        cfg = gg_config(seed & ((1 << 64) - 1), n_hot, carry_over, max_layers, max_window, max_batch,
+                        max_cache_rows, max_input_nodes, staging_mode, host_threads)
+        h = vp()
+        ctx = torch.cuda.device(self.device) if self.device.type == "cuda" else contextlib.nullcontext()
+        with ctx:
+            self._check(self.lib.gg_graph_create(C.byref(csr), C.byref(om), C.byref(fs), C.byref(cfg),
+                                                 C.byref(h)))
+        self.h = h
+
+    def _check(self, rc: int):
+        if rc != GG_OK:
+            raise GreenGNNError(rc, (self.lib.gg_last_error() or b"").decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.gg_graph_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- gg_window_stage ---------------------------------------------------------------------
+    def window_stage(self, window_id: int, first_batch_index: int, batches: Sequence[np.ndarray],
+                     fanouts: Sequence[int]):
+        seeds = np.ascontiguousarray(np.concatenate([np.asarray(b, dtype=np.int32) for b in batches])
+                                     if len(batches) else np.zeros(0, np.int32), dtype=np.int32)
+        off = np.zeros(len(batches) + 1, dtype=np.int64)
+        off[1:] = np.cumsum([len(b) for b in batches])
+        fo = np.ascontiguousarray(fanouts, dtype=np.int32)
+        self._check(self.lib.gg_window_stage(self.h, window_id, first_batch_index, seeds.ctypes.data,
+                                             off.ctypes.data, len(batches), fo.ctypes.data, len(fo)))
+
+    # -- gg_batch_info / gg_batch_gather -----------------------------------------------------
+    def _unpack(self, o: gg_batch_out) -> Dict:
+        dev = self.device
+        blocks = []
+        for h in range(o.num_layers):
+            k = o.blocks[h]
+            blocks.append(dict(n_dst=k.n_dst, n_src=k.n_src, n_edge=k.n_edge,
+                               indptr=_view_i32(k.indptr, k.n_dst + 1, dev),
+                               src_local=_view_i32(k.src_local, k.n_edge, dev),
+                               src_global=_view_i32(k.src_global, k.n_edge, dev)))
+        return dict(blocks=blocks, n_input=o.n_input, input_nodes=_view_i32(o.input_nodes, o.n_input, dev),
+                    _miss=(o.miss_pos, o.miss_id, o.n_miss))
+
+    def batch_info(self, window_id: int, b: int) -> Dict:
+        o = gg_batch_out()
+        self._check(self.lib.gg_batch_info(self.h, window_id, b, C.byref(o)))
+        return self._unpack(o)
+
+    def batch_gather(self, window_id: int, b: int, features: torch.Tensor,
+                     stream: Optional[torch.cuda.Stream] = None) -> Dict:
+        """features: caller-owned device buffer [capacity_rows, dim]; X_b = features[:n_input]."""
+        assert features.is_cuda and features.is_contiguous() and features.shape[1] == self.dim
+        assert features.dtype == self.feat_dtype
+        o = gg_batch_out()
+        o.features = features.data_ptr()
+        o.features_capacity_rows = features.shape[0]
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._check(self.lib.gg_batch_gather(self.h, window_id, b, C.byref(o), st.cuda_stream))
+        r = self._unpack(o)
+        r["features"] = features[:o.n_input]
+        return r
+
+    def misses(self, r: Dict):
+        """(miss_pos, miss_id) of the LAST gather as host arrays (synchronises)."""
+        torch.cuda.synchronize(self.device)
+        mp, mi, nm = r["_miss"]
+        n = int(_view_i32(nm, 1, self.device).cpu()[0])
+        return (_view_i32(mp, n, self.device).cpu().numpy(), _view_i32(mi, n, self.device).cpu().numpy())
+
+    def window_release(self, window_id: int):
+        self._check(self.lib.gg_window_release(self.h, window_id))
+
+    # -- gg_trace / exports --------------------------------------------------------------------
+    def trace(self, window_id: int, W: int) -> Dict:
+        t = gg_window_trace()
+        n_input = np.zeros(W, np.int32)
+        hl = np.zeros(W, np.int32)
+        hc = np.zeros(W, np.int32)
+        miss = np.zeros((W, self.P), np.int32)
+        t.n_input, t.hit_local, t.hit_cache, t.miss = (a.ctypes.data for a in (n_input, hl, hc, miss))
+        self._check(self.lib.gg_trace(self.h, window_id, C.byref(t)))
+        P = self.P
+        d = {k: getattr(t, k) for k in ("W", "num_parts", "n_access", "n_unique", "n_unique_remote", "n_hot",
+                                        "carried_rows", "bulk_copies", "ms_sample", "ms_unique", "ms_select",
+                                        "ms_pack_host", "ms_h2d", "ms_carry", "ms_stage_total",
+                                        "ms_boundary_wait")}
+        d.update(staged_rows=list(t.staged_rows)[:P], bulk_rows=list(t.bulk_rows)[:P],
+                 bulk_bytes=list(t.bulk_bytes)[:P], n_input=n_input, hit_local=hl, hit_cache=hc, miss=miss)
+        return d
+
+    def window_export(self, window_id: int, what: str) -> np.ndarray:
+        code = {"uniq": 0, "cnt": 1, "hot": 2, "req": 3, "carried": 4}[what]
+        n = i64(0)
+        rc = self.lib.gg_window_export(self.h, window_id, code, None, 0, C.byref(n))
+        if rc not in (GG_OK, GG_ERR_CAPACITY):
+            self._check(rc)
+        out = np.empty(max(n.value, 1), dtype=np.int32)
+        self._check(self.lib.gg_window_export(self.h, window_id, code, out.ctypes.data, len(out), C.byref(n)))
+        return out[:n.value].copy()
+
+    def cache_read(self, window_id: int, ids: np.ndarray) -> np.ndarray:
+        ids = np.ascontiguousarray(ids, dtype=np.int32)
+        out = np.empty((len(ids), self.rb), dtype=np.uint8)
+        self._check(self.lib.gg_cache_read(self.h, window_id, ids.ctypes.data, len(ids), out.ctypes.data))
+        return out
+
+    def cache_reset(self):
+        self._check(self.lib.gg_cache_reset(self.h))

@@ -1,0 +1,925 @@
+// Host orchestration behind the C ABI of include/greengnn.h.
+//
+// Threads and streams (Alg. 1):
+//   caller thread   gg_window_stage enqueues a job; gg_batch_gather launches the per-batch kernels
+//                   on the caller's stream after making it wait for the window's cache-ready event
+//   prefetch thread owns the side stream: samples the window, builds U_k / H_k / Delta, runs the
+//                   owner service (host pack) and issues one bulk copy per owner -- all while the
+//                   caller's stream serves the previous window ("Parallel with training", l.8)
+// Two window slots ping-pong (slot = stage counter & 1): each holds the window's blocks, its
+// cache buffer, its ID->slot map and the list of cached IDs (= C_k).
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <condition_variable>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <deque>
+#include <functional>
+#include <mutex>
+#include <string>
+#include <thread>
+#include <vector>
+
+#include "common.cuh"
+#include "kernels.h"
+
+namespace gg {
+
+static thread_local std::string t_err;
+static gg_status fail(gg_status s, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  t_err = buf;
+  return s;
+}
+#define CU(call)                                                                          \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess)                                                                \
+      return fail(GG_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+static double now_ms() {
+  using namespace std::chrono;
+  return duration<double, std::milli>(steady_clock::now().time_since_epoch()).count();
+}
+
+// ---- tiny persistent thread pool for the owner-service pack --------------------------------
+class Pool {
+ public:
+  explicit Pool(int n) : stop_(false), gen_(0), pending_(0) {
+    for (int i = 0; i < n; ++i) th_.emplace_back([this] { run(); });
+  }
+  ~Pool() {
+    {
+      std::lock_guard<std::mutex> l(m_);
+      stop_ = true;
+    }
+    cv_.notify_all();
+    for (auto& t : th_) t.join();
+  }
+  // fn(chunk) for chunk in [0, n); returns when all are done
+  void parallel_for(int64_t n, const std::function<void(int64_t)>& fn) {
+    if (n <= 0) return;
+    if (th_.empty() || n == 1) {
+      for (int64_t i = 0; i < n; ++i) fn(i);
+      return;
+    }
+    {
+      std::lock_guard<std::mutex> l(m_);
+      fn_ = &fn;
+      n_ = n;
+      next_.store(0);
+      pending_ = (int)th_.size();
+      ++gen_;
+    }
+    cv_.notify_all();
+    std::unique_lock<std::mutex> l(m_);
+    done_.wait(l, [this] { return pending_ == 0; });
+  }
+
+ private:
+  void run() {
+    uint64_t seen = 0;
+    for (;;) {
+      const std::function<void(int64_t)>* fn;
+      int64_t n;
+      {
+        std::unique_lock<std::mutex> l(m_);
+        cv_.wait(l, [&] { return stop_ || gen_ != seen; });
+        if (stop_) return;
+        seen = gen_;
+        fn = fn_;
+        n = n_;
+      }
+      for (;;) {
+        const int64_t i = next_.fetch_add(1);
+        if (i >= n) break;
+        (*fn)(i);
+      }
+      std::lock_guard<std::mutex> l(m_);
+      if (--pending_ == 0) done_.notify_all();
+    }
+  }
+  std::vector<std::thread> th_;
+  std::mutex m_;
+  std::condition_variable cv_, done_;
+  bool stop_;
+  uint64_t gen_;
+  int pending_;
+  const std::function<void(int64_t)>* fn_ = nullptr;
+  int64_t n_ = 0;
+  std::atomic<int64_t> next_{0};
+};
+
+template <typename T>
+struct DevBuf {
+  T* p = nullptr;
+  int64_t n = 0;
+  cudaError_t ensure(int64_t want) {
+    if (want <= n) return cudaSuccess;
+    if (p) cudaFree(p);
+    p = nullptr;
+    n = 0;
+    cudaError_t e = cudaMalloc((void**)&p, (size_t)want * sizeof(T));
+    if (e == cudaSuccess) n = want;
+    return e;
+  }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    n = 0;
+  }
+};
+
+struct Hop {
+  DevBuf<int32_t> blk_indptr, src_global, src_local, edge_off_dev;
+  std::vector<int32_t> edge_off;  // host [W+1]
+  std::vector<int32_t> dst_off;   // host [W+1]
+};
+
+struct Window {
+  // identity / arguments
+  int64_t id = -1;
+  bool live = false;
+  int slot = 0;
+  int W = 0, L = 0;
+  int fanouts[GG_MAX_LAYERS] = {0};
+  uint64_t first_batch = 0;
+  std::vector<int32_t> seeds;
+  std::vector<int64_t> boff;
+  // device arena
+  DevBuf<int32_t> nodes, n_front_dev, uniq, cnt, req_ids, carry_src, carry_ids, counters;
+  int64_t node_pitch = 0;
+  Hop hop[GG_MAX_LAYERS];
+  std::vector<int32_t> n_front[GG_MAX_LAYERS + 1];  // host mirrors [W]
+  // cache slot (C_k): buffer, map and cached-ID list persist after release
+  uint8_t* cache = nullptr;
+  int32_t* slot_map = nullptr;
+  DevBuf<int32_t> hot;
+  int64_t n_cached = 0;  // entries of `hot` currently reflected in slot_map
+  // results
+  int64_t n_access = 0, n_unique = 0, n_remote = 0, n_hot = 0, n_delta = 0, n_carry = 0;
+  int64_t staged[GG_MAX_PARTS] = {0}, bulk[GG_MAX_PARTS] = {0};
+  int bulk_copies = 0;
+  bool may_miss = false;
+  float ms_sample = 0, ms_unique = 0, ms_select = 0, ms_pack = 0, ms_h2d = 0, ms_carry = 0,
+        ms_total = 0, ms_wait = 0;
+  // sync
+  cudaEvent_t ready = nullptr, gather_done = nullptr;
+  bool gather_recorded = false;
+  bool enqueued = false;
+  gg_status status = GG_OK;
+  std::string error;
+};
+
+}  // namespace gg
+
+using namespace gg;
+
+struct gg_graph {
+  // inputs
+  int64_t N = 0, nnz = 0;
+  const int64_t* indptr = nullptr;
+  const int32_t* indices = nullptr;
+  OwnerRanges R;
+  StorePtrs store;
+  int dim = 0, rb = 0;
+  gg_dtype dtype = GG_F32;
+  gg_config cfg;
+  int64_t cache_rows = 0, n_hot_eff = 0;
+  int device = 0;
+  // workspaces (prefetch thread only)
+  FrontierBufs F = {};
+  int n_gen = 0;
+  DevBuf<uint32_t> seen, newbits, cnt8;
+  DevBuf<int32_t> wprefix, seed_perm, tiles32, totals, stats, hist, owner_cnt, n_delta_dev, err_flag,
+      seeds_dev;
+  DevBuf<uint64_t> tiles64, total64, key_prefix;
+  DevBuf<uint8_t> cnt_tmp;
+  int64_t cnt_words = 0;  // padded words of cnt8
+  // miss buffers (caller thread, one gather at a time)
+  DevBuf<int32_t> miss_tmp_pos, miss_tmp_id, tile_miss, miss_pos, miss_id, n_miss;
+  // pinned
+  int32_t* h_small = nullptr;  // readback scratch
+  int32_t* h_req = nullptr;    // request IDs (device -> host)
+  uint8_t* h_resp = nullptr;   // packed rows (host -> device), mode 0
+  int32_t* h_seeds = nullptr;
+  int64_t h_seeds_cap = 0, h_req_cap = 0, h_resp_cap = 0;
+  uint64_t* h_kp = nullptr;
+  // streams / thread
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_a = nullptr, ev_b = nullptr;
+  Window win[2];
+  uint64_t stage_counter = 0;
+  bool have_prev = false;
+  int prev_slot = 0;
+  std::thread worker;
+  std::mutex mu;
+  std::condition_variable cv_job, cv_done;
+  std::deque<Window*> jobs;
+  bool stop = false;
+  Pool* pool = nullptr;
+};
+
+namespace gg {
+
+static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// caps derived from the fanouts (frontier_{h+1} <= frontier_h * (1 + f[h]), also <= N)
+static gg_status plan_and_alloc(gg_graph* g, Window* w) {
+  const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
+  int64_t cap_front[GG_MAX_LAYERS + 1];
+  cap_front[0] = g->cfg.max_batch;
+  for (int h = 0; h < L; ++h) {
+    int64_t c = cap_front[h] * (1 + (int64_t)w->fanouts[h]);
+    if (c > g->N) c = g->N;
+    if (g->cfg.max_input_nodes > 0 && c > g->cfg.max_input_nodes) c = g->cfg.max_input_nodes;
+    if (c < cap_front[h]) c = cap_front[h];
+    cap_front[h + 1] = c;
+  }
+  w->node_pitch = ceil_div(cap_front[L], 4) * 4;
+  if ((int64_t)W * w->node_pitch >= (1ll << 31))
+    return fail(GG_ERR_CAPACITY, "W * max_input_nodes = %lld exceeds int32 indexing",
+                (long long)((int64_t)W * w->node_pitch));
+#define ENS(buf, n)                                                                       \
+  do {                                                                                    \
+    if ((buf).ensure(n) != cudaSuccess) {                                                 \
+      cudaGetLastError();                                                                 \
+      return fail(GG_ERR_OOM, "device allocation of %lld elements failed (%s)", (long long)(n), #buf); \
+    }                                                                                     \
+  } while (0)
+  ENS(w->nodes, (int64_t)W * w->node_pitch);
+  ENS(w->n_front_dev, (int64_t)(GG_MAX_LAYERS + 1) * Wmax);
+  int64_t max_tiles = 1;
+  for (int h = 0; h < L; ++h) {
+    const int64_t ecap = (int64_t)W * cap_front[h] * w->fanouts[h];
+    if (ecap >= (1ll << 31))
+      return fail(GG_ERR_CAPACITY, "hop %d edge cap %lld exceeds int32 indexing", h, (long long)ecap);
+    ENS(w->hop[h].blk_indptr, (int64_t)W * cap_front[h] + W);
+    ENS(w->hop[h].src_global, ecap);
+    ENS(w->hop[h].src_local, ecap);
+    ENS(w->hop[h].edge_off_dev, W + 1);
+    max_tiles = std::max(max_tiles, ceil_div(cap_front[h], 256));
+  }
+  const int64_t ucap = std::min<int64_t>(g->N, (int64_t)W * w->node_pitch);
+  ENS(w->uniq, ucap);
+  ENS(w->cnt, ucap);
+  ENS(w->req_ids, std::max<int64_t>(g->cache_rows, 1));
+  ENS(w->carry_src, std::max<int64_t>(g->cache_rows, 1));
+  ENS(w->carry_ids, std::max<int64_t>(g->cache_rows, 1));
+  ENS(w->hot, std::max<int64_t>(g->cache_rows, 1));
+  ENS(w->counters, (int64_t)Wmax * (2 + GG_MAX_PARTS));
+  ENS(g->cnt_tmp, (int64_t)W * cap_front[L - 1]);
+  int64_t t32 = std::max<int64_t>((int64_t)W * max_tiles, (int64_t)W * g->F.n_wtiles);
+  t32 = std::max<int64_t>(t32, g->cnt_words / kWordTile);
+  t32 = std::max<int64_t>(t32, ceil_div(g->cache_rows, 1024) + 1);
+  ENS(g->tiles32, t32);
+  ENS(g->tiles64, ceil_div(ucap, 1024) + 1);
+  // miss buffers are sized by the largest |N_b|
+  const int64_t mcap = ceil_div(w->node_pitch, 64) * 64;
+  ENS(g->miss_tmp_pos, mcap);
+  ENS(g->miss_tmp_id, mcap);
+  ENS(g->tile_miss, mcap / 64);
+  ENS(g->miss_pos, mcap);
+  ENS(g->miss_id, mcap);
+#undef ENS
+  (void)cap_front;
+  return GG_OK;
+}
+
+static gg_status ensure_pinned(void** p, int64_t* cap, int64_t want) {
+  if (want <= *cap) return GG_OK;
+  if (*p) cudaFreeHost(*p);
+  *p = nullptr;
+  *cap = 0;
+  const int64_t n = want + want / 2 + 4096;
+  if (cudaHostAlloc(p, (size_t)n, cudaHostAllocDefault) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(GG_ERR_OOM, "pinned host allocation of %lld bytes failed", (long long)n);
+  }
+  *cap = n;
+  return GG_OK;
+}
+
+}  // namespace gg
+
+namespace gg {
+
+// ---- the prefetcher's work for one window (runs on the prefetch thread, side stream) --------
+static gg_status stage_window(gg_graph* g, Window* w) {
+  const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
+  cudaStream_t st = g->side;
+  const double t0 = now_ms();
+  CU(cudaSetDevice(g->device));
+  gg_status rc = plan_and_alloc(g, w);
+  if (rc != GG_OK) return rc;
+  Window* prev = g->have_prev ? &g->win[g->prev_slot] : nullptr;
+  // the slot's previous tenant (window k-2) may still be read by gathers already enqueued
+  if (w->gather_recorded) CU(cudaStreamWaitEvent(st, w->gather_done, 0));
+
+  // seeds and per-(batch, layer) key prefixes -> device
+  BatchOffsets seed_off;
+  for (int b = 0; b <= W; ++b) seed_off.v[b] = (int32_t)w->boff[b];
+  const int S = seed_off.v[W];
+  std::memcpy(g->h_seeds, w->seeds.data(), (size_t)S * sizeof(int32_t));
+  for (int h = 0; h < L; ++h)
+    for (int b = 0; b < W; ++b)
+      g->h_kp[h * Wmax + b] = key_prefix(g->cfg.seed, w->first_batch + (uint64_t)b, (uint64_t)h);
+  CU(cudaMemcpyAsync(g->seeds_dev.p, g->h_seeds, (size_t)S * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(g->key_prefix.p, g->h_kp, (size_t)L * Wmax * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
+  CU(cudaMemsetAsync(g->err_flag.p, 0, sizeof(int32_t), st));
+
+  // a-1 / a-2, hop by hop over the whole window
+  w->n_front[0].assign(W, 0);
+  for (int b = 0; b < W; ++b) w->n_front[0][b] = seed_off.v[b + 1] - seed_off.v[b];
+  launch_seed_init(st, g->F, g->seeds_dev.p, seed_off, W, w->nodes.p, w->node_pitch, g->cnt8.p,
+                   w->n_front_dev.p, g->tiles32.p, g->totals.p + Wmax);
+  int32_t* edge_totals = g->totals.p;          // [Wmax]
+  int32_t* new_totals = g->totals.p + Wmax;    // [Wmax]
+  for (int h = 0; h < L; ++h) {
+    Hop& H = w->hop[h];
+    BatchOffsets n_dst, dst_off;
+    int max_nd = 0;
+    H.dst_off.assign(W + 1, 0);
+    for (int b = 0; b < W; ++b) {
+      n_dst.v[b] = w->n_front[h][b];
+      dst_off.v[b] = H.dst_off[b];
+      H.dst_off[b + 1] = H.dst_off[b] + n_dst.v[b];
+      max_nd = std::max(max_nd, n_dst.v[b]);
+    }
+    dst_off.v[W] = H.dst_off[W];
+    const int max_tiles = (int)ceil_div(max_nd, 256);
+    const int64_t cnt_pitch = max_nd;
+    launch_sample_hop(st, g->indptr, g->indices, w->nodes.p, w->node_pitch, n_dst, dst_off, W, max_nd,
+                      w->fanouts[h], g->key_prefix.p + h * Wmax, g->cnt_tmp.p, cnt_pitch, g->tiles32.p,
+                      max_tiles, edge_totals, H.blk_indptr.p, H.edge_off_dev.p, H.src_global.p);
+    const int64_t max_edges = (int64_t)H.dst_off[W] * w->fanouts[h];
+    launch_frontier_hop(st, g->F, h, W, H.src_global.p, H.edge_off_dev.p, max_edges, n_dst,
+                        (int32_t)w->node_pitch, w->nodes.p, w->node_pitch, g->cnt8.p, w->n_front_dev.p,
+                        Wmax, g->tiles32.p, new_totals, g->err_flag.p, H.src_local.p);
+    // sizes of the next frontier and of this hop's blocks -> host
+    CU(cudaMemcpyAsync(g->h_small, w->n_front_dev.p + (h + 1) * Wmax, W * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(g->h_small + Wmax, H.edge_off_dev.p, (W + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(g->h_small + 2 * Wmax + 2, g->err_flag.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (g->h_small[2 * Wmax + 2])
+      return fail(GG_ERR_CAPACITY, "hop %d: a batch's frontier exceeds max_input_nodes = %lld", h,
+                  (long long)w->node_pitch);
+    w->n_front[h + 1].assign(g->h_small, g->h_small + W);
+    H.edge_off.assign(g->h_small + Wmax, g->h_small + Wmax + W + 1);
+  }
+  int max_n = 0;
+  w->n_access = 0;
+  for (int b = 0; b < W; ++b) {
+    max_n = std::max(max_n, w->n_front[L][b]);
+    w->n_access += w->n_front[L][b];
+  }
+  launch_bitmap_clear(st, g->F, w->nodes.p, w->node_pitch, w->n_front_dev.p + L * Wmax, max_n, W, L + 1);
+  const double t1 = now_ms();
+  w->ms_sample = (float)(t1 - t0);
+
+  // a-3 unique + count
+  launch_unique_count(st, g->cnt8.p, g->cnt_words, g->R, g->tiles32.p, g->stats.p, g->hist.p, w->uniq.p, w->cnt.p);
+  CU(cudaMemcpyAsync(g->h_small, g->stats.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(g->h_small + 1, g->hist.p, 256 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  w->n_unique = g->h_small[0];
+  const int32_t* hist = g->h_small + 1;
+  w->n_remote = 0;
+  for (int c = 1; c < 256; ++c) w->n_remote += hist[c];
+  const double t2 = now_ms();
+  w->ms_unique = (float)(t2 - t1);
+
+  // a-4 hot set: threshold t and quota of count == t nodes from the histogram
+  int32_t thr = 0;
+  uint32_t quota = 0;
+  if (w->n_remote <= g->n_hot_eff) {
+    w->n_hot = w->n_remote;
+    w->may_miss = false;
+  } else {
+    w->n_hot = g->n_hot_eff;
+    w->may_miss = true;
+    int64_t above = 0;
+    for (thr = 255; thr >= 1; --thr) {
+      if (above + hist[thr] > w->n_hot) break;
+      above += hist[thr];
+    }
+    quota = (uint32_t)(w->n_hot - above);
+  }
+  launch_slots_clear(st, w->hot.p, (int)w->n_cached, w->slot_map);
+  w->n_cached = 0;
+  if (w->n_hot > 0)
+    launch_hot_select(st, w->uniq.p, w->cnt.p, (int)w->n_unique, g->R, thr, quota, g->tiles64.p, g->total64.p, w->hot.p);
+  // a-5 delta against C_{k-1}
+  const int carry = (g->cfg.carry_over && prev) ? 1 : 0;
+  launch_delta_split(st, w->hot.p, (int)w->n_hot, g->R, prev ? prev->slot_map : nullptr, carry, g->tiles32.p,
+                     g->n_delta_dev.p, g->owner_cnt.p, w->slot_map, w->req_ids.p, w->carry_src.p, w->carry_ids.p);
+  w->n_cached = w->n_hot;
+  CU(cudaMemcpyAsync(g->h_small, g->owner_cnt.p, 2 * GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(g->h_small + 2 * GG_MAX_PARTS, g->n_delta_dev.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  w->n_delta = w->n_hot > 0 ? g->h_small[2 * GG_MAX_PARTS] : 0;
+  w->n_carry = w->n_hot - w->n_delta;
+  for (int m = 0; m < GG_MAX_PARTS; ++m) {
+    w->staged[m] = w->n_hot > 0 ? g->h_small[m] : 0;
+    w->bulk[m] = w->n_hot > 0 ? g->h_small[GG_MAX_PARTS + m] : 0;
+  }
+  const double t3 = now_ms();
+  w->ms_select = (float)(t3 - t2);
+
+  // a-6 staging: one bulk transfer per owner into that owner's contiguous slot range
+  w->bulk_copies = 0;
+  w->ms_pack = 0;
+  const int64_t rb = g->rb;
+  CU(cudaEventRecord(g->ev_a, st));
+  if (g->cfg.staging_mode == 0 && w->n_delta > 0) {
+    void* pr = g->h_req;
+    rc = ensure_pinned(&pr, &g->h_req_cap, w->n_delta * (int64_t)sizeof(int32_t));
+    g->h_req = (int32_t*)pr;
+    if (rc != GG_OK) return rc;
+    void* pp = g->h_resp;
+    rc = ensure_pinned(&pp, &g->h_resp_cap, w->n_delta * rb);
+    g->h_resp = (uint8_t*)pp;
+    if (rc != GG_OK) return rc;
+    CU(cudaMemcpyAsync(g->h_req, w->req_ids.p, (size_t)w->n_delta * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaEventRecord(g->ev_a, st));
+    int64_t q0 = 0;
+    for (int m = 0; m < g->R.P; ++m) {
+      const int64_t nm = w->bulk[m];
+      if (nm == 0) continue;
+      // owner service: gather owner m's requested rows into a contiguous response
+      const double p0 = now_ms();
+      const uint8_t* base = g->store.base[m];
+      const int64_t lo = g->R.lo[m], stride = g->store.stride;
+      const int32_t* ids = g->h_req + q0;
+      uint8_t* resp = g->h_resp + q0 * rb;
+      const int64_t chunk = 512;
+      g->pool->parallel_for(ceil_div(nm, chunk), [&](int64_t c) {
+        const int64_t i1 = std::min(nm, (c + 1) * chunk);
+        for (int64_t i = c * chunk; i < i1; ++i)
+          std::memcpy(resp + i * rb, base + (ids[i] - lo) * stride, (size_t)rb);
+      });
+      w->ms_pack += (float)(now_ms() - p0);
+      CU(cudaMemcpyAsync(w->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, st));
+      w->bulk_copies += 1;
+      q0 += nm;
+    }
+  } else if (w->n_delta > 0) {
+    // staging_mode 1: GPU-initiated pull, one launch per owner, no host pack / no ID read-back
+    int64_t q0 = 0;
+    for (int m = 0; m < g->R.P; ++m) {
+      const int64_t nm = w->bulk[m];
+      if (nm == 0) continue;
+      launch_rows_from_store(st, w->req_ids.p + q0, (int)nm, g->store, g->R, w->cache, q0, rb, (int)rb);
+      w->bulk_copies += 1;
+      q0 += nm;
+    }
+  }
+  CU(cudaEventRecord(g->ev_b, st));
+  // carried rows: D2D out of the previous buffer, after the delta rows
+  if (w->n_carry > 0)
+    launch_rows_from_list(st, w->carry_src.p, (int)w->n_carry, prev->cache, rb, w->cache, w->n_delta, rb, (int)rb);
+  CU(cudaMemsetAsync(w->counters.p, 0, (size_t)Wmax * (2 + GG_MAX_PARTS) * sizeof(int32_t), st));
+  CU(cudaEventRecord(w->ready, st));
+  CU(cudaEventSynchronize(w->ready));
+  float ms = 0;
+  cudaEventElapsedTime(&ms, g->ev_a, g->ev_b);
+  w->ms_h2d = ms;
+  cudaEventElapsedTime(&ms, g->ev_b, w->ready);
+  w->ms_carry = ms;
+  CU(cudaGetLastError());
+  g->have_prev = true;
+  g->prev_slot = w->slot;
+  w->ms_total = (float)(now_ms() - t0);
+  return GG_OK;
+}
+
+static void worker_main(gg_graph* g) {
+  cudaSetDevice(g->device);
+  for (;;) {
+    Window* w;
+    {
+      std::unique_lock<std::mutex> l(g->mu);
+      g->cv_job.wait(l, [&] { return g->stop || !g->jobs.empty(); });
+      if (g->jobs.empty()) return;
+      w = g->jobs.front();
+      g->jobs.pop_front();
+    }
+    gg_status rc = stage_window(g, w);
+    {
+      std::lock_guard<std::mutex> l(g->mu);
+      w->status = rc;
+      if (rc != GG_OK) w->error = t_err;
+      w->enqueued = true;
+    }
+    g->cv_done.notify_all();
+  }
+}
+
+}  // namespace gg
+
+// =================================== C ABI ====================================================
+extern "C" {
+
+const char* gg_last_error(void) { return t_err.c_str(); }
+const char* gg_version(void) { return "greengnn-b200 0.1 (sm_100a)"; }
+
+uint64_t gg_key(uint64_t seed, uint64_t batch, uint64_t layer, uint64_t dst, uint64_t edge_pos) {
+  return key_edge(key_hdst(key_prefix(seed, batch, layer), dst), edge_pos);
+}
+
+static bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+static bool is_pinned_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return a.type == cudaMemoryTypeHost;
+}
+
+gg_status gg_graph_destroy(gg_graph* g) {
+  if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
+  if (g->worker.joinable()) {
+    {
+      std::lock_guard<std::mutex> l(g->mu);
+      g->stop = true;
+    }
+    g->cv_job.notify_all();
+    g->worker.join();
+  }
+  cudaSetDevice(g->device);
+  cudaDeviceSynchronize();
+  delete g->pool;
+  for (int s = 0; s < 2; ++s) {
+    Window& w = g->win[s];
+    w.nodes.release(); w.n_front_dev.release(); w.uniq.release(); w.cnt.release();
+    w.req_ids.release(); w.carry_src.release(); w.carry_ids.release(); w.counters.release();
+    w.hot.release();
+    for (int h = 0; h < GG_MAX_LAYERS; ++h) {
+      w.hop[h].blk_indptr.release(); w.hop[h].src_global.release();
+      w.hop[h].src_local.release(); w.hop[h].edge_off_dev.release();
+    }
+    if (w.cache) cudaFree(w.cache);
+    if (w.slot_map) cudaFree(w.slot_map);
+    if (w.ready) cudaEventDestroy(w.ready);
+    if (w.gather_done) cudaEventDestroy(w.gather_done);
+  }
+  g->seen.release(); g->newbits.release(); g->cnt8.release(); g->wprefix.release();
+  g->seed_perm.release(); g->tiles32.release(); g->totals.release(); g->stats.release();
+  g->hist.release(); g->owner_cnt.release(); g->n_delta_dev.release(); g->err_flag.release();
+  g->seeds_dev.release(); g->tiles64.release(); g->total64.release(); g->key_prefix.release();
+  g->cnt_tmp.release(); g->miss_tmp_pos.release(); g->miss_tmp_id.release(); g->tile_miss.release();
+  g->miss_pos.release(); g->miss_id.release(); g->n_miss.release();
+  if (g->h_small) cudaFreeHost(g->h_small);
+  if (g->h_req) cudaFreeHost(g->h_req);
+  if (g->h_resp) cudaFreeHost(g->h_resp);
+  if (g->h_seeds) cudaFreeHost(g->h_seeds);
+  if (g->h_kp) cudaFreeHost(g->h_kp);
+  if (g->ev_a) cudaEventDestroy(g->ev_a);
+  if (g->ev_b) cudaEventDestroy(g->ev_b);
+  if (g->side) cudaStreamDestroy(g->side);
+  delete g;
+  return GG_OK;
+}
+
+gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const gg_feature_store* store,
+                          const gg_config* cfg, gg_graph** out) {
+  if (!csr || !owners || !store || !cfg || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
+  *out = nullptr;
+  if (csr->num_nodes < 1 || csr->num_nodes >= (1ll << 31) || csr->num_edges < 0)
+    return fail(GG_ERR_INVALID_ARG, "num_nodes must be in [1, 2^31), num_edges >= 0");
+  if (!csr->indptr || (!csr->indices && csr->num_edges > 0)) return fail(GG_ERR_INVALID_ARG, "null CSR array");
+  const int P = owners->num_parts;
+  if (P < 1 || P > GG_MAX_PARTS) return fail(GG_ERR_INVALID_ARG, "num_parts must be in [1, %d]", GG_MAX_PARTS);
+  if (owners->local_part < 0 || owners->local_part >= P) return fail(GG_ERR_INVALID_ARG, "local_part out of range");
+  if (!owners->part_offsets) return fail(GG_ERR_INVALID_ARG, "null part_offsets");
+  if (owners->part_offsets[0] != 0 || owners->part_offsets[P] != csr->num_nodes)
+    return fail(GG_ERR_INVALID_ARG, "part_offsets must start at 0 and end at num_nodes");
+  for (int m = 0; m < P; ++m)
+    if (owners->part_offsets[m] > owners->part_offsets[m + 1])
+      return fail(GG_ERR_INVALID_ARG, "part_offsets must be non-decreasing");
+  const int esz = store->dtype == GG_F32 ? 4 : (store->dtype == GG_BF16 ? 2 : 0);
+  if (!esz) return fail(GG_ERR_INVALID_ARG, "unknown dtype");
+  if (store->dim < 1 || !store->part_base) return fail(GG_ERR_INVALID_ARG, "bad feature store");
+  const int64_t rb = (int64_t)store->dim * esz;
+  if (rb % 4) return fail(GG_ERR_INVALID_ARG, "row bytes must be a multiple of 4");
+  if (store->row_stride_bytes < rb || store->row_stride_bytes % 4)
+    return fail(GG_ERR_INVALID_ARG, "row_stride_bytes must be >= row bytes and a multiple of 4");
+  if (cfg->max_layers < 1 || cfg->max_layers > GG_MAX_LAYERS) return fail(GG_ERR_INVALID_ARG, "max_layers out of range");
+  if (cfg->max_window < 1 || cfg->max_window > GG_MAX_WINDOW) return fail(GG_ERR_INVALID_ARG, "max_window out of range");
+  if (cfg->max_batch < 1) return fail(GG_ERR_INVALID_ARG, "max_batch must be >= 1");
+  if (cfg->staging_mode != 0 && cfg->staging_mode != 1) return fail(GG_ERR_INVALID_ARG, "staging_mode must be 0 or 1");
+  if (!is_device_ptr(csr->indptr) || (csr->num_edges > 0 && !is_device_ptr(csr->indices)))
+    return fail(GG_ERR_INVALID_ARG, "indptr / indices must be device memory");
+  for (int m = 0; m < P; ++m) {
+    const bool empty = owners->part_offsets[m] == owners->part_offsets[m + 1];
+    if (empty) continue;
+    if (!store->part_base[m]) return fail(GG_ERR_INVALID_ARG, "part_base[%d] is null", m);
+    if (m == owners->local_part) {
+      if (!is_device_ptr(store->part_base[m])) return fail(GG_ERR_INVALID_ARG, "local part's store must be device memory");
+    } else if (!is_pinned_ptr(store->part_base[m]) && !is_device_ptr(store->part_base[m])) {
+      return fail(GG_ERR_INVALID_ARG, "part_base[%d] must be pinned host memory (page-locked, CUDA-registered)", m);
+    }
+  }
+
+  gg_graph* g = new gg_graph();
+  g->N = csr->num_nodes; g->nnz = csr->num_edges; g->indptr = csr->indptr; g->indices = csr->indices;
+  g->R.P = P; g->R.local = owners->local_part;
+  for (int m = 0; m <= P; ++m) g->R.lo[m] = owners->part_offsets[m];
+  for (int m = P + 1; m <= GG_MAX_PARTS; ++m) g->R.lo[m] = g->N;
+  for (int m = 0; m < GG_MAX_PARTS; ++m) g->store.base[m] = m < P ? (const uint8_t*)store->part_base[m] : nullptr;
+  g->store.stride = store->row_stride_bytes;
+  g->dim = store->dim; g->rb = (int)rb; g->dtype = store->dtype; g->cfg = *cfg;
+  cudaGetDevice(&g->device);
+  const int64_t n_remote_nodes = g->N - (g->R.lo[g->R.local + 1] - g->R.lo[g->R.local]);
+  g->cache_rows = cfg->max_cache_rows > 0 ? std::min<int64_t>(cfg->max_cache_rows, n_remote_nodes) : n_remote_nodes;
+  g->n_hot_eff = cfg->n_hot < 0 ? g->cache_rows : std::min<int64_t>(cfg->n_hot, g->cache_rows);
+
+  gg_status rc = GG_OK;
+  auto bad = [&](gg_status s) { gg_graph_destroy(g); return s; };
+#define CUC(call)                                                                              \
+  do {                                                                                         \
+    cudaError_t e_ = (call);                                                                   \
+    if (e_ != cudaSuccess) {                                                                   \
+      rc = fail(e_ == cudaErrorMemoryAllocation ? GG_ERR_OOM : GG_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+      cudaGetLastError();                                                                      \
+      return bad(rc);                                                                          \
+    }                                                                                          \
+  } while (0)
+  const int Wmax = cfg->max_window, Lmax = cfg->max_layers;
+  g->n_gen = Lmax + 1;
+  g->F.word_pitch = ceil_div(ceil_div(g->N, 32), kWordTile) * kWordTile;
+  g->F.gen_pitch = (int64_t)Wmax * g->F.word_pitch;
+  g->F.n_wtiles = (int)(g->F.word_pitch / kWordTile);
+  g->F.perm_pitch = cfg->max_batch;
+  CUC(g->seen.ensure(g->F.gen_pitch));
+  CUC(g->newbits.ensure(g->F.gen_pitch * g->n_gen));
+  CUC(g->wprefix.ensure(g->F.gen_pitch * g->n_gen));
+  CUC(g->seed_perm.ensure((int64_t)Wmax * cfg->max_batch));
+  g->F.seen = g->seen.p; g->F.newbits = g->newbits.p; g->F.wprefix = g->wprefix.p; g->F.seed_perm = g->seed_perm.p;
+  g->cnt_words = ceil_div(ceil_div(g->N, 4), kWordTile) * kWordTile;
+  CUC(g->cnt8.ensure(g->cnt_words));
+  CUC(cudaMemset(g->seen.p, 0, (size_t)g->F.gen_pitch * 4));
+  CUC(cudaMemset(g->newbits.p, 0, (size_t)g->F.gen_pitch * g->n_gen * 4));
+  CUC(cudaMemset(g->cnt8.p, 0, (size_t)g->cnt_words * 4));
+  CUC(g->totals.ensure(2 * Wmax + 2));
+  CUC(g->stats.ensure(4)); CUC(g->hist.ensure(256)); CUC(g->owner_cnt.ensure(2 * GG_MAX_PARTS));
+  CUC(g->n_delta_dev.ensure(1)); CUC(g->err_flag.ensure(1)); CUC(g->total64.ensure(1)); CUC(g->n_miss.ensure(1));
+  CUC(cudaMemset(g->n_miss.p, 0, 4));
+  CUC(g->seeds_dev.ensure((int64_t)Wmax * cfg->max_batch));
+  CUC(g->key_prefix.ensure((int64_t)GG_MAX_LAYERS * Wmax));
+  CUC(cudaHostAlloc((void**)&g->h_small, 4096 * sizeof(int32_t), cudaHostAllocDefault));
+  CUC(cudaHostAlloc((void**)&g->h_seeds, (size_t)Wmax * cfg->max_batch * sizeof(int32_t), cudaHostAllocDefault));
+  CUC(cudaHostAlloc((void**)&g->h_kp, (size_t)GG_MAX_LAYERS * Wmax * sizeof(uint64_t), cudaHostAllocDefault));
+  CUC(cudaStreamCreateWithFlags(&g->side, cudaStreamNonBlocking));
+  CUC(cudaEventCreate(&g->ev_a)); CUC(cudaEventCreate(&g->ev_b));
+  for (int s = 0; s < 2; ++s) {
+    Window& w = g->win[s];
+    w.slot = s;
+    CUC(cudaMalloc((void**)&w.cache, (size_t)std::max<int64_t>(g->cache_rows, 1) * rb));
+    CUC(cudaMalloc((void**)&w.slot_map, (size_t)g->N * sizeof(int32_t)));
+    launch_fill_i32(0, w.slot_map, g->N, -1);
+    CUC(cudaEventCreateWithFlags(&w.ready, cudaEventDefault));
+    CUC(cudaEventCreateWithFlags(&w.gather_done, cudaEventDisableTiming));
+  }
+  CUC(cudaDeviceSynchronize());
+#undef CUC
+  int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(1u, std::thread::hardware_concurrency()));
+  g->pool = new Pool(nt > 1 ? nt : 0);
+  g->worker = std::thread(worker_main, g);
+  *out = g;
+  return GG_OK;
+}
+
+}  // extern "C"
+
+namespace gg {
+static Window* find_window(gg_graph* g, int64_t id) {
+  for (int s = 0; s < 2; ++s)
+    if (g->win[s].live && g->win[s].id == id) return &g->win[s];
+  return nullptr;
+}
+// Alg. 1 l.5: block until the prefetcher is done with this window
+static gg_status wait_enqueued(gg_graph* g, Window* w) {
+  const double t0 = now_ms();
+  std::unique_lock<std::mutex> l(g->mu);
+  if (!w->enqueued) {
+    g->cv_done.wait(l, [&] { return w->enqueued; });
+    w->ms_wait += (float)(now_ms() - t0);
+  }
+  if (w->status != GG_OK) {
+    t_err = w->error;
+    return w->status;
+  }
+  return GG_OK;
+}
+static void fill_batch_out(Window* w, int b, gg_batch_out* out, gg_graph* g) {
+  out->num_layers = w->L;
+  for (int h = 0; h < w->L; ++h) {
+    Hop& H = w->hop[h];
+    gg_block& k = out->blocks[h];
+    k.n_dst = w->n_front[h][b];
+    k.n_src = w->n_front[h + 1][b];
+    k.n_edge = H.edge_off[b + 1] - H.edge_off[b];
+    k.indptr = H.blk_indptr.p + H.dst_off[b] + b;
+    k.src_local = H.src_local.p + H.edge_off[b];
+    k.src_global = H.src_global.p + H.edge_off[b];
+  }
+  out->n_input = w->n_front[w->L][b];
+  out->input_nodes = w->nodes.p + (int64_t)b * w->node_pitch;
+  out->miss_pos = g->miss_pos.p;
+  out->miss_id = g->miss_id.p;
+  out->n_miss = g->n_miss.p;
+}
+}  // namespace gg
+
+extern "C" {
+
+gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_index, const int32_t* seeds,
+                          const int64_t* batch_offsets, int32_t W, const int32_t* fanouts, int32_t num_layers) {
+  if (!g || !seeds || !batch_offsets || !fanouts) return fail(GG_ERR_INVALID_ARG, "null argument");
+  if (W < 1 || W > g->cfg.max_window) return fail(GG_ERR_INVALID_ARG, "W = %d outside [1, max_window = %d]", W, g->cfg.max_window);
+  if (num_layers < 1 || num_layers > g->cfg.max_layers)
+    return fail(GG_ERR_INVALID_ARG, "num_layers = %d outside [1, max_layers = %d]", num_layers, g->cfg.max_layers);
+  for (int h = 0; h < num_layers; ++h)
+    if (fanouts[h] < 1 || fanouts[h] > GG_MAX_FANOUT)
+      return fail(GG_ERR_INVALID_ARG, "fanouts[%d] = %d outside [1, %d]", h, fanouts[h], GG_MAX_FANOUT);
+  if (batch_offsets[0] != 0) return fail(GG_ERR_INVALID_ARG, "batch_offsets[0] must be 0");
+  for (int b = 0; b < W; ++b) {
+    const int64_t n = batch_offsets[b + 1] - batch_offsets[b];
+    if (n < 1 || n > g->cfg.max_batch)
+      return fail(GG_ERR_INVALID_ARG, "batch %d has %lld seeds; must be in [1, max_batch = %d]", b, (long long)n, g->cfg.max_batch);
+  }
+  const int64_t S = batch_offsets[W];
+  for (int64_t i = 0; i < S; ++i)
+    if (seeds[i] < 0 || seeds[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "seed %lld = %d outside [0, N)", (long long)i, seeds[i]);
+  if (find_window(g, window_id)) return fail(GG_ERR_STATE, "window %lld is already live", (long long)window_id);
+  Window* w = &g->win[g->stage_counter & 1];
+  if (w->live) return fail(GG_ERR_STATE, "two windows are live; release window %lld first", (long long)w->id);
+  if (g->win[0].live && g->win[1].live) return fail(GG_ERR_STATE, "two windows are live");
+  w->id = window_id; w->live = true; w->W = W; w->L = num_layers; w->first_batch = first_batch_index;
+  for (int h = 0; h < num_layers; ++h) w->fanouts[h] = fanouts[h];
+  w->seeds.assign(seeds, seeds + S);
+  w->boff.assign(batch_offsets, batch_offsets + W + 1);
+  w->ms_wait = 0;
+  {
+    std::lock_guard<std::mutex> l(g->mu);
+    w->enqueued = false; w->status = GG_OK; w->error.clear();
+    g->jobs.push_back(w);
+  }
+  g->stage_counter += 1;
+  g->cv_job.notify_one();
+  return GG_OK;
+}
+
+gg_status gg_batch_info(gg_graph* g, int64_t window_id, int32_t b, gg_batch_out* out) {
+  if (!g || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
+  Window* w = find_window(g, window_id);
+  if (!w) return fail(GG_ERR_STATE, "window %lld is not live (never staged or already released)", (long long)window_id);
+  if (b < 0 || b >= w->W) return fail(GG_ERR_INVALID_ARG, "batch_in_window = %d outside [0, %d)", b, w->W);
+  gg_status rc = wait_enqueued(g, w);
+  if (rc != GG_OK) return rc;
+  fill_batch_out(w, b, out, g);
+  return GG_OK;
+}
+
+gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_out* out, void* cuda_stream) {
+  if (!g || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
+  Window* w = find_window(g, window_id);
+  if (!w) return fail(GG_ERR_STATE, "window %lld is not live (never staged or already released)", (long long)window_id);
+  if (b < 0 || b >= w->W) return fail(GG_ERR_INVALID_ARG, "batch_in_window = %d outside [0, %d)", b, w->W);
+  if (!out->features || ((uintptr_t)out->features & 3)) return fail(GG_ERR_INVALID_ARG, "features must be a 4-byte aligned device buffer");
+  gg_status rc = wait_enqueued(g, w);
+  if (rc != GG_OK) return rc;
+  const int n = w->n_front[w->L][b];
+  if (out->features_capacity_rows < n)
+    return fail(GG_ERR_CAPACITY, "features_capacity_rows = %lld < n_input = %d", (long long)out->features_capacity_rows, n);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CU(cudaStreamWaitEvent(st, w->ready, 0));
+  GatherLaunch G;
+  G.nodes = w->nodes.p + (int64_t)b * w->node_pitch; G.n = n; G.slot_of = w->slot_map;
+  G.local_base = g->store.base[g->R.local]; G.local_stride = g->store.stride;
+  G.cache_base = w->cache; G.cache_stride = g->rb;
+  G.out = (uint8_t*)out->features; G.rb = g->rb; G.R = g->R; G.store = g->store;
+  G.may_miss = w->may_miss;
+  G.miss_tmp_pos = g->miss_tmp_pos.p; G.miss_tmp_id = g->miss_tmp_id.p; G.tile_miss = g->tile_miss.p;
+  G.miss_pos = g->miss_pos.p; G.miss_id = g->miss_id.p; G.n_miss = g->n_miss.p;
+  G.counters = w->counters.p + (int64_t)b * (2 + GG_MAX_PARTS);
+  launch_gather(st, G);
+  CU(cudaEventRecord(w->gather_done, st));
+  w->gather_recorded = true;
+  CU(cudaGetLastError());
+  fill_batch_out(w, b, out, g);
+  return GG_OK;
+}
+
+gg_status gg_window_release(gg_graph* g, int64_t window_id) {
+  if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
+  Window* w = find_window(g, window_id);
+  if (!w) return fail(GG_ERR_STATE, "window %lld is not live", (long long)window_id);
+  wait_enqueued(g, w);  // the prefetcher must be done touching the slot before it can be re-staged
+  w->live = false;
+  return GG_OK;
+}
+
+gg_status gg_trace(gg_graph* g, int64_t window_id, gg_window_trace* out) {
+  if (!g || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
+  Window* w = find_window(g, window_id);
+  if (!w) return fail(GG_ERR_STATE, "window %lld is not live", (long long)window_id);
+  gg_status rc = wait_enqueued(g, w);
+  if (rc != GG_OK) return rc;
+  CU(cudaEventSynchronize(w->ready));
+  if (w->gather_recorded) CU(cudaEventSynchronize(w->gather_done));
+  out->W = w->W; out->num_parts = g->R.P;
+  out->n_access = w->n_access; out->n_unique = w->n_unique; out->n_unique_remote = w->n_remote;
+  out->n_hot = w->n_hot; out->carried_rows = w->n_carry; out->bulk_copies = w->bulk_copies;
+  for (int m = 0; m < GG_MAX_PARTS; ++m) {
+    out->staged_rows[m] = w->staged[m];
+    out->bulk_rows[m] = w->bulk[m];
+    out->bulk_bytes[m] = w->bulk[m] * g->rb;
+  }
+  std::vector<int32_t> c((size_t)w->W * (2 + GG_MAX_PARTS));
+  CU(cudaMemcpy(c.data(), w->counters.p, c.size() * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  for (int b = 0; b < w->W; ++b) {
+    const int32_t* r = c.data() + (size_t)b * (2 + GG_MAX_PARTS);
+    if (out->n_input) out->n_input[b] = w->n_front[w->L][b];
+    if (out->hit_local) out->hit_local[b] = r[0];
+    if (out->hit_cache) out->hit_cache[b] = r[1];
+    if (out->miss) for (int m = 0; m < g->R.P; ++m) out->miss[b * g->R.P + m] = r[2 + m];
+  }
+  out->ms_sample = w->ms_sample; out->ms_unique = w->ms_unique; out->ms_select = w->ms_select;
+  out->ms_pack_host = w->ms_pack; out->ms_h2d = w->ms_h2d; out->ms_carry = w->ms_carry;
+  out->ms_stage_total = w->ms_total; out->ms_boundary_wait = w->ms_wait;
+  return GG_OK;
+}
+
+gg_status gg_window_export(gg_graph* g, int64_t window_id, int32_t what, int32_t* out, int64_t capacity, int64_t* n_out) {
+  if (!g || !n_out || (!out && capacity > 0)) return fail(GG_ERR_INVALID_ARG, "null argument");
+  Window* w = find_window(g, window_id);
+  if (!w) return fail(GG_ERR_STATE, "window %lld is not live", (long long)window_id);
+  gg_status rc = wait_enqueued(g, w);
+  if (rc != GG_OK) return rc;
+  CU(cudaEventSynchronize(w->ready));
+  const int32_t* src = nullptr;
+  int64_t n = 0;
+  switch (what) {
+    case 0: src = w->uniq.p; n = w->n_unique; break;
+    case 1: src = w->cnt.p; n = w->n_unique; break;
+    case 2: src = w->hot.p; n = w->n_hot; break;
+    case 3: src = w->req_ids.p; n = w->n_delta; break;
+    case 4: src = w->carry_ids.p; n = w->n_carry; break;
+    default: return fail(GG_ERR_INVALID_ARG, "what = %d", what);
+  }
+  *n_out = n;
+  if (capacity < n) return fail(GG_ERR_CAPACITY, "capacity %lld < %lld", (long long)capacity, (long long)n);
+  if (n > 0) CU(cudaMemcpy(out, src, (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  return GG_OK;
+}
+
+gg_status gg_cache_read(gg_graph* g, int64_t window_id, const int32_t* ids, int64_t n, void* out) {
+  if (!g || !ids || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
+  Window* w = find_window(g, window_id);
+  if (!w) return fail(GG_ERR_STATE, "window %lld is not live", (long long)window_id);
+  gg_status rc = wait_enqueued(g, w);
+  if (rc != GG_OK) return rc;
+  CU(cudaEventSynchronize(w->ready));
+  for (int64_t i = 0; i < n; ++i) {
+    if (ids[i] < 0 || ids[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "id out of range");
+    int32_t s = -1;
+    CU(cudaMemcpy(&s, w->slot_map + ids[i], sizeof(int32_t), cudaMemcpyDeviceToHost));
+    if (s < 0) return fail(GG_ERR_INVALID_ARG, "id %d is not cached in window %lld", ids[i], (long long)window_id);
+    CU(cudaMemcpy((uint8_t*)out + i * g->rb, w->cache + (int64_t)s * g->rb, (size_t)g->rb, cudaMemcpyDeviceToHost));
+  }
+  return GG_OK;
+}
+
+gg_status gg_cache_reset(gg_graph* g) {
+  if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
+  if (g->win[0].live || g->win[1].live) return fail(GG_ERR_STATE, "release every window before gg_cache_reset");
+  CU(cudaDeviceSynchronize());
+  for (int s = 0; s < 2; ++s) {
+    Window& w = g->win[s];
+    launch_slots_clear(g->side, w.hot.p, (int)w.n_cached, w.slot_map);
+    w.n_cached = 0;
+  }
+  CU(cudaStreamSynchronize(g->side));
+  g->have_prev = false;
+  return GG_OK;
+}
+
+}  // extern "C"

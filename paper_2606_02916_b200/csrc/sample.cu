@@ -1,0 +1,232 @@
+// a-1: neighbor sampling for one hop of a whole window (all W batches in one launch set).
+//
+// Keep rule (include/greengnn.h; readings S3-S5): for destination v with CSR row of
+// `deg` entries, keep every position if deg <= f, else the f positions j with the smallest
+// (key(j), j), key(j) = fmix(h_dst + (j+1)*gamma); kept neighbors are emitted in ascending
+// edge position.  The key depends on (seed, batch, layer, dst, j) only -- never on the
+// neighbor id -- so the adjacency row is not read to select; only the <= f chosen entries are.
+//
+// Three launches per hop:
+//   k_sample_count   one thread per destination: c = min(deg, f) -> cnt_tmp, per-tile sums
+//   k_tile_scan      one CTA per batch: exclusive scan of that batch's tile sums, batch total
+//   k_sample_select  one CTA per tile of 256 destinations: in-tile scan -> block indptr and
+//                    final output offsets (no atomics => deterministic), then one WARP PER
+//                    DESTINATION (dynamic in-CTA queue) does the keyed selection.
+#include "common.cuh"
+#include "kernels.h"
+
+namespace gg {
+
+constexpr int kTile = 256;      // destinations per CTA tile
+constexpr int kCand = 256;      // candidate buffer per warp
+constexpr int kWarps = 8;
+
+__global__ void __launch_bounds__(kTile)
+k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ nodes,
+               int64_t node_pitch, BatchOffsets n_dst, int fanout, int max_tiles,
+               uint8_t* __restrict__ cnt_tmp, int64_t cnt_pitch, int32_t* __restrict__ tile_sums) {
+  __shared__ int32_t sm[33];
+  const int b = blockIdx.y, t = blockIdx.x;
+  const int nd = n_dst.v[b];
+  if (t * kTile >= nd) return;
+  const int i = t * kTile + threadIdx.x;
+  int c = 0;
+  if (i < nd) {
+    const int32_t v = nodes[b * node_pitch + i];
+    const int64_t r0 = __ldg(indptr + v), r1 = __ldg(indptr + v + 1);
+    const int64_t deg = r1 - r0;
+    c = deg < fanout ? (int)deg : fanout;
+    cnt_tmp[b * cnt_pitch + i] = (uint8_t)c;
+  }
+  int32_t total;
+  block_exclusive_scan<int32_t>(c, sm, &total);
+  if (threadIdx.x == 0) tile_sums[b * max_tiles + t] = total;
+}
+
+// One CTA per batch (row): in-place exclusive scan of row[0..n_tiles[b]) ; totals[b] = sum.
+__global__ void __launch_bounds__(1024)
+k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, int items_per_tile,
+            int32_t* __restrict__ totals) {
+  __shared__ int32_t sm[33];
+  __shared__ int32_t carry_s;
+  const int b = blockIdx.x;
+  const int n = (n_items.v[b] + items_per_tile - 1) / items_per_tile;
+  int32_t* row = tiles + (int64_t)b * row_pitch;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < n; base += blockDim.x) {
+    const int i = base + threadIdx.x;
+    int32_t v = i < n ? row[i] : 0, tot;
+    int32_t ex = block_exclusive_scan<int32_t>(v, sm, &tot);
+    const int32_t carry = carry_s;
+    if (i < n) row[i] = carry + ex;
+    __syncthreads();
+    if (threadIdx.x == 0) carry_s = carry + tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) totals[b] = carry_s;
+}
+
+// Exact top-f of `deg` keyed positions by one warp.  Writes the kept positions' neighbor ids,
+// ascending in position, to out[0..f).
+__device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int64_t deg, int f,
+                                            uint64_t hdst, uint64_t* s_key, int32_t* s_pos,
+                                            int32_t* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  // slack so that a Binomial(deg, (f+slack)/deg) count falls below f with prob < ~1e-6
+  const int want = f + 8 + (int)(5.0f * sqrtf((float)f));
+  int cnt;
+  if (deg <= (want > 64 ? want : 64)) {
+    // small row: every position is a candidate
+    cnt = (int)deg;
+    for (int j = lane; j < cnt; j += 32) {
+      s_key[j] = key_edge(hdst, (uint64_t)j);
+      s_pos[j] = j;
+    }
+  } else {
+    // threshold guess: keys are uniform, so the f-th smallest is near f/deg * 2^64.  The
+    // threshold only prunes; the exact rank below decides, so its rounding is immaterial.
+    uint64_t T = (uint64_t)((double)want / (double)deg * 18446744073709551616.0);
+    uint64_t lo = 0, hi = ~0ull;  // count(lo) < f known; count(hi) > kCand known (or hi = max)
+    bool have_hi = false;
+    for (;;) {
+      cnt = 0;
+      for (int64_t j0 = 0; j0 < deg; j0 += 32) {
+        const int64_t j = j0 + lane;
+        uint64_t k = 0;
+        bool p = false;
+        if (j < deg) {
+          k = key_edge(hdst, (uint64_t)j);
+          p = k <= T;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, p);
+        if (p) {
+          const int q = cnt + __popc(m & lanemask_lt());
+          if (q < kCand) {
+            s_key[q] = k;
+            s_pos[q] = (int32_t)j;
+          }
+        }
+        cnt += __popc(m);
+      }
+      if (cnt >= f && cnt <= kCand) break;
+      if (cnt < f) {
+        lo = T;
+        T = have_hi ? lo + ((hi - lo) >> 1) : (T > (~0ull >> 1) ? ~0ull : T * 2 + 1);
+      } else {
+        hi = T;
+        have_hi = true;
+        T = lo + ((hi - lo) >> 1);
+      }
+    }
+  }
+  __syncwarp();
+  // exact rank among candidates under (key, position); candidates are in ascending position
+  int emitted = 0;
+  for (int i0 = 0; i0 < cnt; i0 += 32) {
+    const int i = i0 + lane;
+    bool keep = false;
+    int32_t pos = 0;
+    if (i < cnt) {
+      const uint64_t ki = s_key[i];
+      pos = s_pos[i];
+      int rank = 0;
+      for (int c = 0; c < cnt; ++c) {
+        const uint64_t kc = s_key[c];
+        rank += (kc < ki) || (kc == ki && s_pos[c] < pos);
+      }
+      keep = rank < f;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, keep);
+    if (keep) out[emitted + __popc(m & lanemask_lt())] = __ldg(row + pos);
+    emitted += __popc(m);
+  }
+  __syncwarp();
+}
+
+__global__ void __launch_bounds__(kTile)
+k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
+                const int32_t* __restrict__ nodes, int64_t node_pitch, BatchOffsets n_dst,
+                BatchOffsets dst_off, int W, int fanout, int max_tiles,
+                const uint64_t* __restrict__ key_prefix_b, const uint8_t* __restrict__ cnt_tmp,
+                int64_t cnt_pitch, const int32_t* __restrict__ tile_sums,
+                const int32_t* __restrict__ totals, int32_t* __restrict__ blk_indptr,
+                int32_t* __restrict__ edge_off_out, int32_t* __restrict__ src_global) {
+  __shared__ int32_t sm[33];
+  __shared__ int32_t s_off[kTile + 1];
+  __shared__ int32_t s_edge_base, s_next;
+  __shared__ uint64_t s_key[kWarps][kCand];
+  __shared__ int32_t s_pos[kWarps][kCand];
+  const int b = blockIdx.y, t = blockIdx.x;
+  const int nd = n_dst.v[b];
+  if (t * kTile >= nd) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  // edge offset of this batch = sum of the totals of the batches before it
+  if (wid == 0) {
+    int32_t s = 0;
+    for (int k = lane; k < b; k += 32) s += totals[k];
+#pragma unroll
+    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) {
+      s_edge_base = s;
+      s_next = kWarps;
+      if (t == 0) {
+        edge_off_out[b] = s;
+        if (b == W - 1) edge_off_out[W] = s + totals[b];
+      }
+    }
+  }
+  const int i = t * kTile + threadIdx.x;
+  const int c = i < nd ? cnt_tmp[b * cnt_pitch + i] : 0;
+  int32_t tot;
+  const int32_t ex = block_exclusive_scan<int32_t>(c, sm, &tot);
+  const int32_t tile_base = tile_sums[b * max_tiles + t];
+  s_off[threadIdx.x] = tile_base + ex;
+  // block indptr (0-based inside the batch's block); batch b's row starts at dst_off[b] + b
+  int32_t* ip = blk_indptr + dst_off.v[b] + b;
+  if (i < nd) ip[i] = tile_base + ex;
+  if (i == nd - 1) ip[nd] = tile_base + ex + c;
+  __syncthreads();
+  const int n_here = min(kTile, nd - t * kTile);
+  const uint64_t prefix = key_prefix_b[b];
+  int32_t* out_b = src_global + s_edge_base;
+  // warp per destination, dynamic queue inside the tile (rows differ in cost by 1000x)
+  int d = wid;
+  while (d < n_here) {
+    const int32_t v = nodes[b * node_pitch + t * kTile + d];
+    const int64_t r0 = __ldg(indptr + v), r1 = __ldg(indptr + v + 1);
+    const int64_t deg = r1 - r0;
+    int32_t* out = out_b + s_off[d];
+    if (deg <= fanout) {
+      for (int j = lane; j < deg; j += 32) out[j] = __ldg(indices + r0 + j);
+    } else {
+      warp_select(indices + r0, deg, fanout, key_hdst(prefix, (uint64_t)(uint32_t)v),
+                  s_key[wid], s_pos[wid], out);
+    }
+    if (lane == 0) d = atomicAdd(&s_next, 1);
+    d = __shfl_sync(0xffffffffu, d, 0);
+  }
+}
+
+void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
+                      int items_per_tile, int32_t* totals) {
+  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals);
+}
+
+void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* indices,
+                       const int32_t* nodes, int64_t node_pitch, const BatchOffsets& n_dst,
+                       const BatchOffsets& dst_off, int W, int max_nd, int fanout,
+                       const uint64_t* key_prefix_b, uint8_t* cnt_tmp, int64_t cnt_pitch,
+                       int32_t* tile_sums, int max_tiles, int32_t* totals, int32_t* blk_indptr,
+                       int32_t* edge_off_out, int32_t* src_global) {
+  const int tiles = (max_nd + kTile - 1) / kTile;
+  dim3 grid(tiles, W);
+  k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
+                                         cnt_tmp, cnt_pitch, tile_sums);
+  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals);
+  k_sample_select<<<grid, kTile, 0, st>>>(indptr, indices, nodes, node_pitch, n_dst, dst_off, W,
+                                          fanout, max_tiles, key_prefix_b, cnt_tmp, cnt_pitch,
+                                          tile_sums, totals, blk_indptr, edge_off_out, src_global);
+}
+
+}  // namespace gg

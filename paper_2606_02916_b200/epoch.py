@@ -1,0 +1,58 @@
+"""Epoch driver over the C ABI: the pipelined loop of Algorithm 1.
+
+    stage(0); for k: stage(k+1); gather every batch of window k; release(k)
+
+Pure call sequencing -- all computation happens in libgreengnn.so.  `on_batch` receives every
+gathered batch (used by the parity tests and by the end-to-end bench leg).
+"""
+from __future__ import annotations
+
+from typing import Callable, Dict, List, Optional, Sequence
+
+import numpy as np
+import torch
+
+from .binding import Graph
+
+
+def graph_from_workload(w, n_hot: int = -1, carry_over: int = 1, max_window: int = 32,
+                        staging_mode: int = 0, max_cache_rows: int = 0, host_threads: int = 0,
+                        max_batch: Optional[int] = None) -> Graph:
+    """Builds a gg_graph over an inputs.Workload whose graph and local features are on a CUDA device."""
+    mb = max_batch or max(len(b) for b in w.batches)
+    return Graph(w.indptr, w.indices, w.part_offsets, w.local_part, w.feat_parts, seed=w.seed,
+                 n_hot=n_hot, carry_over=carry_over, max_layers=len(w.fanouts), max_window=max_window,
+                 max_batch=mb, max_cache_rows=max_cache_rows, staging_mode=staging_mode,
+                 host_threads=host_threads)
+
+
+def windows_of(n_batches: int, W: int) -> List[range]:
+    """ceil(B/W) windows of W consecutive batches, the last one partial."""
+    return [range(s, min(n_batches, s + W)) for s in range(0, n_batches, W)]
+
+
+def run_epoch(g: Graph, batches: Sequence[np.ndarray], fanouts: Sequence[int], W: int,
+              features: torch.Tensor, on_batch: Optional[Callable[[int, int, int, Dict], None]] = None,
+              on_window: Optional[Callable[[int, range], None]] = None,
+              stream: Optional[torch.cuda.Stream] = None, first_window_id: int = 0) -> int:
+    """One epoch.  Returns the number of gather launches issued.  `features` is the caller's
+    [capacity_rows, dim] device buffer reused for every batch."""
+    wins = windows_of(len(batches), W)
+    if not wins:
+        return 0
+    wid = first_window_id
+    g.window_stage(wid, wins[0].start, [batches[i] for i in wins[0]], fanouts)
+    n = 0
+    for k, win in enumerate(wins):
+        if k + 1 < len(wins):
+            nxt = wins[k + 1]
+            g.window_stage(wid + k + 1, nxt.start, [batches[i] for i in nxt], fanouts)
+        for j, bi in enumerate(win):
+            r = g.batch_gather(wid + k, j, features, stream)
+            n += 1
+            if on_batch is not None:
+                on_batch(k, j, bi, r)
+        if on_window is not None:
+            on_window(wid + k, win)
+        g.window_release(wid + k)
+    return n

@@ -1,0 +1,127 @@
+"""GPU parity: the CUDA path through the C ABI vs the CPU oracle, bit-exact (all integer /
+byte work; BASELINE.json:north_star).  Sizes span several tiles and ragged tails."""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+from tests import parity_util as pu  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return "cuda:0"
+
+
+def test_library_key_matches_golden_and_oracle(dev):
+    from oracle import ggo
+    from paper_2606_02916_b200 import binding
+    for args in [(0, 0, 0, 0, 0), (42, 3, 1, 1234, 7), (0xDEADBEEF, (1 << 40) + 5, 2, 110999999, 19999)]:
+        assert binding.gg_key(*args) == ggo.key(*args)
+
+
+@pytest.mark.parametrize("n_hot,carry,mode", [(-1, 1, 0), (200, 1, 0), (200, 0, 0), (-1, 1, 1), (0, 1, 0)])
+def test_tiny_one_window(workload, dev, n_hot, carry, mode):
+    w = workload("tiny", dev)
+    s = pu.check_epoch(w, W=4, n_hot=n_hot, carry_over=carry, staging_mode=mode)
+    assert s["batches"] == 4 and s["windows"] == 1
+    if n_hot == -1:
+        assert s["misses"] == 0
+    else:
+        assert s["misses"] > 0
+
+
+@pytest.mark.parametrize("W", [1, 4, 8])
+@pytest.mark.parametrize("n_hot", [-1, 7500])
+def test_small_full_epoch(workload, dev, W, n_hot):
+    w = workload("small", dev)
+    s = pu.check_epoch(w, W=W, n_hot=n_hot)
+    assert s["batches"] == 10 and s["windows"] == -(-10 // W)
+
+
+def test_small_no_carry_and_pull_mode(workload, dev):
+    w = workload("small", dev)
+    pu.check_epoch(w, W=4, n_hot=-1, carry_over=0)
+    pu.check_epoch(w, W=4, n_hot=7500, carry_over=1, staging_mode=1)
+    pu.check_epoch(w, W=3, n_hot=-1, max_cache_rows=5000)      # cache cap spills to the miss path
+
+
+@pytest.mark.parametrize("W", [1, 4])
+def test_products_mini_three_layers(workload, dev, W):
+    w = workload("products_mini", dev)
+    pu.check_epoch(w, W=W, n_hot=-1)
+    pu.check_epoch(w, W=W, n_hot=4500)
+
+
+def test_dense_mini_high_degree_rows_and_8_byte_rows(workload, dev):
+    # avg degree ~100, tail ~2000, fanout 25: exercises threshold selection; rb = 2408 is
+    # only 8-byte aligned
+    w = workload("dense_mini", dev)
+    pu.check_epoch(w, W=4, n_hot=-1)
+    pu.check_epoch(w, W=1, n_hot=600)
+
+
+def test_large_mini_directed_bf16(workload, dev):
+    w = workload("large_mini", dev)
+    pu.check_epoch(w, W=4, n_hot=-1)
+    pu.check_epoch(w, W=4, n_hot=11250, staging_mode=1)
+
+
+def test_determinism_two_epochs_identical(workload, dev):
+    from paper_2606_02916_b200 import epoch as ep
+    w = workload("small", dev)
+    g = ep.graph_from_workload(w, max_window=4)
+    feats = torch.empty(w.num_nodes, w.dim, dtype=w.dtype, device=dev)
+    runs = []
+    for e in range(2):
+        got = []
+        ep.run_epoch(g, w.batches, w.fanouts, 4, feats,
+                     on_batch=lambda k, j, bi, r: got.append((r["input_nodes"].cpu().numpy().copy(),
+                                                              r["blocks"][-1]["src_local"].cpu().numpy().copy(),
+                                                              r["features"].cpu().clone())),
+                     first_window_id=100 * e)
+        runs.append(got)
+        g.cache_reset()
+    for a, b in zip(*runs):
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and torch.equal(a[2], b[2])
+    g.close()
+
+
+def test_error_codes(workload, dev):
+    from paper_2606_02916_b200 import binding, epoch as ep
+    w = workload("tiny", dev)
+    g = ep.graph_from_workload(w, max_window=4)
+    feats = torch.empty(8, w.dim, dtype=w.dtype, device=dev)
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.batch_info(5, 0)
+    assert e.value.status == binding.GG_ERR_STATE
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.window_stage(0, 0, w.batches[:4] + w.batches[:1], w.fanouts)      # W > max_window
+    assert e.value.status == binding.GG_ERR_INVALID_ARG
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.window_stage(0, 0, [np.array([w.num_nodes], np.int32)], w.fanouts)  # seed out of range
+    assert e.value.status == binding.GG_ERR_INVALID_ARG
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.window_stage(0, 0, w.batches[:1], [0, 5])                          # fanout <= 0
+    assert e.value.status == binding.GG_ERR_INVALID_ARG
+    g.window_stage(0, 0, w.batches[:2], w.fanouts)
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.batch_gather(0, 0, feats)                                          # buffer too small
+    assert e.value.status == binding.GG_ERR_CAPACITY
+    g.window_stage(1, 2, w.batches[2:4], w.fanouts)
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.window_stage(2, 4, w.batches[:1], w.fanouts)                       # third live window
+    assert e.value.status == binding.GG_ERR_STATE
+    g.window_release(0)
+    g.window_release(1)
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.window_release(1)
+    assert e.value.status == binding.GG_ERR_STATE
+    g.close()
+    # host memory where device memory is required
+    with pytest.raises(binding.GreenGNNError) as e:
+        binding.Graph(w.indptr.cpu(), w.indices.cpu(), w.part_offsets, 0, w.feat_parts, seed=1)
+    assert e.value.status == binding.GG_ERR_INVALID_ARG
