@@ -1,0 +1,387 @@
+#!/usr/bin/env python
+"""bench.py -- mini-batches/s of the whole hot path (sample + stage + gather) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config products] [--batch 1024] [--window 16] [--n-hot -1]
+
+A STEP is one epoch of the named workload: ceil(B/W) windows, every mini-batch sampled,
+staged and gathered (all SURVEY.md Sec. 8(a) rows), cache reset before each epoch.  Prints
+ONE JSON line (DESIGN.md "Measurement" explains every key).
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+
+METRIC = "mini-batches/s (sample+stage+gather), one epoch per step"
+UNIT = "mini-batches/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="products")
+    ap.add_argument("--batch", type=int, default=1024)
+    ap.add_argument("--window", type=int, default=16)
+    ap.add_argument("--n-hot", type=int, default=-1)
+    ap.add_argument("--staging-mode", type=int, default=0)
+    ap.add_argument("--no-sweep", action="store_true", help="skip the W sweep")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-sample-batches", type=int, default=4)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """dram read+write bytes per k_gather launch from the committed ncu --set full summary."""
+    p = os.path.join(ROOT, "profiles", "r01_gather_ncu_summary.txt")
+    if os.path.exists(p):
+        for line in open(p):
+            if line.startswith("traffic_bytes_per_launch:"):
+                return float(line.split(":")[1])
+    return None
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0]))
+                mx.append(float(t[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, t[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_reference(args):
+    """The CPU oracle as it stands, timed on the host cores (the reference arm of this tier)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2606_02916_b200 import inputs
+    from oracle import ggo
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+    w = inputs.make_workload(args.config, device=dev, pin=False, batch=args.batch)
+    g = ggo.Graph(*w.host_graph())
+    feat = w.host_features()
+    po = w.part_offsets
+    parts = [np.ascontiguousarray(feat[po[m]:po[m + 1]]) for m in range(len(po) - 1)]
+    S = 1                                   # mini-batches per step (bounded sample of the epoch)
+    st = ggo.State(g.n, po, 0, args.n_hot, 1)
+
+    def step(i):
+        bs = [ggo.Batch(g, w.batches[(i * S + j) % len(w.batches)], w.fanouts, w.seed, (i * S + j) % len(w.batches))
+              for j in range(S)]
+        st.run_window(bs)
+        for b in bs:
+            ggo.gather(b.nodes, po, parts, w.row_bytes)
+
+    for i in range(args.warmup):
+        step(i)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        step(args.warmup + i)
+    dt = time.perf_counter() - t0
+    v = args.steps * S / dt
+    sample = "%d mini-batch(es) per step as W=%d windows of the same workload (sample + window + gather)" % (S, S)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/int32/uint64",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args, w), "step": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def workload_name(args, w):
+    return ("%s: N=%d nnz=%d dim=%d %s, %d train seeds, batch=%d (%d mini-batches/epoch), fanouts=%s, "
+            "4 owner ranges (local in HBM, 3 in pinned host)"
+            % (args.config, w.num_nodes, w.indices.numel(), w.dim, str(w.dtype).replace("torch.", ""),
+               sum(len(b) for b in w.batches), args.batch, len(w.batches), w.fanouts))
+
+
+class E2ESink:
+    """End-to-end leg: every batch's results are read back into pinned HOST buffers.
+    Two device feature buffers alternate; a copy stream drains batch i while batch i+1 is
+    gathered (user-level double buffering, all inside the timed region)."""
+
+    def __init__(self, w, cap_rows, dev):
+        self.dev = dev
+        self.feats = [torch.empty(cap_rows, w.dim, dtype=w.dtype, device=dev) for _ in range(2)]
+        self.h_x = [torch.empty(cap_rows, w.dim, dtype=w.dtype, pin_memory=True) for _ in range(2)]
+        self.h_nodes = [torch.empty(cap_rows, dtype=torch.int32, pin_memory=True) for _ in range(2)]
+        ecap = cap_rows * 2
+        self.h_blk = [torch.empty(ecap * 2 + cap_rows * 2, dtype=torch.int32, pin_memory=True) for _ in range(2)]
+        self.copy_stream = torch.cuda.Stream(dev)
+        self.done = [None, None]
+        self.i = 0
+        self.d2h_bytes = 0
+
+    def buffer(self):
+        k = self.i & 1
+        if self.done[k] is not None:
+            torch.cuda.current_stream(self.dev).wait_event(self.done[k])   # buffer k drained
+        return self.feats[k]
+
+    def consume(self, r):
+        k = self.i & 1
+        ev = torch.cuda.Event()
+        ev.record(torch.cuda.current_stream(self.dev))
+        with torch.cuda.stream(self.copy_stream):
+            self.copy_stream.wait_event(ev)
+            n = r["n_input"]
+            self.h_x[k][:n].copy_(r["features"], non_blocking=True)
+            self.h_nodes[k][:n].copy_(r["input_nodes"], non_blocking=True)
+            self.d2h_bytes += n * (r["features"].shape[1] * r["features"].element_size() + 4)
+            off = 0
+            for blk in r["blocks"]:
+                for key in ("indptr", "src_local"):
+                    t = blk[key]
+                    self.h_blk[k][off:off + t.numel()].copy_(t, non_blocking=True)
+                    off += t.numel()
+                    self.d2h_bytes += 4 * t.numel()
+            d = torch.cuda.Event()
+            d.record(self.copy_stream)
+            self.done[k] = d
+        self.i += 1
+
+    def finish(self):
+        self.copy_stream.synchronize()
+
+
+def run_ours(args):
+    from paper_2606_02916_b200 import build, dist as gdist, epoch as ep, inputs, binding
+    build.build_library()
+    rank, local_rank, world = gdist.init("nccl")
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    P = inputs.CONFIGS[args.config]["parts"]
+    w = inputs.make_workload(args.config, device=dev, batch=args.batch, local_part=rank % P)
+    n_b = len(w.batches)
+    _, order = gdist.shard_plan(rank, world, P, n_b)
+    batches = [w.batches[i] for i in order]
+    W = args.window
+    sweep_ws = [] if args.no_sweep or world > 1 else [x for x in w.cfg["windows"] if x != W]
+    g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
+                               staging_mode=args.staging_mode)
+    stream = torch.cuda.current_stream(dev)
+
+    # size the output buffer from the first window (|N_b| varies little between batches)
+    g.window_stage(10 ** 9, 0, batches[:min(W, 4)], w.fanouts)
+    cap_rows = int(max(g.batch_info(10 ** 9, j)["n_input"] for j in range(min(W, 4), )) * 1.25) + 1024
+    g.window_release(10 ** 9)
+    g.cache_reset()
+    feats = torch.empty(cap_rows, w.dim, dtype=w.dtype, device=dev)
+
+    def one_epoch(Wx, sink=None, wid0=0):
+        if sink is None:
+            ep.run_epoch(g, batches, w.fanouts, Wx, feats, stream=stream, first_window_id=wid0)
+        else:
+            wins = ep.windows_of(n_b, Wx)
+            g.window_stage(wid0, wins[0].start, [batches[i] for i in wins[0]], w.fanouts)
+            for k, win in enumerate(wins):
+                if k + 1 < len(wins):
+                    nxt = wins[k + 1]
+                    g.window_stage(wid0 + k + 1, nxt.start, [batches[i] for i in nxt], w.fanouts)
+                for j, _bi in enumerate(win):
+                    sink.consume(g.batch_gather(wid0 + k, j, sink.buffer(), stream))
+                g.window_release(wid0 + k)
+            sink.finish()
+        torch.cuda.synchronize(dev)
+        g.cache_reset()
+
+    def timed(Wx, K, warm, sink=None, profile=False, clocks=None):
+        for e in range(warm):
+            one_epoch(Wx, sink, wid0=1000 * e)
+        if profile:
+            g.profile_enable(True)
+        l0 = binding.launch_count()
+        torch.cuda.synchronize(dev)
+        gdist.barrier()
+        if clocks:
+            clocks.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for e in range(K):
+            one_epoch(Wx, sink, wid0=1000 * (warm + e))
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        wall = time.perf_counter() - t0
+        gdist.barrier()
+        ck = clocks.stop() if clocks else None
+        sec = e0.elapsed_time(e1) / 1e3
+        prof = g.profile_get() if profile else None
+        if profile:
+            g.profile_enable(False)
+        return dict(sec=sec, wall=wall, launches=binding.launch_count() - l0, prof=prof, clocks=ck)
+
+    # ---- headline: device-resident inputs --------------------------------------------------
+    main = timed(W, args.steps, args.warmup, profile=True, clocks=ClockSampler(local_rank))
+    value, tmax = gdist.aggregate_throughput(args.steps * n_b, main["sec"], dev)
+    # per-window trace of one more epoch (bytes over the host link, stall, timings)
+    tr_acc = dict(bulk_bytes=0, bulk_copies=0, wait_ms=0.0, stage_ms=0.0, pack_ms=0.0, h2d_ms=0.0, n_access=0)
+
+    def on_window(wid, win):
+        t = g.trace(wid, len(win))
+        tr_acc["bulk_bytes"] += sum(t["bulk_bytes"])
+        tr_acc["bulk_copies"] += t["bulk_copies"]
+        tr_acc["wait_ms"] += t["ms_boundary_wait"]
+        tr_acc["stage_ms"] += t["ms_stage_total"]
+        tr_acc["pack_ms"] += t["ms_pack_host"]
+        tr_acc["h2d_ms"] += t["ms_h2d"]
+        tr_acc["n_access"] += t["n_access"]
+
+    ep.run_epoch(g, batches, w.fanouts, W, feats, on_window=on_window, stream=stream, first_window_id=5 * 10 ** 6)
+    torch.cuda.synchronize(dev)
+    g.cache_reset()
+
+    # ---- end to end: results read back to pinned host buffers every batch -------------------
+    e2e = None
+    if not args.no_e2e:
+        sink = E2ESink(w, cap_rows, dev)
+        r = timed(W, max(1, min(args.steps, 2)), 1, sink=sink)
+        k_e = max(1, min(args.steps, 2))
+        ev, _ = gdist.aggregate_throughput(k_e * n_b, r["sec"], dev)
+        seeds_bytes = 4 * sum(len(b) for b in batches)
+        e2e = {"value": ev, "unit": UNIT,
+               "h2d_bytes_per_step": int(seeds_bytes + tr_acc["bulk_bytes"]),
+               "d2h_bytes_per_step": int(sink.d2h_bytes / (k_e + 1)),
+               "note": "seeds from host buffers via gg_window_stage; remote rows staged pinned->HBM inside the "
+                       "library; X_b, N_b, block indptr/src_local copied to pinned host every batch"}
+        del sink
+
+    # ---- W sweep (the metric is 'per epoch vs W'): 1 warm + 1 timed epoch per point ----------
+    vs_w = {str(W): value}
+    for Wx in sweep_ws:
+        r = timed(Wx, 1, 1)
+        vs_w[str(Wx)] = n_b / r["sec"]
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel (slot-map gather) ------------------------------------
+    peak, peak_src = measured_peaks()
+    pg = main["prof"]["gather"]
+    ach = pg["bytes"] / (pg["ms"] * 1e-3) / 1e9 if pg["ms"] > 0 else 0.0
+    roof = {"bound": "hbm", "kernel": "k_gather", "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak, "traffic": ncu_traffic(), "peak_source": peak_src,
+            "launches": pg["regions"], "avg_launch_us": 1e3 * pg["ms"] / max(pg["regions"], 1),
+            "algorithmic_bytes_per_launch": pg["bytes"] / max(pg["regions"], 1),
+            "share_of_step": pg["ms"] * 1e-3 / main["sec"]}
+    stages = {}
+    for k, v in main["prof"].items():
+        if v["regions"]:
+            stages[k] = {"ms_per_step": v["ms"] / args.steps, "regions_per_step": v["regions"] / args.steps,
+                         "GB/s": (v["bytes"] / (v["ms"] * 1e-3) / 1e9) if v["ms"] > 0 and v["bytes"] else None}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu = cpu_baseline(args, w, batches)
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u8 rows / int32 ids / uint64 keys",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot,
+                   "staging_mode": args.staging_mode, "carry_over": 1,
+                   "step": "one epoch = %d mini-batches in %d windows, cache reset per epoch" % (n_b, -(-n_b // W)),
+                   "l2": "inputs larger than L2 (feature store %.0f MB, X_b %.0f MB per batch)"
+                         % (w.num_nodes * w.row_bytes / 1e6, tr_acc["n_access"] / n_b * w.row_bytes / 1e6)},
+        "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
+        "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
+        "roofline": roof, "stages": stages, "vs_W": vs_w,
+        "staging": {"host_link_bytes_per_step": int(tr_acc["bulk_bytes"]), "bulk_copies_per_step": tr_acc["bulk_copies"],
+                    "h2d_GB/s": tr_acc["bulk_bytes"] / (tr_acc["h2d_ms"] * 1e-3) / 1e9 if tr_acc["h2d_ms"] > 0 else None,
+                    "host_pack_ms_per_step": tr_acc["pack_ms"], "stage_ms_per_step": tr_acc["stage_ms"],
+                    "boundary_stall_ms_per_step": tr_acc["wait_ms"]},
+        "e2e": e2e, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+    g.close()
+
+
+def cpu_baseline(args, w, batches):
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    from oracle import ggo
+    S = min(args.cpu_sample_batches, len(batches), args.window)
+    g = ggo.Graph(*w.host_graph())
+    feat = w.host_features()
+    po = w.part_offsets
+    parts = [np.ascontiguousarray(feat[po[m]:po[m + 1]]) for m in range(len(po) - 1)]
+    st = ggo.State(g.n, po, w.local_part, args.n_hot, 1)
+    t0 = time.perf_counter()
+    bs = [ggo.Batch(g, batches[j], w.fanouts, w.seed, j) for j in range(S)]
+    st.run_window(bs)
+    for b in bs:
+        ggo.gather(b.nodes, po, parts, w.row_bytes)
+    dt = time.perf_counter() - t0
+    return {"value": S / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "first %d mini-batches of the epoch as one W=%d window (sample + window + gather), %.1f s"
+                      % (S, S, dt)}
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -212,6 +212,31 @@ gg_status gg_cache_reset(gg_graph* g);
  * pin against tests/golden/keys.txt). */
 uint64_t gg_key(uint64_t seed, uint64_t batch, uint64_t layer, uint64_t dst, uint64_t edge_pos);
 
+/* Live measurement support (bench.py roofline leg).  When enabled, the library brackets its own
+ * kernel groups with CUDA events ON THE STREAM THEY ARE LAUNCHED ON (caller's stream for the
+ * gather and miss path, the side stream for everything else) and counts algorithmic bytes:
+ *   GATHER  one k_gather launch per region; bytes = |N_b| * (2*row_bytes + 8)
+ *   MISS    miss compaction + fill;          bytes = misses * 2*row_bytes   (counted at gg_trace time: 0 here)
+ *   SAMPLE  count + scan + select of a hop;  bytes = 24*n_dst + 8*n_edge
+ *   FRONTIER mark + word scan + emit + relabel of a hop; bytes = 8*n_edge + 4*n_new
+ *   UNIQUE  counter compaction;              bytes = 4*n_access + 8*n_unique
+ *   SELECT  hot select + delta split;        bytes = 12*n_unique
+ *   STAGE_COPY the per-owner bulk transfers; bytes = sum |Delta_m| * row_bytes (host link)
+ *   CARRY   carry-over D2D copy;             bytes = 2 * carried * row_bytes
+ * gg_profile_enable(g, on) clears the accumulators; gg_profile_get synchronises the device. */
+#define GG_PROF_KINDS 8
+enum { GG_PROF_GATHER = 0, GG_PROF_MISS = 1, GG_PROF_SAMPLE = 2, GG_PROF_FRONTIER = 3,
+       GG_PROF_UNIQUE = 4, GG_PROF_SELECT = 5, GG_PROF_STAGE_COPY = 6, GG_PROF_CARRY = 7 };
+typedef struct {
+  double ms[GG_PROF_KINDS];
+  int64_t regions[GG_PROF_KINDS];
+  int64_t bytes[GG_PROF_KINDS];
+} gg_profile;
+gg_status gg_profile_enable(gg_graph* g, int32_t on);
+gg_status gg_profile_get(gg_graph* g, gg_profile* out);
+/* number of kernels this library has launched in this process (all graphs) */
+uint64_t gg_launch_count(void);
+
 const char* gg_last_error(void);
 const char* gg_version(void);
 

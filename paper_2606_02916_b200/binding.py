@@ -64,7 +64,13 @@ class gg_window_trace(C.Structure):
                 ("ms_h2d", f32), ("ms_carry", f32), ("ms_stage_total", f32), ("ms_boundary_wait", f32)]
 
 
-SYMBOLS = ["gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
+class gg_profile(C.Structure):
+    _fields_ = [("ms", C.c_double * 8), ("regions", i64 * 8), ("bytes", i64 * 8)]
+
+
+PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage_copy", "carry"]
+
+SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
            "gg_cache_reset", "gg_key", "gg_last_error", "gg_version"]
 
@@ -98,16 +104,23 @@ def load_library(path: Optional[str] = None):
     lib.gg_window_export.argtypes = [vp, i64, i32, vp, i64, P(i64)]
     lib.gg_cache_read.argtypes = [vp, i64, vp, i64, vp]
     lib.gg_cache_reset.argtypes = [vp]
+    lib.gg_profile_enable.argtypes = [vp, i32]
+    lib.gg_profile_get.argtypes = [vp, P(gg_profile)]
+    lib.gg_launch_count.restype = u64
     lib.gg_key.argtypes = [u64] * 5
     lib.gg_key.restype = u64
     lib.gg_last_error.restype = C.c_char_p
     lib.gg_version.restype = C.c_char_p
     for s in SYMBOLS:
         getattr(lib, s)
-        if s not in ("gg_key", "gg_last_error", "gg_version"):
+        if s not in ("gg_key", "gg_last_error", "gg_version", "gg_launch_count"):
             getattr(lib, s).restype = i32
     _lib = lib
     return lib
+
+
+def launch_count() -> int:
+    return int(load_library().gg_launch_count())
 
 
 def gg_key(seed: int, batch: int, layer: int, dst: int, edge_pos: int) -> int:
@@ -263,6 +276,14 @@ class Graph:
         out = np.empty((len(ids), self.rb), dtype=np.uint8)
         self._check(self.lib.gg_cache_read(self.h, window_id, ids.ctypes.data, len(ids), out.ctypes.data))
         return out
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.gg_profile_enable(self.h, 1 if on else 0))
+
+    def profile_get(self) -> Dict:
+        p = gg_profile()
+        self._check(self.lib.gg_profile_get(self.h, C.byref(p)))
+        return {k: dict(ms=p.ms[i], regions=p.regions[i], bytes=p.bytes[i]) for i, k in enumerate(PROF_KINDS)}
 
     def cache_reset(self):
         self._check(self.lib.gg_cache_reset(self.h))

@@ -178,11 +178,66 @@ struct Window {
   std::string error;
 };
 
+// live measurement: event pairs recorded on the launching stream, resolved at gg_profile_get
+struct Profiler {
+  struct Rec { cudaEvent_t a, b; int kind; };
+  std::mutex m;
+  bool on = false;
+  std::vector<Rec> recs;
+  std::vector<cudaEvent_t> pool;
+  double ms[GG_PROF_KINDS] = {0};
+  int64_t regions[GG_PROF_KINDS] = {0}, bytes[GG_PROF_KINDS] = {0};
+  cudaEvent_t get() {
+    if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+  }
+  // returns the start event (recorded) or nullptr when profiling is off
+  cudaEvent_t begin(cudaStream_t st) {
+    std::lock_guard<std::mutex> l(m);
+    if (!on) return nullptr;
+    cudaEvent_t a = get();
+    cudaEventRecord(a, st);
+    return a;
+  }
+  void end(cudaStream_t st, cudaEvent_t a, int kind, int64_t nbytes) {
+    if (!a) return;
+    std::lock_guard<std::mutex> l(m);
+    cudaEvent_t b = get();
+    cudaEventRecord(b, st);
+    recs.push_back({a, b, kind});
+    bytes[kind] += nbytes;
+  }
+  void resolve() {
+    std::lock_guard<std::mutex> l(m);
+    for (auto& r : recs) {
+      float t = 0;
+      cudaEventSynchronize(r.b);
+      if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) { ms[r.kind] += t; regions[r.kind] += 1; }
+      pool.push_back(r.a);
+      pool.push_back(r.b);
+    }
+    recs.clear();
+  }
+  void clear() {
+    resolve();
+    std::lock_guard<std::mutex> l(m);
+    for (int k = 0; k < GG_PROF_KINDS; ++k) { ms[k] = 0; regions[k] = 0; bytes[k] = 0; }
+  }
+  void destroy() {
+    resolve();
+    for (auto e : pool) cudaEventDestroy(e);
+    pool.clear();
+  }
+};
+
 }  // namespace gg
 
 using namespace gg;
 
 struct gg_graph {
+  Profiler prof;
   // inputs
   int64_t N = 0, nnz = 0;
   const int64_t* indptr = nullptr;
@@ -215,6 +270,7 @@ struct gg_graph {
   // streams / thread
   cudaStream_t side = nullptr;
   cudaEvent_t ev_a = nullptr, ev_b = nullptr;
+  cudaEvent_t ev_copy[2 * GG_MAX_PARTS] = {nullptr};
   Window win[2];
   uint64_t stage_counter = 0;
   bool have_prev = false;
@@ -356,13 +412,17 @@ static gg_status stage_window(gg_graph* g, Window* w) {
     dst_off.v[W] = H.dst_off[W];
     const int max_tiles = (int)ceil_div(max_nd, 256);
     const int64_t cnt_pitch = max_nd;
+    cudaEvent_t pe = g->prof.begin(st);
     launch_sample_hop(st, g->indptr, g->indices, w->nodes.p, w->node_pitch, n_dst, dst_off, W, max_nd,
                       w->fanouts[h], g->key_prefix.p + h * Wmax, g->cnt_tmp.p, cnt_pitch, g->tiles32.p,
                       max_tiles, edge_totals, H.blk_indptr.p, H.edge_off_dev.p, H.src_global.p);
+    g->prof.end(st, pe, GG_PROF_SAMPLE, 0);
     const int64_t max_edges = (int64_t)H.dst_off[W] * w->fanouts[h];
+    pe = g->prof.begin(st);
     launch_frontier_hop(st, g->F, h, W, H.src_global.p, H.edge_off_dev.p, max_edges, n_dst,
                         (int32_t)w->node_pitch, w->nodes.p, w->node_pitch, g->cnt8.p, w->n_front_dev.p,
                         Wmax, g->tiles32.p, new_totals, g->err_flag.p, H.src_local.p);
+    g->prof.end(st, pe, GG_PROF_FRONTIER, 0);
     // sizes of the next frontier and of this hop's blocks -> host
     CU(cudaMemcpyAsync(g->h_small, w->n_front_dev.p + (h + 1) * Wmax, W * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(g->h_small + Wmax, H.edge_off_dev.p, (W + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -373,6 +433,13 @@ static gg_status stage_window(gg_graph* g, Window* w) {
                   (long long)w->node_pitch);
     w->n_front[h + 1].assign(g->h_small, g->h_small + W);
     H.edge_off.assign(g->h_small + Wmax, g->h_small + Wmax + W + 1);
+    if (g->prof.on) {
+      int64_t n_new = 0;
+      for (int b = 0; b < W; ++b) n_new += w->n_front[h + 1][b] - w->n_front[h][b];
+      std::lock_guard<std::mutex> l(g->prof.m);
+      g->prof.bytes[GG_PROF_SAMPLE] += 24ll * H.dst_off[W] + 8ll * H.edge_off[W];
+      g->prof.bytes[GG_PROF_FRONTIER] += 8ll * H.edge_off[W] + 4ll * n_new;
+    }
   }
   int max_n = 0;
   w->n_access = 0;
@@ -385,7 +452,9 @@ static gg_status stage_window(gg_graph* g, Window* w) {
   w->ms_sample = (float)(t1 - t0);
 
   // a-3 unique + count
+  cudaEvent_t pe = g->prof.begin(st);
   launch_unique_count(st, g->cnt8.p, g->cnt_words, g->R, g->tiles32.p, g->stats.p, g->hist.p, w->uniq.p, w->cnt.p);
+  g->prof.end(st, pe, GG_PROF_UNIQUE, 0);
   CU(cudaMemcpyAsync(g->h_small, g->stats.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CU(cudaMemcpyAsync(g->h_small + 1, g->hist.p, 256 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
@@ -412,6 +481,7 @@ static gg_status stage_window(gg_graph* g, Window* w) {
     }
     quota = (uint32_t)(w->n_hot - above);
   }
+  pe = g->prof.begin(st);
   launch_slots_clear(st, w->hot.p, (int)w->n_cached, w->slot_map);
   w->n_cached = 0;
   if (w->n_hot > 0)
@@ -421,6 +491,11 @@ static gg_status stage_window(gg_graph* g, Window* w) {
   launch_delta_split(st, w->hot.p, (int)w->n_hot, g->R, prev ? prev->slot_map : nullptr, carry, g->tiles32.p,
                      g->n_delta_dev.p, g->owner_cnt.p, w->slot_map, w->req_ids.p, w->carry_src.p, w->carry_ids.p);
   w->n_cached = w->n_hot;
+  g->prof.end(st, pe, GG_PROF_SELECT, 12ll * w->n_unique);
+  if (g->prof.on) {
+    std::lock_guard<std::mutex> l(g->prof.m);
+    g->prof.bytes[GG_PROF_UNIQUE] += 4ll * w->n_access + 8ll * w->n_unique;
+  }
   CU(cudaMemcpyAsync(g->h_small, g->owner_cnt.p, 2 * GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CU(cudaMemcpyAsync(g->h_small + 2 * GG_MAX_PARTS, g->n_delta_dev.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
@@ -467,7 +542,9 @@ static gg_status stage_window(gg_graph* g, Window* w) {
           std::memcpy(resp + i * rb, base + (ids[i] - lo) * stride, (size_t)rb);
       });
       w->ms_pack += (float)(now_ms() - p0);
+      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));
       CU(cudaMemcpyAsync(w->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, st));
+      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies + 1], st));
       w->bulk_copies += 1;
       q0 += nm;
     }
@@ -477,21 +554,35 @@ static gg_status stage_window(gg_graph* g, Window* w) {
     for (int m = 0; m < g->R.P; ++m) {
       const int64_t nm = w->bulk[m];
       if (nm == 0) continue;
+      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));
       launch_rows_from_store(st, w->req_ids.p + q0, (int)nm, g->store, g->R, w->cache, q0, rb, (int)rb);
+      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies + 1], st));
       w->bulk_copies += 1;
       q0 += nm;
     }
   }
   CU(cudaEventRecord(g->ev_b, st));
+  pe = g->prof.begin(st);
   // carried rows: D2D out of the previous buffer, after the delta rows
   if (w->n_carry > 0)
     launch_rows_from_list(st, w->carry_src.p, (int)w->n_carry, prev->cache, rb, w->cache, w->n_delta, rb, (int)rb);
+  g->prof.end(st, pe, GG_PROF_CARRY, 2ll * w->n_carry * rb);
   CU(cudaMemsetAsync(w->counters.p, 0, (size_t)Wmax * (2 + GG_MAX_PARTS) * sizeof(int32_t), st));
   CU(cudaEventRecord(w->ready, st));
   CU(cudaEventSynchronize(w->ready));
   float ms = 0;
-  cudaEventElapsedTime(&ms, g->ev_a, g->ev_b);
-  w->ms_h2d = ms;
+  w->ms_h2d = 0;
+  for (int c = 0; c < w->bulk_copies; ++c) {
+    cudaEventElapsedTime(&ms, g->ev_copy[2 * c], g->ev_copy[2 * c + 1]);
+    w->ms_h2d += ms;
+  }
+  ms = w->ms_h2d;
+  if (g->prof.on && w->n_delta > 0) {
+    std::lock_guard<std::mutex> l(g->prof.m);
+    g->prof.ms[GG_PROF_STAGE_COPY] += ms;
+    g->prof.regions[GG_PROF_STAGE_COPY] += w->bulk_copies;
+    g->prof.bytes[GG_PROF_STAGE_COPY] += w->n_delta * rb;
+  }
   cudaEventElapsedTime(&ms, g->ev_b, w->ready);
   w->ms_carry = ms;
   CU(cudaGetLastError());
@@ -565,6 +656,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
   cudaSetDevice(g->device);
   cudaDeviceSynchronize();
   delete g->pool;
+  g->prof.destroy();
   for (int s = 0; s < 2; ++s) {
     Window& w = g->win[s];
     w.nodes.release(); w.n_front_dev.release(); w.uniq.release(); w.cnt.release();
@@ -592,6 +684,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
   if (g->h_kp) cudaFreeHost(g->h_kp);
   if (g->ev_a) cudaEventDestroy(g->ev_a);
   if (g->ev_b) cudaEventDestroy(g->ev_b);
+  for (int c = 0; c < 2 * GG_MAX_PARTS; ++c) if (g->ev_copy[c]) cudaEventDestroy(g->ev_copy[c]);
   if (g->side) cudaStreamDestroy(g->side);
   delete g;
   return GG_OK;
@@ -688,6 +781,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   CUC(cudaHostAlloc((void**)&g->h_kp, (size_t)GG_MAX_LAYERS * Wmax * sizeof(uint64_t), cudaHostAllocDefault));
   CUC(cudaStreamCreateWithFlags(&g->side, cudaStreamNonBlocking));
   CUC(cudaEventCreate(&g->ev_a)); CUC(cudaEventCreate(&g->ev_b));
+  for (int c = 0; c < 2 * GG_MAX_PARTS; ++c) CUC(cudaEventCreate(&g->ev_copy[c]));
   for (int s = 0; s < 2; ++s) {
     Window& w = g->win[s];
     w.slot = s;
@@ -820,7 +914,14 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   G.miss_tmp_pos = g->miss_tmp_pos.p; G.miss_tmp_id = g->miss_tmp_id.p; G.tile_miss = g->tile_miss.p;
   G.miss_pos = g->miss_pos.p; G.miss_id = g->miss_id.p; G.n_miss = g->n_miss.p;
   G.counters = w->counters.p + (int64_t)b * (2 + GG_MAX_PARTS);
+  cudaEvent_t pe = g->prof.begin(st);
   launch_gather(st, G);
+  g->prof.end(st, pe, GG_PROF_GATHER, (int64_t)n * (2ll * g->rb + 8));
+  if (w->may_miss) {
+    pe = g->prof.begin(st);
+    launch_miss_path(st, G);
+    g->prof.end(st, pe, GG_PROF_MISS, 0);
+  }
   CU(cudaEventRecord(w->gather_done, st));
   w->gather_recorded = true;
   CU(cudaGetLastError());
@@ -907,6 +1008,30 @@ gg_status gg_cache_read(gg_graph* g, int64_t window_id, const int32_t* ids, int6
   }
   return GG_OK;
 }
+
+gg_status gg_profile_enable(gg_graph* g, int32_t on) {
+  if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
+  CU(cudaDeviceSynchronize());
+  g->prof.clear();
+  std::lock_guard<std::mutex> l(g->prof.m);
+  g->prof.on = on != 0;
+  return GG_OK;
+}
+
+gg_status gg_profile_get(gg_graph* g, gg_profile* out) {
+  if (!g || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
+  CU(cudaDeviceSynchronize());
+  g->prof.resolve();
+  std::lock_guard<std::mutex> l(g->prof.m);
+  for (int k = 0; k < GG_PROF_KINDS; ++k) {
+    out->ms[k] = g->prof.ms[k];
+    out->regions[k] = g->prof.regions[k];
+    out->bytes[k] = g->prof.bytes[k];
+  }
+  return GG_OK;
+}
+
+uint64_t gg_launch_count(void) { return (uint64_t)g_launches.load(); }
 
 gg_status gg_cache_reset(gg_graph* g) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");

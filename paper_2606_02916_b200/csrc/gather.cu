@@ -237,7 +237,13 @@ void launch_gather(cudaStream_t st, const GatherLaunch& G) {
   if (vec == 16) k_gather<16><<<tiles, kThreads, 0, st>>>(A);
   else if (vec == 8) k_gather<8><<<tiles, kThreads, 0, st>>>(A);
   else k_gather<4><<<tiles, kThreads, 0, st>>>(A);
-  if (!G.may_miss) return;
+  count_launches(1);
+}
+
+void launch_miss_path(cudaStream_t st, const GatherLaunch& G) {
+  if (G.n <= 0 || !G.may_miss) return;
+  const int tiles = (G.n + kRows - 1) / kRows;
+  count_launches(2);
   k_miss_compact<<<1, 1024, 0, st>>>(G.tile_miss, tiles, G.miss_tmp_pos, G.miss_tmp_id, G.miss_pos,
                                      G.miss_id, G.n_miss);
   // a-8: fill the missed rows straight from the owners' pinned stores (zero-copy reads)
@@ -273,6 +279,7 @@ void launch_rows_from_list(cudaStream_t st, const int32_t* src_idx, int n, const
   if (vec == 16) k_rows<16, 0><<<grid, kThreads, 0, st>>>(A);
   else if (vec == 8) k_rows<8, 0><<<grid, kThreads, 0, st>>>(A);
   else k_rows<4, 0><<<grid, kThreads, 0, st>>>(A);
+  count_launches(1);
 }
 
 void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const StorePtrs& store,
@@ -293,6 +300,7 @@ void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const St
   if (ok16) k_rows<16, 1><<<grid, kThreads, 0, st>>>(A);
   else if (ok8) k_rows<8, 1><<<grid, kThreads, 0, st>>>(A);
   else k_rows<4, 1><<<grid, kThreads, 0, st>>>(A);
+  count_launches(1);
 }
 
 }  // namespace gg

@@ -1,8 +1,13 @@
 // Host-callable launchers of the sm_100a kernels (one translation unit per path step).
 #pragma once
+#include <atomic>
+
 #include "common.cuh"
 
 namespace gg {
+
+extern std::atomic<unsigned long long> g_launches;  // kernels launched by this library
+inline void count_launches(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 
 constexpr int kWordThreads = 256;
 constexpr int kWordTile = 2048;  // 32-bit words per CTA tile in the bitmap / counter passes
@@ -77,7 +82,8 @@ struct GatherLaunch {
   int32_t* n_miss;        // device scalar
   int32_t* counters;      // [2 + P]
 };
-void launch_gather(cudaStream_t st, const GatherLaunch& G);
+void launch_gather(cudaStream_t st, const GatherLaunch& G);      // a-7: one k_gather launch
+void launch_miss_path(cudaStream_t st, const GatherLaunch& G);   // a-8: compaction + fill (only if may_miss)
 void launch_rows_from_list(cudaStream_t st, const int32_t* src_idx, int n, const uint8_t* src_base,
                            int64_t src_stride, uint8_t* dst_base, int64_t dst_row0, int64_t dst_stride,
                            int rb);

@@ -211,6 +211,7 @@ k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ 
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
                       int items_per_tile, int32_t* totals) {
   k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals);
+  count_launches(1);
 }
 
 void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* indices,
@@ -221,6 +222,7 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
                        int32_t* edge_off_out, int32_t* src_global) {
   const int tiles = (max_nd + kTile - 1) / kTile;
   dim3 grid(tiles, W);
+  count_launches(3);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
                                          cnt_tmp, cnt_pitch, tile_sums);
   k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals);

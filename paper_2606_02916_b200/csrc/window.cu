@@ -16,6 +16,8 @@
 
 namespace gg {
 
+std::atomic<unsigned long long> g_launches{0};
+
 template <typename T>
 __global__ void __launch_bounds__(1024) k_row_scan(T* __restrict__ tiles, int n, T* __restrict__ total) {
   __shared__ T sm[33];
@@ -237,6 +239,7 @@ void launch_unique_count(cudaStream_t st, uint32_t* cnt8, int64_t n_words_padded
                          int32_t* tile_sums, int32_t* stats, int32_t* hist, int32_t* uniq, int32_t* cnt) {
   const int tiles = (int)(n_words_padded / kWordTile);
   cudaMemsetAsync(hist, 0, 256 * sizeof(int32_t), st);
+  count_launches(3);
   k_cnt_reduce<<<tiles, kWordThreads, 0, st>>>(cnt8, R, tile_sums, hist);
   k_row_scan<int32_t><<<1, 1024, 0, st>>>(tile_sums, tiles, stats);
   k_cnt_emit<<<tiles, kWordThreads, 0, st>>>(cnt8, tile_sums, uniq, cnt);
@@ -247,6 +250,7 @@ void launch_hot_select(cudaStream_t st, const int32_t* uniq, const int32_t* cnt,
                        uint64_t* total64, int32_t* hot) {
   if (n_unique <= 0) return;
   const int tiles = (n_unique + kSelTile - 1) / kSelTile;
+  count_launches(3);
   k_select_reduce<<<tiles, kSelThreads, 0, st>>>(uniq, cnt, n_unique, R, thr, tile_sums64);
   k_row_scan<uint64_t><<<1, 1024, 0, st>>>(tile_sums64, tiles, total64);
   k_select_emit<<<tiles, kSelThreads, 0, st>>>(uniq, cnt, n_unique, R, thr, quota_eq, tile_sums64, hot);
@@ -260,6 +264,7 @@ void launch_delta_split(cudaStream_t st, const int32_t* hot, int n_hot, const Ow
   cudaMemsetAsync(n_delta, 0, sizeof(int32_t), st);
   if (n_hot <= 0) return;
   const int tiles = (n_hot + kSelTile - 1) / kSelTile;
+  count_launches(3);
   k_delta_reduce<<<tiles, kSelThreads, 0, st>>>(hot, n_hot, R, slot_prev, carry_over, tile_sums, owner_cnt);
   k_row_scan<int32_t><<<1, 1024, 0, st>>>(tile_sums, tiles, n_delta);
   k_delta_emit<<<tiles, kSelThreads, 0, st>>>(hot, n_hot, slot_prev, carry_over, tile_sums, n_delta,
@@ -271,6 +276,7 @@ void launch_slots_clear(cudaStream_t st, const int32_t* ids, int n, int32_t* slo
   int g = (n + 255) / 256;
   if (g > 148 * 8) g = 148 * 8;
   k_slots_clear<<<g, 256, 0, st>>>(ids, n, slot_map);
+  count_launches(1);
 }
 
 void launch_fill_i32(cudaStream_t st, int32_t* p, int64_t n, int32_t v) {
@@ -278,6 +284,7 @@ void launch_fill_i32(cudaStream_t st, int32_t* p, int64_t n, int32_t v) {
   int64_t g = (n + 255) / 256;
   if (g > 148 * 16) g = 148 * 16;
   k_fill_i32<<<(int)g, 256, 0, st>>>(p, n, v);
+  count_launches(1);
 }
 
 }  // namespace gg

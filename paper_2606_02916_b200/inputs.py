@@ -364,7 +364,7 @@ def master_seed(cfg: dict) -> int:
 
 
 def make_workload(name: str, device="cpu", pin: Optional[bool] = None,
-                  batch: Optional[int] = None) -> Workload:
+                  batch: Optional[int] = None, local_part: int = 0) -> Workload:
     cfg = dict(CONFIGS[name])
     if batch is not None:
         cfg["batch"] = batch
@@ -395,7 +395,7 @@ def make_workload(name: str, device="cpu", pin: Optional[bool] = None,
     parts: List[torch.Tensor] = []
     for m in range(P):
         lo, hi = int(part_offsets[m]), int(part_offsets[m + 1])
-        if m == 0:
+        if m == local_part:
             parts.append(feature_rows(lo, hi - lo, cfg["dim"], dtype, fseed, device))
         else:
             host = torch.empty(hi - lo, cfg["dim"], dtype=dtype, pin_memory=bool(pin))
@@ -411,6 +411,6 @@ def make_workload(name: str, device="cpu", pin: Optional[bool] = None,
     if cfg["max_batches"]:
         batches = batches[:cfg["max_batches"]]
     return Workload(name=name, cfg=cfg, num_nodes=n, indptr=indptr, indices=indices,
-                    part_offsets=part_offsets, local_part=0, feat_parts=parts, dim=cfg["dim"],
+                    part_offsets=part_offsets, local_part=local_part, feat_parts=parts, dim=cfg["dim"],
                     dtype=dtype, batches=batches, fanouts=list(cfg["fanouts"]),
                     seed=substream(ms, 400))
