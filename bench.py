@@ -236,11 +236,12 @@ def run_ours(args):
             ep.run_epoch(g, batches, w.fanouts, Wx, feats, stream=stream, first_window_id=wid0)
         else:
             wins = ep.windows_of(n_b, Wx)
-            g.window_stage(wid0, wins[0].start, [batches[i] for i in wins[0]], w.fanouts)
+            for k in range(min(2, len(wins))):
+                g.window_stage(wid0 + k, wins[k].start, [batches[i] for i in wins[k]], w.fanouts)
             for k, win in enumerate(wins):
-                if k + 1 < len(wins):
-                    nxt = wins[k + 1]
-                    g.window_stage(wid0 + k + 1, nxt.start, [batches[i] for i in nxt], w.fanouts)
+                if k + 2 < len(wins):
+                    nxt = wins[k + 2]
+                    g.window_stage(wid0 + k + 2, nxt.start, [batches[i] for i in nxt], w.fanouts)
                 for j, _bi in enumerate(win):
                     sink.consume(g.batch_gather(wid0 + k, j, sink.buffer(), stream))
                 g.window_release(wid0 + k)

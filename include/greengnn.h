@@ -40,8 +40,11 @@
  *    hop whose n_src = n_input.  fanouts[h] belongs to hop h counted outward (reading S2).
  *  - Every function returns a gg_status; none aborts or throws; on error no output is
  *    partially valid.  gg_last_error() gives the text for the calling thread's last failure.
- *  - One caller thread per gg_graph.  At most two windows are live (k being served, k+1
- *    being staged).
+ *  - One caller thread per gg_graph.  At most THREE windows are live: k being served, k+1
+ *    whose cache is being staged, k+2 being sampled (the two prefetch phases run on two library
+ *    threads and two side streams).  There are two cache buffers: window k+2's cache is built
+ *    only after window k is released, so asking for k+2's batches while k is live is
+ *    GG_ERR_STATE.  Staging one window ahead (the literal loop of Alg. 1) is equally valid.
  */
 #ifndef GREENGNN_H_
 #define GREENGNN_H_
@@ -62,7 +65,7 @@ typedef struct gg_graph gg_graph; /* opaque */
 typedef enum {
   GG_OK = 0,
   GG_ERR_INVALID_ARG = 1, /* null pointer, out-of-range value, wrong memory kind */
-  GG_ERR_STATE = 2,       /* window never staged / already released / third live window */
+  GG_ERR_STATE = 2,       /* window never staged / already released / fourth live window */
   GG_ERR_CAPACITY = 3,    /* a caller buffer or a create-time cap is too small; nothing truncated */
   GG_ERR_OOM = 4,
   GG_ERR_CUDA = 5
@@ -124,7 +127,7 @@ gg_status gg_graph_destroy(gg_graph* g);
  *                  keyed with first_batch_index+i (reading S7: epoch is not hashed)
  *   fanouts        host int32 [num_layers], hop order outward from the seeds, 1..GG_MAX_FANOUT
  * Errors: INVALID_ARG (nulls, W<1 or >max_window, L<1 or >max_layers, a batch larger than
- * max_batch or empty window, seed outside [0,N)), STATE (two windows already live, or
+ * max_batch or empty window, seed outside [0,N)), STATE (three windows already live, or
  * window_id already live), CAPACITY (caps derived from fanouts exceed int32 indexing). */
 gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_index,
                           const int32_t* seeds, const int64_t* batch_offsets, int32_t W,

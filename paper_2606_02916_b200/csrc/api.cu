@@ -143,11 +143,24 @@ struct Hop {
   std::vector<int32_t> dst_off;   // host [W+1]
 };
 
+struct Window;
+
+// One of the two cache buffers: rows, ID->slot map and the cached-ID list (= C_k).  They
+// outlive the window that filled them: the next window's delta is taken against them.
+struct CacheSlot {
+  uint8_t* cache = nullptr;
+  int32_t* slot_map = nullptr;
+  DevBuf<int32_t> hot;
+  int64_t n_cached = 0;        // entries of `hot` currently reflected in slot_map
+  Window* tenant = nullptr;    // window whose H_k is in here (may already be released)
+};
+
+// One of the three window arenas (k being served, k+1 being staged, k+2 being sampled).
 struct Window {
   // identity / arguments
   int64_t id = -1;
+  uint64_t seq = 0;   // stage order
   bool live = false;
-  int slot = 0;
   int W = 0, L = 0;
   int fanouts[GG_MAX_LAYERS] = {0};
   uint64_t first_batch = 0;
@@ -158,27 +171,26 @@ struct Window {
   int64_t node_pitch = 0;
   Hop hop[GG_MAX_LAYERS];
   std::vector<int32_t> n_front[GG_MAX_LAYERS + 1];  // host mirrors [W]
-  // cache slot (C_k): buffer, map and cached-ID list persist after release
-  uint8_t* cache = nullptr;
-  int32_t* slot_map = nullptr;
-  DevBuf<int32_t> hot;
-  int64_t n_cached = 0;  // entries of `hot` currently reflected in slot_map
+  CacheSlot* cs = nullptr;
   // results
+  int32_t hist[256] = {0};
   int64_t n_access = 0, n_unique = 0, n_remote = 0, n_hot = 0, n_delta = 0, n_carry = 0;
   int64_t staged[GG_MAX_PARTS] = {0}, bulk[GG_MAX_PARTS] = {0};
   int bulk_copies = 0;
   bool may_miss = false;
   float ms_sample = 0, ms_unique = 0, ms_select = 0, ms_pack = 0, ms_h2d = 0, ms_carry = 0,
         ms_total = 0, ms_wait = 0;
+  double t_enqueue = 0;
   // sync
-  cudaEvent_t ready = nullptr, gather_done = nullptr;
+  cudaEvent_t sampled = nullptr;  // phase A complete (stream A)
+  cudaEvent_t ready = nullptr;    // cache ready (stream B)
+  cudaEvent_t gather_done = nullptr;
   bool gather_recorded = false;
-  bool enqueued = false;
+  bool enqueued = false;          // phase B finished on the host (or an error was recorded)
   gg_status status = GG_OK;
   std::string error;
 };
 
-// live measurement: event pairs recorded on the launching stream, resolved at gg_profile_get
 struct Profiler {
   struct Rec { cudaEvent_t a, b; int kind; };
   std::mutex m;
@@ -249,36 +261,41 @@ struct gg_graph {
   gg_config cfg;
   int64_t cache_rows = 0, n_hot_eff = 0;
   int device = 0;
-  // workspaces (prefetch thread only)
+  // phase A workspaces (sampler thread only)
   FrontierBufs F = {};
   int n_gen = 0;
   DevBuf<uint32_t> seen, newbits, cnt8;
-  DevBuf<int32_t> wprefix, seed_perm, tiles32, totals, stats, hist, owner_cnt, n_delta_dev, err_flag,
-      seeds_dev;
-  DevBuf<uint64_t> tiles64, total64, key_prefix;
+  DevBuf<int32_t> wprefix, seed_perm, tiles32, totals, stats, hist, err_flag, seeds_dev;
+  DevBuf<uint64_t> key_prefix;
   DevBuf<uint8_t> cnt_tmp;
   int64_t cnt_words = 0;  // padded words of cnt8
+  int64_t planned_t32 = 0, planned_cnt_tmp = 0, planned_miss = 0, planned_t64 = 0;
+  // phase B workspaces (stager thread only)
+  DevBuf<int32_t> tiles32_b, owner_cnt, n_delta_dev;
+  DevBuf<uint64_t> tiles64, total64;
   // miss buffers (caller thread, one gather at a time)
   DevBuf<int32_t> miss_tmp_pos, miss_tmp_id, tile_miss, miss_pos, miss_id, n_miss;
   // pinned
-  int32_t* h_small = nullptr;  // readback scratch
-  int32_t* h_req = nullptr;    // request IDs (device -> host)
-  uint8_t* h_resp = nullptr;   // packed rows (host -> device), mode 0
+  int32_t* h_small = nullptr;    // phase A readback scratch
+  int32_t* h_small_b = nullptr;  // phase B readback scratch
+  int32_t* h_req = nullptr;      // request IDs (device -> host)
+  uint8_t* h_resp = nullptr;     // packed rows (host -> device), mode 0
   int32_t* h_seeds = nullptr;
   int64_t h_seeds_cap = 0, h_req_cap = 0, h_resp_cap = 0;
   uint64_t* h_kp = nullptr;
-  // streams / thread
-  cudaStream_t side = nullptr;
-  cudaEvent_t ev_a = nullptr, ev_b = nullptr;
+  // streams / threads
+  cudaStream_t side = nullptr;    // phase A: sample, frontier, unique
+  cudaStream_t side_b = nullptr;  // phase B: select, delta, bulk copies, carry
   cudaEvent_t ev_copy[2 * GG_MAX_PARTS] = {nullptr};
-  Window win[2];
+  Window win[3];
+  CacheSlot cslot[2];
   uint64_t stage_counter = 0;
-  bool have_prev = false;
-  int prev_slot = 0;
-  std::thread worker;
+  CacheSlot* prev_cs = nullptr;   // holds C_{k-1} for the next phase B (stager thread)
+  std::thread worker_a, worker_b;
   std::mutex mu;
-  std::condition_variable cv_job, cv_done;
-  std::deque<Window*> jobs;
+  std::condition_variable cv_a, cv_b, cv_done;
+  std::deque<Window*> jobs_a, jobs_b;
+  int busy = 0;                   // jobs queued or in flight
   bool stop = false;
   Pool* pool = nullptr;
 };
@@ -288,21 +305,17 @@ namespace gg {
 static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // caps derived from the fanouts (frontier_{h+1} <= frontier_h * (1 + f[h]), also <= N)
-static gg_status plan_and_alloc(gg_graph* g, Window* w) {
-  const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
-  int64_t cap_front[GG_MAX_LAYERS + 1];
+static void plan_caps(const gg_graph* g, int L, const int* fanouts, int64_t* cap_front) {
   cap_front[0] = g->cfg.max_batch;
   for (int h = 0; h < L; ++h) {
-    int64_t c = cap_front[h] * (1 + (int64_t)w->fanouts[h]);
+    int64_t c = cap_front[h] * (1 + (int64_t)fanouts[h]);
     if (c > g->N) c = g->N;
     if (g->cfg.max_input_nodes > 0 && c > g->cfg.max_input_nodes) c = g->cfg.max_input_nodes;
     if (c < cap_front[h]) c = cap_front[h];
     cap_front[h + 1] = c;
   }
-  w->node_pitch = ceil_div(cap_front[L], 4) * 4;
-  if ((int64_t)W * w->node_pitch >= (1ll << 31))
-    return fail(GG_ERR_CAPACITY, "W * max_input_nodes = %lld exceeds int32 indexing",
-                (long long)((int64_t)W * w->node_pitch));
+}
+
 #define ENS(buf, n)                                                                       \
   do {                                                                                    \
     if ((buf).ensure(n) != cudaSuccess) {                                                 \
@@ -310,18 +323,21 @@ static gg_status plan_and_alloc(gg_graph* g, Window* w) {
       return fail(GG_ERR_OOM, "device allocation of %lld elements failed (%s)", (long long)(n), #buf); \
     }                                                                                     \
   } while (0)
+
+// window-local arena (the arena is free: its previous tenant was released)
+static gg_status alloc_window(gg_graph* g, Window* w) {
+  const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
+  int64_t cap_front[GG_MAX_LAYERS + 1];
+  plan_caps(g, L, w->fanouts, cap_front);
+  w->node_pitch = ceil_div(cap_front[L], 4) * 4;
   ENS(w->nodes, (int64_t)W * w->node_pitch);
   ENS(w->n_front_dev, (int64_t)(GG_MAX_LAYERS + 1) * Wmax);
-  int64_t max_tiles = 1;
   for (int h = 0; h < L; ++h) {
     const int64_t ecap = (int64_t)W * cap_front[h] * w->fanouts[h];
-    if (ecap >= (1ll << 31))
-      return fail(GG_ERR_CAPACITY, "hop %d edge cap %lld exceeds int32 indexing", h, (long long)ecap);
     ENS(w->hop[h].blk_indptr, (int64_t)W * cap_front[h] + W);
     ENS(w->hop[h].src_global, ecap);
     ENS(w->hop[h].src_local, ecap);
     ENS(w->hop[h].edge_off_dev, W + 1);
-    max_tiles = std::max(max_tiles, ceil_div(cap_front[h], 256));
   }
   const int64_t ucap = std::min<int64_t>(g->N, (int64_t)W * w->node_pitch);
   ENS(w->uniq, ucap);
@@ -329,25 +345,53 @@ static gg_status plan_and_alloc(gg_graph* g, Window* w) {
   ENS(w->req_ids, std::max<int64_t>(g->cache_rows, 1));
   ENS(w->carry_src, std::max<int64_t>(g->cache_rows, 1));
   ENS(w->carry_ids, std::max<int64_t>(g->cache_rows, 1));
-  ENS(w->hot, std::max<int64_t>(g->cache_rows, 1));
   ENS(w->counters, (int64_t)Wmax * (2 + GG_MAX_PARTS));
-  ENS(g->cnt_tmp, (int64_t)W * cap_front[L - 1]);
+  return GG_OK;
+}
+
+// Shared scratch whose size depends on (W, fanouts).  Called from gg_window_stage on the caller
+// thread; grows only after both pipeline threads are idle and the device is quiet.
+static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bool* need_drain) {
+  int64_t cap_front[GG_MAX_LAYERS + 1];
+  plan_caps(g, L, fanouts, cap_front);
+  const int64_t node_pitch = ceil_div(cap_front[L], 4) * 4;
+  if ((int64_t)W * node_pitch >= (1ll << 31))
+    return fail(GG_ERR_CAPACITY, "W * max_input_nodes = %lld exceeds int32 indexing", (long long)((int64_t)W * node_pitch));
+  int64_t max_tiles = 1;
+  for (int h = 0; h < L; ++h) {
+    const int64_t ecap = (int64_t)W * cap_front[h] * fanouts[h];
+    if (ecap >= (1ll << 31))
+      return fail(GG_ERR_CAPACITY, "hop %d edge cap %lld exceeds int32 indexing", h, (long long)ecap);
+    max_tiles = std::max(max_tiles, ceil_div(cap_front[h], 256));
+  }
+  const int64_t ucap = std::min<int64_t>(g->N, (int64_t)W * node_pitch);
   int64_t t32 = std::max<int64_t>((int64_t)W * max_tiles, (int64_t)W * g->F.n_wtiles);
   t32 = std::max<int64_t>(t32, g->cnt_words / kWordTile);
-  t32 = std::max<int64_t>(t32, ceil_div(g->cache_rows, 1024) + 1);
+  const int64_t cnt_tmp = (int64_t)W * cap_front[L - 1];
+  const int64_t t64 = ceil_div(ucap, 1024) + 1;
+  const int64_t mcap = ceil_div(node_pitch, 64) * 64;
+  const bool grow = t32 > g->planned_t32 || cnt_tmp > g->planned_cnt_tmp || t64 > g->planned_t64 ||
+                    mcap > g->planned_miss;
+  if (!grow) return GG_OK;
+  if (need_drain) {
+    *need_drain = true;
+    return GG_OK;
+  }
   ENS(g->tiles32, t32);
-  ENS(g->tiles64, ceil_div(ucap, 1024) + 1);
-  // miss buffers are sized by the largest |N_b|
-  const int64_t mcap = ceil_div(w->node_pitch, 64) * 64;
+  ENS(g->cnt_tmp, cnt_tmp);
+  ENS(g->tiles64, t64);
   ENS(g->miss_tmp_pos, mcap);
   ENS(g->miss_tmp_id, mcap);
   ENS(g->tile_miss, mcap / 64);
   ENS(g->miss_pos, mcap);
   ENS(g->miss_id, mcap);
-#undef ENS
-  (void)cap_front;
+  g->planned_t32 = std::max(g->planned_t32, t32);
+  g->planned_cnt_tmp = std::max(g->planned_cnt_tmp, cnt_tmp);
+  g->planned_t64 = std::max(g->planned_t64, t64);
+  g->planned_miss = std::max(g->planned_miss, mcap);
   return GG_OK;
 }
+#undef ENS
 
 static gg_status ensure_pinned(void** p, int64_t* cap, int64_t want) {
   if (want <= *cap) return GG_OK;
@@ -363,21 +407,17 @@ static gg_status ensure_pinned(void** p, int64_t* cap, int64_t want) {
   return GG_OK;
 }
 
-}  // namespace gg
-
-namespace gg {
-
-// ---- the prefetcher's work for one window (runs on the prefetch thread, side stream) --------
-static gg_status stage_window(gg_graph* g, Window* w) {
+// ---- phase A (sampler thread, stream `side`): a-1, a-2, a-3 ---------------------------------
+static gg_status stage_a(gg_graph* g, Window* w) {
   const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
   cudaStream_t st = g->side;
   const double t0 = now_ms();
   CU(cudaSetDevice(g->device));
-  gg_status rc = plan_and_alloc(g, w);
+  gg_status rc = alloc_window(g, w);
   if (rc != GG_OK) return rc;
-  Window* prev = g->have_prev ? &g->win[g->prev_slot] : nullptr;
-  // the slot's previous tenant (window k-2) may still be read by gathers already enqueued
+  // the arena's previous tenant may still be read by gathers already enqueued
   if (w->gather_recorded) CU(cudaStreamWaitEvent(st, w->gather_done, 0));
+  w->gather_recorded = false;
 
   // seeds and per-(batch, layer) key prefixes -> device
   BatchOffsets seed_off;
@@ -457,13 +497,41 @@ static gg_status stage_window(gg_graph* g, Window* w) {
   g->prof.end(st, pe, GG_PROF_UNIQUE, 0);
   CU(cudaMemcpyAsync(g->h_small, g->stats.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CU(cudaMemcpyAsync(g->h_small + 1, g->hist.p, 256 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(w->sampled, st));
   CU(cudaStreamSynchronize(st));
   w->n_unique = g->h_small[0];
-  const int32_t* hist = g->h_small + 1;
+  std::memcpy(w->hist, g->h_small + 1, 256 * sizeof(int32_t));
   w->n_remote = 0;
-  for (int c = 1; c < 256; ++c) w->n_remote += hist[c];
-  const double t2 = now_ms();
-  w->ms_unique = (float)(t2 - t1);
+  for (int c = 1; c < 256; ++c) w->n_remote += w->hist[c];
+  if (g->prof.on) {
+    std::lock_guard<std::mutex> l(g->prof.m);
+    g->prof.bytes[GG_PROF_UNIQUE] += 4ll * w->n_access + 8ll * w->n_unique;
+  }
+  w->ms_unique = (float)(now_ms() - t1);
+  CU(cudaGetLastError());
+  return GG_OK;
+}
+
+// ---- phase B (stager thread, stream `side_b`): a-4, a-5, a-6 --------------------------------
+static gg_status stage_b(gg_graph* g, Window* w) {
+  const int Wmax = g->cfg.max_window;
+  cudaStream_t st = g->side_b;
+  CU(cudaSetDevice(g->device));
+  CacheSlot* cs = w->cs;
+  // The slot still belongs to window seq-2 until the caller releases it (its batches may still
+  // be gathered).  Alg. 1 has the same order: the cache for k+1 is warmed while k trains.
+  {
+    std::unique_lock<std::mutex> l(g->mu);
+    g->cv_done.wait(l, [&] {
+      Window* t = cs->tenant;
+      return g->stop || !t || t->seq + 2 != w->seq || !t->live;
+    });
+    if (g->stop) return fail(GG_ERR_STATE, "graph is being destroyed");
+  }
+  const double t0 = now_ms();
+  CU(cudaStreamWaitEvent(st, w->sampled, 0));
+  if (cs->tenant && cs->tenant->gather_recorded) CU(cudaStreamWaitEvent(st, cs->tenant->gather_done, 0));
+  CacheSlot* prev = g->prev_cs;
 
   // a-4 hot set: threshold t and quota of count == t nodes from the histogram
   int32_t thr = 0;
@@ -476,43 +544,41 @@ static gg_status stage_window(gg_graph* g, Window* w) {
     w->may_miss = true;
     int64_t above = 0;
     for (thr = 255; thr >= 1; --thr) {
-      if (above + hist[thr] > w->n_hot) break;
-      above += hist[thr];
+      if (above + w->hist[thr] > w->n_hot) break;
+      above += w->hist[thr];
     }
     quota = (uint32_t)(w->n_hot - above);
   }
-  pe = g->prof.begin(st);
-  launch_slots_clear(st, w->hot.p, (int)w->n_cached, w->slot_map);
-  w->n_cached = 0;
+  cudaEvent_t pe = g->prof.begin(st);
+  launch_slots_clear(st, cs->hot.p, (int)cs->n_cached, cs->slot_map);
+  cs->n_cached = 0;
   if (w->n_hot > 0)
-    launch_hot_select(st, w->uniq.p, w->cnt.p, (int)w->n_unique, g->R, thr, quota, g->tiles64.p, g->total64.p, w->hot.p);
+    launch_hot_select(st, w->uniq.p, w->cnt.p, (int)w->n_unique, g->R, thr, quota, g->tiles64.p, g->total64.p, cs->hot.p);
   // a-5 delta against C_{k-1}
   const int carry = (g->cfg.carry_over && prev) ? 1 : 0;
-  launch_delta_split(st, w->hot.p, (int)w->n_hot, g->R, prev ? prev->slot_map : nullptr, carry, g->tiles32.p,
-                     g->n_delta_dev.p, g->owner_cnt.p, w->slot_map, w->req_ids.p, w->carry_src.p, w->carry_ids.p);
-  w->n_cached = w->n_hot;
+  launch_delta_split(st, cs->hot.p, (int)w->n_hot, g->R, prev ? prev->slot_map : nullptr, carry, g->tiles32_b.p,
+                     g->n_delta_dev.p, g->owner_cnt.p, cs->slot_map, w->req_ids.p, w->carry_src.p, w->carry_ids.p);
+  cs->n_cached = w->n_hot;
+  cs->tenant = w;
   g->prof.end(st, pe, GG_PROF_SELECT, 12ll * w->n_unique);
-  if (g->prof.on) {
-    std::lock_guard<std::mutex> l(g->prof.m);
-    g->prof.bytes[GG_PROF_UNIQUE] += 4ll * w->n_access + 8ll * w->n_unique;
-  }
-  CU(cudaMemcpyAsync(g->h_small, g->owner_cnt.p, 2 * GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-  CU(cudaMemcpyAsync(g->h_small + 2 * GG_MAX_PARTS, g->n_delta_dev.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  int32_t* hs = g->h_small_b;
+  CU(cudaMemcpyAsync(hs, g->owner_cnt.p, 2 * GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(hs + 2 * GG_MAX_PARTS, g->n_delta_dev.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
-  w->n_delta = w->n_hot > 0 ? g->h_small[2 * GG_MAX_PARTS] : 0;
+  w->n_delta = w->n_hot > 0 ? hs[2 * GG_MAX_PARTS] : 0;
   w->n_carry = w->n_hot - w->n_delta;
   for (int m = 0; m < GG_MAX_PARTS; ++m) {
-    w->staged[m] = w->n_hot > 0 ? g->h_small[m] : 0;
-    w->bulk[m] = w->n_hot > 0 ? g->h_small[GG_MAX_PARTS + m] : 0;
+    w->staged[m] = w->n_hot > 0 ? hs[m] : 0;
+    w->bulk[m] = w->n_hot > 0 ? hs[GG_MAX_PARTS + m] : 0;
   }
-  const double t3 = now_ms();
-  w->ms_select = (float)(t3 - t2);
+  const double t1 = now_ms();
+  w->ms_select = (float)(t1 - t0);
 
   // a-6 staging: one bulk transfer per owner into that owner's contiguous slot range
   w->bulk_copies = 0;
   w->ms_pack = 0;
   const int64_t rb = g->rb;
-  CU(cudaEventRecord(g->ev_a, st));
+  gg_status rc;
   if (g->cfg.staging_mode == 0 && w->n_delta > 0) {
     void* pr = g->h_req;
     rc = ensure_pinned(&pr, &g->h_req_cap, w->n_delta * (int64_t)sizeof(int32_t));
@@ -524,7 +590,6 @@ static gg_status stage_window(gg_graph* g, Window* w) {
     if (rc != GG_OK) return rc;
     CU(cudaMemcpyAsync(g->h_req, w->req_ids.p, (size_t)w->n_delta * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
-    CU(cudaEventRecord(g->ev_a, st));
     int64_t q0 = 0;
     for (int m = 0; m < g->R.P; ++m) {
       const int64_t nm = w->bulk[m];
@@ -543,7 +608,7 @@ static gg_status stage_window(gg_graph* g, Window* w) {
       });
       w->ms_pack += (float)(now_ms() - p0);
       CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));
-      CU(cudaMemcpyAsync(w->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, st));
+      CU(cudaMemcpyAsync(cs->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, st));
       CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies + 1], st));
       w->bulk_copies += 1;
       q0 += nm;
@@ -555,17 +620,19 @@ static gg_status stage_window(gg_graph* g, Window* w) {
       const int64_t nm = w->bulk[m];
       if (nm == 0) continue;
       CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));
-      launch_rows_from_store(st, w->req_ids.p + q0, (int)nm, g->store, g->R, w->cache, q0, rb, (int)rb);
+      launch_rows_from_store(st, w->req_ids.p + q0, (int)nm, g->store, g->R, cs->cache, q0, rb, (int)rb);
       CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies + 1], st));
       w->bulk_copies += 1;
       q0 += nm;
     }
   }
-  CU(cudaEventRecord(g->ev_b, st));
-  pe = g->prof.begin(st);
   // carried rows: D2D out of the previous buffer, after the delta rows
+  pe = g->prof.begin(st);
+  cudaEvent_t carry_a = g->ev_copy[2 * GG_MAX_PARTS - 2], carry_b = g->ev_copy[2 * GG_MAX_PARTS - 1];
+  CU(cudaEventRecord(carry_a, st));
   if (w->n_carry > 0)
-    launch_rows_from_list(st, w->carry_src.p, (int)w->n_carry, prev->cache, rb, w->cache, w->n_delta, rb, (int)rb);
+    launch_rows_from_list(st, w->carry_src.p, (int)w->n_carry, prev->cache, rb, cs->cache, w->n_delta, rb, (int)rb);
+  CU(cudaEventRecord(carry_b, st));
   g->prof.end(st, pe, GG_PROF_CARRY, 2ll * w->n_carry * rb);
   CU(cudaMemsetAsync(w->counters.p, 0, (size_t)Wmax * (2 + GG_MAX_PARTS) * sizeof(int32_t), st));
   CU(cudaEventRecord(w->ready, st));
@@ -576,45 +643,72 @@ static gg_status stage_window(gg_graph* g, Window* w) {
     cudaEventElapsedTime(&ms, g->ev_copy[2 * c], g->ev_copy[2 * c + 1]);
     w->ms_h2d += ms;
   }
-  ms = w->ms_h2d;
   if (g->prof.on && w->n_delta > 0) {
     std::lock_guard<std::mutex> l(g->prof.m);
-    g->prof.ms[GG_PROF_STAGE_COPY] += ms;
+    g->prof.ms[GG_PROF_STAGE_COPY] += w->ms_h2d;
     g->prof.regions[GG_PROF_STAGE_COPY] += w->bulk_copies;
     g->prof.bytes[GG_PROF_STAGE_COPY] += w->n_delta * rb;
   }
-  cudaEventElapsedTime(&ms, g->ev_b, w->ready);
+  cudaEventElapsedTime(&ms, carry_a, carry_b);
   w->ms_carry = ms;
   CU(cudaGetLastError());
-  g->have_prev = true;
-  g->prev_slot = w->slot;
-  w->ms_total = (float)(now_ms() - t0);
+  g->prev_cs = cs;
+  w->ms_total = w->ms_sample + w->ms_unique + (float)(now_ms() - t0);
   return GG_OK;
 }
 
-static void worker_main(gg_graph* g) {
+static void finish_job(gg_graph* g, Window* w, gg_status rc) {
+  {
+    std::lock_guard<std::mutex> l(g->mu);
+    w->status = rc;
+    if (rc != GG_OK) w->error = t_err;
+    w->enqueued = true;
+    g->busy -= 1;
+  }
+  g->cv_done.notify_all();
+}
+
+static void worker_a_main(gg_graph* g) {
   cudaSetDevice(g->device);
   for (;;) {
     Window* w;
     {
       std::unique_lock<std::mutex> l(g->mu);
-      g->cv_job.wait(l, [&] { return g->stop || !g->jobs.empty(); });
-      if (g->jobs.empty()) return;
-      w = g->jobs.front();
-      g->jobs.pop_front();
+      g->cv_a.wait(l, [&] { return g->stop || !g->jobs_a.empty(); });
+      if (g->jobs_a.empty()) return;
+      w = g->jobs_a.front();
+      g->jobs_a.pop_front();
     }
-    gg_status rc = stage_window(g, w);
+    gg_status rc = stage_a(g, w);
+    if (rc != GG_OK) {
+      finish_job(g, w, rc);
+      continue;
+    }
     {
       std::lock_guard<std::mutex> l(g->mu);
-      w->status = rc;
-      if (rc != GG_OK) w->error = t_err;
-      w->enqueued = true;
+      g->jobs_b.push_back(w);
     }
-    g->cv_done.notify_all();
+    g->cv_b.notify_one();
+  }
+}
+
+static void worker_b_main(gg_graph* g) {
+  cudaSetDevice(g->device);
+  for (;;) {
+    Window* w;
+    {
+      std::unique_lock<std::mutex> l(g->mu);
+      g->cv_b.wait(l, [&] { return g->stop || !g->jobs_b.empty(); });
+      if (g->jobs_b.empty()) return;
+      w = g->jobs_b.front();
+      g->jobs_b.pop_front();
+    }
+    finish_job(g, w, stage_b(g, w));
   }
 }
 
 }  // namespace gg
+
 
 // =================================== C ABI ====================================================
 extern "C" {
@@ -645,32 +739,38 @@ static bool is_pinned_ptr(const void* p) {
 
 gg_status gg_graph_destroy(gg_graph* g) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
-  if (g->worker.joinable()) {
-    {
-      std::lock_guard<std::mutex> l(g->mu);
-      g->stop = true;
-    }
-    g->cv_job.notify_all();
-    g->worker.join();
+  {
+    std::lock_guard<std::mutex> l(g->mu);
+    g->stop = true;
   }
+  g->cv_a.notify_all();
+  g->cv_b.notify_all();
+  g->cv_done.notify_all();
+  if (g->worker_a.joinable()) g->worker_a.join();
+  if (g->worker_b.joinable()) g->worker_b.join();
   cudaSetDevice(g->device);
   cudaDeviceSynchronize();
   delete g->pool;
   g->prof.destroy();
-  for (int s = 0; s < 2; ++s) {
+  for (int s = 0; s < 3; ++s) {
     Window& w = g->win[s];
     w.nodes.release(); w.n_front_dev.release(); w.uniq.release(); w.cnt.release();
     w.req_ids.release(); w.carry_src.release(); w.carry_ids.release(); w.counters.release();
-    w.hot.release();
     for (int h = 0; h < GG_MAX_LAYERS; ++h) {
       w.hop[h].blk_indptr.release(); w.hop[h].src_global.release();
       w.hop[h].src_local.release(); w.hop[h].edge_off_dev.release();
     }
-    if (w.cache) cudaFree(w.cache);
-    if (w.slot_map) cudaFree(w.slot_map);
+    if (w.sampled) cudaEventDestroy(w.sampled);
     if (w.ready) cudaEventDestroy(w.ready);
     if (w.gather_done) cudaEventDestroy(w.gather_done);
   }
+  for (int s = 0; s < 2; ++s) {
+    CacheSlot& c = g->cslot[s];
+    c.hot.release();
+    if (c.cache) cudaFree(c.cache);
+    if (c.slot_map) cudaFree(c.slot_map);
+  }
+  g->tiles32_b.release();
   g->seen.release(); g->newbits.release(); g->cnt8.release(); g->wprefix.release();
   g->seed_perm.release(); g->tiles32.release(); g->totals.release(); g->stats.release();
   g->hist.release(); g->owner_cnt.release(); g->n_delta_dev.release(); g->err_flag.release();
@@ -678,14 +778,14 @@ gg_status gg_graph_destroy(gg_graph* g) {
   g->cnt_tmp.release(); g->miss_tmp_pos.release(); g->miss_tmp_id.release(); g->tile_miss.release();
   g->miss_pos.release(); g->miss_id.release(); g->n_miss.release();
   if (g->h_small) cudaFreeHost(g->h_small);
+  if (g->h_small_b) cudaFreeHost(g->h_small_b);
   if (g->h_req) cudaFreeHost(g->h_req);
   if (g->h_resp) cudaFreeHost(g->h_resp);
   if (g->h_seeds) cudaFreeHost(g->h_seeds);
   if (g->h_kp) cudaFreeHost(g->h_kp);
-  if (g->ev_a) cudaEventDestroy(g->ev_a);
-  if (g->ev_b) cudaEventDestroy(g->ev_b);
   for (int c = 0; c < 2 * GG_MAX_PARTS; ++c) if (g->ev_copy[c]) cudaEventDestroy(g->ev_copy[c]);
   if (g->side) cudaStreamDestroy(g->side);
+  if (g->side_b) cudaStreamDestroy(g->side_b);
   delete g;
   return GG_OK;
 }
@@ -777,17 +877,23 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   CUC(g->seeds_dev.ensure((int64_t)Wmax * cfg->max_batch));
   CUC(g->key_prefix.ensure((int64_t)GG_MAX_LAYERS * Wmax));
   CUC(cudaHostAlloc((void**)&g->h_small, 4096 * sizeof(int32_t), cudaHostAllocDefault));
+  CUC(cudaHostAlloc((void**)&g->h_small_b, 4096 * sizeof(int32_t), cudaHostAllocDefault));
+  CUC(g->tiles32_b.ensure(ceil_div(std::max<int64_t>(g->cache_rows, 1), 1024) + 2));
   CUC(cudaHostAlloc((void**)&g->h_seeds, (size_t)Wmax * cfg->max_batch * sizeof(int32_t), cudaHostAllocDefault));
   CUC(cudaHostAlloc((void**)&g->h_kp, (size_t)GG_MAX_LAYERS * Wmax * sizeof(uint64_t), cudaHostAllocDefault));
   CUC(cudaStreamCreateWithFlags(&g->side, cudaStreamNonBlocking));
-  CUC(cudaEventCreate(&g->ev_a)); CUC(cudaEventCreate(&g->ev_b));
+  CUC(cudaStreamCreateWithFlags(&g->side_b, cudaStreamNonBlocking));
   for (int c = 0; c < 2 * GG_MAX_PARTS; ++c) CUC(cudaEventCreate(&g->ev_copy[c]));
   for (int s = 0; s < 2; ++s) {
+    CacheSlot& c = g->cslot[s];
+    CUC(cudaMalloc((void**)&c.cache, (size_t)std::max<int64_t>(g->cache_rows, 1) * rb));
+    CUC(cudaMalloc((void**)&c.slot_map, (size_t)g->N * sizeof(int32_t)));
+    CUC(c.hot.ensure(std::max<int64_t>(g->cache_rows, 1)));
+    launch_fill_i32(0, c.slot_map, g->N, -1);
+  }
+  for (int s = 0; s < 3; ++s) {
     Window& w = g->win[s];
-    w.slot = s;
-    CUC(cudaMalloc((void**)&w.cache, (size_t)std::max<int64_t>(g->cache_rows, 1) * rb));
-    CUC(cudaMalloc((void**)&w.slot_map, (size_t)g->N * sizeof(int32_t)));
-    launch_fill_i32(0, w.slot_map, g->N, -1);
+    CUC(cudaEventCreateWithFlags(&w.sampled, cudaEventDisableTiming));
     CUC(cudaEventCreateWithFlags(&w.ready, cudaEventDefault));
     CUC(cudaEventCreateWithFlags(&w.gather_done, cudaEventDisableTiming));
   }
@@ -795,7 +901,8 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
 #undef CUC
   int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(1u, std::thread::hardware_concurrency()));
   g->pool = new Pool(nt > 1 ? nt : 0);
-  g->worker = std::thread(worker_main, g);
+  g->worker_a = std::thread(worker_a_main, g);
+  g->worker_b = std::thread(worker_b_main, g);
   *out = g;
   return GG_OK;
 }
@@ -804,7 +911,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
 
 namespace gg {
 static Window* find_window(gg_graph* g, int64_t id) {
-  for (int s = 0; s < 2; ++s)
+  for (int s = 0; s < 3; ++s)
     if (g->win[s].live && g->win[s].id == id) return &g->win[s];
   return nullptr;
 }
@@ -813,6 +920,15 @@ static gg_status wait_enqueued(gg_graph* g, Window* w) {
   const double t0 = now_ms();
   std::unique_lock<std::mutex> l(g->mu);
   if (!w->enqueued) {
+    // window k+2's cache buffer is window k's: it cannot be built before k is released
+    Window* t = w->cs ? w->cs->tenant : nullptr;
+    for (int s = 0; s < 3; ++s) {
+      Window* o = &g->win[s];
+      if (o != w && o->live && o->seq + 2 == w->seq)
+        return fail(GG_ERR_STATE, "window %lld shares its cache buffer with live window %lld: release that one first",
+                    (long long)w->id, (long long)o->id);
+    }
+    (void)t;
     g->cv_done.wait(l, [&] { return w->enqueued; });
     w->ms_wait += (float)(now_ms() - t0);
   }
@@ -863,10 +979,24 @@ gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_i
   for (int64_t i = 0; i < S; ++i)
     if (seeds[i] < 0 || seeds[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "seed %lld = %d outside [0, N)", (long long)i, seeds[i]);
   if (find_window(g, window_id)) return fail(GG_ERR_STATE, "window %lld is already live", (long long)window_id);
-  Window* w = &g->win[g->stage_counter & 1];
-  if (w->live) return fail(GG_ERR_STATE, "two windows are live; release window %lld first", (long long)w->id);
-  if (g->win[0].live && g->win[1].live) return fail(GG_ERR_STATE, "two windows are live");
+  Window* w = &g->win[g->stage_counter % 3];
+  if (w->live) return fail(GG_ERR_STATE, "three windows are live; release window %lld first", (long long)w->id);
+  // shared scratch sized by (W, fanouts): grow only with both pipeline threads idle
+  bool need_drain = false;
+  gg_status rc = ensure_shared(g, W, num_layers, fanouts, &need_drain);
+  if (rc != GG_OK) return rc;
+  if (need_drain) {
+    {
+      std::unique_lock<std::mutex> l(g->mu);
+      g->cv_done.wait(l, [&] { return g->busy == 0; });
+    }
+    CU(cudaDeviceSynchronize());
+    rc = ensure_shared(g, W, num_layers, fanouts, nullptr);
+    if (rc != GG_OK) return rc;
+  }
   w->id = window_id; w->live = true; w->W = W; w->L = num_layers; w->first_batch = first_batch_index;
+  w->seq = g->stage_counter;
+  w->cs = &g->cslot[g->stage_counter & 1];
   for (int h = 0; h < num_layers; ++h) w->fanouts[h] = fanouts[h];
   w->seeds.assign(seeds, seeds + S);
   w->boff.assign(batch_offsets, batch_offsets + W + 1);
@@ -874,10 +1004,11 @@ gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_i
   {
     std::lock_guard<std::mutex> l(g->mu);
     w->enqueued = false; w->status = GG_OK; w->error.clear();
-    g->jobs.push_back(w);
+    g->jobs_a.push_back(w);
+    g->busy += 1;
   }
   g->stage_counter += 1;
-  g->cv_job.notify_one();
+  g->cv_a.notify_one();
   return GG_OK;
 }
 
@@ -906,9 +1037,9 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CU(cudaStreamWaitEvent(st, w->ready, 0));
   GatherLaunch G;
-  G.nodes = w->nodes.p + (int64_t)b * w->node_pitch; G.n = n; G.slot_of = w->slot_map;
+  G.nodes = w->nodes.p + (int64_t)b * w->node_pitch; G.n = n; G.slot_of = w->cs->slot_map;
   G.local_base = g->store.base[g->R.local]; G.local_stride = g->store.stride;
-  G.cache_base = w->cache; G.cache_stride = g->rb;
+  G.cache_base = w->cs->cache; G.cache_stride = g->rb;
   G.out = (uint8_t*)out->features; G.rb = g->rb; G.R = g->R; G.store = g->store;
   G.may_miss = w->may_miss;
   G.miss_tmp_pos = g->miss_tmp_pos.p; G.miss_tmp_id = g->miss_tmp_id.p; G.tile_miss = g->tile_miss.p;
@@ -933,8 +1064,18 @@ gg_status gg_window_release(gg_graph* g, int64_t window_id) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
   Window* w = find_window(g, window_id);
   if (!w) return fail(GG_ERR_STATE, "window %lld is not live", (long long)window_id);
-  wait_enqueued(g, w);  // the prefetcher must be done touching the slot before it can be re-staged
-  w->live = false;
+  // the pipeline threads must be done with the arena before it can be re-staged
+  {
+    std::unique_lock<std::mutex> l(g->mu);
+    bool blocked = false;
+    if (!w->enqueued)
+      for (int s = 0; s < 3; ++s)
+        if (&g->win[s] != w && g->win[s].live && g->win[s].seq + 2 == w->seq) blocked = true;
+    if (blocked) return fail(GG_ERR_STATE, "release the older live window first");
+    g->cv_done.wait(l, [&] { return w->enqueued; });
+    w->live = false;
+  }
+  g->cv_done.notify_all();
   return GG_OK;
 }
 
@@ -981,7 +1122,7 @@ gg_status gg_window_export(gg_graph* g, int64_t window_id, int32_t what, int32_t
   switch (what) {
     case 0: src = w->uniq.p; n = w->n_unique; break;
     case 1: src = w->cnt.p; n = w->n_unique; break;
-    case 2: src = w->hot.p; n = w->n_hot; break;
+    case 2: src = w->cs->hot.p; n = w->n_hot; break;
     case 3: src = w->req_ids.p; n = w->n_delta; break;
     case 4: src = w->carry_ids.p; n = w->n_carry; break;
     default: return fail(GG_ERR_INVALID_ARG, "what = %d", what);
@@ -1002,9 +1143,9 @@ gg_status gg_cache_read(gg_graph* g, int64_t window_id, const int32_t* ids, int6
   for (int64_t i = 0; i < n; ++i) {
     if (ids[i] < 0 || ids[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "id out of range");
     int32_t s = -1;
-    CU(cudaMemcpy(&s, w->slot_map + ids[i], sizeof(int32_t), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(&s, w->cs->slot_map + ids[i], sizeof(int32_t), cudaMemcpyDeviceToHost));
     if (s < 0) return fail(GG_ERR_INVALID_ARG, "id %d is not cached in window %lld", ids[i], (long long)window_id);
-    CU(cudaMemcpy((uint8_t*)out + i * g->rb, w->cache + (int64_t)s * g->rb, (size_t)g->rb, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy((uint8_t*)out + i * g->rb, w->cs->cache + (int64_t)s * g->rb, (size_t)g->rb, cudaMemcpyDeviceToHost));
   }
   return GG_OK;
 }
@@ -1035,15 +1176,21 @@ uint64_t gg_launch_count(void) { return (uint64_t)g_launches.load(); }
 
 gg_status gg_cache_reset(gg_graph* g) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
-  if (g->win[0].live || g->win[1].live) return fail(GG_ERR_STATE, "release every window before gg_cache_reset");
+  if (g->win[0].live || g->win[1].live || g->win[2].live)
+    return fail(GG_ERR_STATE, "release every window before gg_cache_reset");
+  {
+    std::unique_lock<std::mutex> l(g->mu);
+    g->cv_done.wait(l, [&] { return g->busy == 0; });
+  }
   CU(cudaDeviceSynchronize());
   for (int s = 0; s < 2; ++s) {
-    Window& w = g->win[s];
-    launch_slots_clear(g->side, w.hot.p, (int)w.n_cached, w.slot_map);
-    w.n_cached = 0;
+    CacheSlot& c = g->cslot[s];
+    launch_slots_clear(g->side_b, c.hot.p, (int)c.n_cached, c.slot_map);
+    c.n_cached = 0;
+    c.tenant = nullptr;
   }
-  CU(cudaStreamSynchronize(g->side));
-  g->have_prev = false;
+  CU(cudaStreamSynchronize(g->side_b));
+  g->prev_cs = nullptr;
   return GG_OK;
 }
 

@@ -67,16 +67,63 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
   if (threadIdx.x == 0) totals[b] = carry_s;
 }
 
+// One 32-key step of the threshold pass: lane evaluates the key of position j (state x =
+// hdst + (j+1)*gamma) and the warp appends the keys that pass to the candidate buffer in
+// ascending position.  Only the key's HIGH word is formed for the test (the low word is
+// finished for the few keys that pass); FULL switches to the exact 64-bit test, which the
+// bisection falls back to only if two thresholds ever share a high word.
+template <bool FULL>
+__device__ __forceinline__ void select_step(uint64_t x, uint32_t j, uint32_t deg, uint64_t T,
+                                            int& cnt, uint64_t* s_key, int32_t* s_pos) {
+  uint64_t z = x;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  const uint32_t zh = (uint32_t)(z >> 32);
+  bool p;
+  if (FULL) p = (j < deg) && ((z ^ (z >> 31)) <= T);
+  else p = (j < deg) && ((zh ^ (zh >> 31)) <= (uint32_t)(T >> 32));
+  const unsigned m = __ballot_sync(0xffffffffu, p);
+  if (m) {
+    if (p) {
+      const int q = cnt + __popc(m & lanemask_lt());
+      if (q < kCand) {
+        s_key[q] = z ^ (z >> 31);
+        s_pos[q] = (int32_t)j;
+      }
+    }
+    cnt += __popc(m);
+  }
+}
+
+template <bool FULL>
+__device__ __forceinline__ int select_pass(uint64_t hdst, uint32_t deg, uint64_t T,
+                                           uint64_t* s_key, int32_t* s_pos) {
+  const uint32_t lane = threadIdx.x & 31;
+  int cnt = 0;
+  uint64_t x = hdst + (uint64_t)(lane + 1) * kGamma;
+  uint32_t j = lane;
+  // two independent key chains per lane per iteration
+  for (uint32_t j0 = 0; j0 < deg; j0 += 64) {
+    select_step<FULL>(x, j, deg, T, cnt, s_key, s_pos);
+    select_step<FULL>(x + 32 * kGamma, j + 32, deg, T, cnt, s_key, s_pos);
+    x += 64 * kGamma;
+    j += 64;
+  }
+  return cnt;
+}
+
 // Exact top-f of `deg` keyed positions by one warp.  Writes the kept positions' neighbor ids,
 // ascending in position, to out[0..f).
-__device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int64_t deg, int f,
+__device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int64_t deg64, int f,
                                             uint64_t hdst, uint64_t* s_key, int32_t* s_pos,
                                             int32_t* __restrict__ out) {
   const int lane = threadIdx.x & 31;
-  // slack so that a Binomial(deg, (f+slack)/deg) count falls below f with prob < ~1e-6
-  const int want = f + 8 + (int)(5.0f * sqrtf((float)f));
+  const uint32_t deg = (uint32_t)deg64;
+  // candidates wanted: f plus a slack so that a Binomial(deg, want/deg) count falls below f
+  // with probability ~3e-4 (a miss only costs one more pass)
+  const int want = f + 6 + (int)(4.0f * sqrtf((float)f));
   int cnt;
-  if (deg <= (want > 64 ? want : 64)) {
+  if (deg <= (uint32_t)want) {
     // small row: every position is a candidate
     cnt = (int)deg;
     for (int j = lane; j < cnt; j += 32) {
@@ -86,29 +133,13 @@ __device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int
   } else {
     // threshold guess: keys are uniform, so the f-th smallest is near f/deg * 2^64.  The
     // threshold only prunes; the exact rank below decides, so its rounding is immaterial.
-    uint64_t T = (uint64_t)((double)want / (double)deg * 18446744073709551616.0);
-    uint64_t lo = 0, hi = ~0ull;  // count(lo) < f known; count(hi) > kCand known (or hi = max)
-    bool have_hi = false;
+    uint64_t T = (uint64_t)((float)want / (float)deg * 18446744073709551616.0f);
+    T |= 0xffffffffull;
+    uint64_t lo = 0, hi = ~0ull;  // count(lo) < f known; count(hi) > kCand known once have_hi
+    bool have_hi = false, full = false;
     for (;;) {
-      cnt = 0;
-      for (int64_t j0 = 0; j0 < deg; j0 += 32) {
-        const int64_t j = j0 + lane;
-        uint64_t k = 0;
-        bool p = false;
-        if (j < deg) {
-          k = key_edge(hdst, (uint64_t)j);
-          p = k <= T;
-        }
-        const unsigned m = __ballot_sync(0xffffffffu, p);
-        if (p) {
-          const int q = cnt + __popc(m & lanemask_lt());
-          if (q < kCand) {
-            s_key[q] = k;
-            s_pos[q] = (int32_t)j;
-          }
-        }
-        cnt += __popc(m);
-      }
+      cnt = full ? select_pass<true>(hdst, deg, T, s_key, s_pos)
+                 : select_pass<false>(hdst, deg, T, s_key, s_pos);
       if (cnt >= f && cnt <= kCand) break;
       if (cnt < f) {
         lo = T;
@@ -118,23 +149,23 @@ __device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int
         have_hi = true;
         T = lo + ((hi - lo) >> 1);
       }
+      if (have_hi && (hi >> 32) == (lo >> 32)) full = true;  // high words can no longer separate
+      if (!full) T |= 0xffffffffull;
     }
   }
   __syncwarp();
   // exact rank among candidates under (key, position); candidates are in ascending position
+  typedef unsigned __int128 u128;
   int emitted = 0;
   for (int i0 = 0; i0 < cnt; i0 += 32) {
     const int i = i0 + lane;
     bool keep = false;
     int32_t pos = 0;
     if (i < cnt) {
-      const uint64_t ki = s_key[i];
       pos = s_pos[i];
+      const u128 mine = ((u128)s_key[i] << 32) | (uint32_t)pos;
       int rank = 0;
-      for (int c = 0; c < cnt; ++c) {
-        const uint64_t kc = s_key[c];
-        rank += (kc < ki) || (kc == ki && s_pos[c] < pos);
-      }
+      for (int c = 0; c < cnt; ++c) rank += ((((u128)s_key[c]) << 32) | (uint32_t)s_pos[c]) < mine;
       keep = rank < f;
     }
     const unsigned m = __ballot_sync(0xffffffffu, keep);

@@ -1,6 +1,10 @@
 """Epoch driver over the C ABI: the pipelined loop of Algorithm 1.
 
-    stage(0); for k: stage(k+1); gather every batch of window k; release(k)
+    stage(0) .. stage(d-1); for k: stage(k+d); gather every batch of window k; release(k)
+
+with lookahead d = 2 by default: while window k is served, window k+1's cache is being staged
+(select / delta / bulk copies) and window k+2 is being sampled (the library runs the two phases
+on two threads and two side streams).  d = 1 is the literal loop of Algorithm 1.
 
 Pure call sequencing -- all computation happens in libgreengnn.so.  `on_batch` receives every
 gathered batch (used by the parity tests and by the end-to-end bench leg).
@@ -34,19 +38,22 @@ def windows_of(n_batches: int, W: int) -> List[range]:
 def run_epoch(g: Graph, batches: Sequence[np.ndarray], fanouts: Sequence[int], W: int,
               features: torch.Tensor, on_batch: Optional[Callable[[int, int, int, Dict], None]] = None,
               on_window: Optional[Callable[[int, range], None]] = None,
-              stream: Optional[torch.cuda.Stream] = None, first_window_id: int = 0) -> int:
+              stream: Optional[torch.cuda.Stream] = None, first_window_id: int = 0,
+              lookahead: int = 2) -> int:
     """One epoch.  Returns the number of gather launches issued.  `features` is the caller's
     [capacity_rows, dim] device buffer reused for every batch."""
     wins = windows_of(len(batches), W)
     if not wins:
         return 0
     wid = first_window_id
-    g.window_stage(wid, wins[0].start, [batches[i] for i in wins[0]], fanouts)
+    assert 1 <= lookahead <= 2
+    for k in range(min(lookahead, len(wins))):
+        g.window_stage(wid + k, wins[k].start, [batches[i] for i in wins[k]], fanouts)
     n = 0
     for k, win in enumerate(wins):
-        if k + 1 < len(wins):
-            nxt = wins[k + 1]
-            g.window_stage(wid + k + 1, nxt.start, [batches[i] for i in nxt], fanouts)
+        if k + lookahead < len(wins):
+            nxt = wins[k + lookahead]
+            g.window_stage(wid + k + lookahead, nxt.start, [batches[i] for i in nxt], fanouts)
         for j, bi in enumerate(win):
             r = g.batch_gather(wid + k, j, features, stream)
             n += 1

@@ -70,6 +70,24 @@ def test_large_mini_directed_bf16(workload, dev):
     pu.check_epoch(w, W=4, n_hot=11250, staging_mode=1)
 
 
+def test_lookahead_one_is_algorithm_1_literal(workload, dev):
+    """stage(k+1) / serve k (Alg. 1) gives the same results as the deeper pipeline."""
+    from paper_2606_02916_b200 import epoch as ep
+    w = workload("small", dev)
+    outs = []
+    for la in (1, 2):
+        g = ep.graph_from_workload(w, n_hot=7500, max_window=4)
+        feats = torch.empty(w.num_nodes, w.dim, dtype=w.dtype, device=dev)
+        got = []
+        ep.run_epoch(g, w.batches, w.fanouts, 4, feats, lookahead=la,
+                     on_batch=lambda k, j, bi, r: got.append((r["input_nodes"].cpu().numpy().copy(),
+                                                              r["features"].cpu().clone(), g.misses(r)[0].copy())))
+        outs.append(got)
+        g.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a[0], b[0]) and torch.equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
 def test_determinism_two_epochs_identical(workload, dev):
     from paper_2606_02916_b200 import epoch as ep
     w = workload("small", dev)
@@ -112,11 +130,17 @@ def test_error_codes(workload, dev):
         g.batch_gather(0, 0, feats)                                          # buffer too small
     assert e.value.status == binding.GG_ERR_CAPACITY
     g.window_stage(1, 2, w.batches[2:4], w.fanouts)
+    g.window_stage(2, 4, w.batches[:1], w.fanouts)
     with pytest.raises(binding.GreenGNNError) as e:
-        g.window_stage(2, 4, w.batches[:1], w.fanouts)                       # third live window
+        g.window_stage(3, 5, w.batches[:1], w.fanouts)                       # fourth live window
+    assert e.value.status == binding.GG_ERR_STATE
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.batch_info(2, 0)              # window 2 shares its cache buffer with live window 0
     assert e.value.status == binding.GG_ERR_STATE
     g.window_release(0)
+    assert g.batch_info(2, 0)["n_input"] > 0
     g.window_release(1)
+    g.window_release(2)
     with pytest.raises(binding.GreenGNNError) as e:
         g.window_release(1)
     assert e.value.status == binding.GG_ERR_STATE
