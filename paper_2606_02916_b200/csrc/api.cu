@@ -8,6 +8,9 @@
 //                   caller's stream serves the previous window ("Parallel with training", l.8)
 // Two window slots ping-pong (slot = stage counter & 1): each holds the window's blocks, its
 // cache buffer, its ID->slot map and the list of cached IDs (= C_k).
+#include <emmintrin.h>
+#include <xmmintrin.h>
+
 #include <algorithm>
 #include <atomic>
 #include <chrono>
@@ -512,6 +515,31 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   return GG_OK;
 }
 
+// Owner-service pack of rows [i0, i1): response row i <- store row of ids[i].  Destination rows
+// are written with non-temporal stores (no read-for-ownership of a buffer the CPU never reads
+// again: the DMA engine is its only consumer) and the next source rows are prefetched, since
+// the requested IDs scatter over the owner's store.
+static void pack_rows(uint8_t* resp, const uint8_t* base, const int32_t* ids, int64_t lo, int64_t stride,
+                      int64_t rb, int64_t i0, int64_t i1) {
+  const bool nt = (rb % 16 == 0) && (((uintptr_t)resp) % 16 == 0);
+  const int64_t ahead = 6;
+  for (int64_t i = i0; i < i1; ++i) {
+    if (i + ahead < i1) {
+      const uint8_t* nx = base + (ids[i + ahead] - lo) * stride;
+      for (int64_t k = 0; k < rb; k += 64) _mm_prefetch((const char*)(nx + k), _MM_HINT_T0);
+    }
+    const uint8_t* src = base + (ids[i] - lo) * stride;
+    uint8_t* dst = resp + i * rb;
+    if (nt) {
+      for (int64_t k = 0; k < rb; k += 16)
+        _mm_stream_si128((__m128i*)(dst + k), _mm_loadu_si128((const __m128i*)(src + k)));
+    } else {
+      std::memcpy(dst, src, (size_t)rb);
+    }
+  }
+  if (nt) _mm_sfence();
+}
+
 // ---- phase B (stager thread, stream `side_b`): a-4, a-5, a-6 --------------------------------
 static gg_status stage_b(gg_graph* g, Window* w) {
   const int Wmax = g->cfg.max_window;
@@ -602,9 +630,7 @@ static gg_status stage_b(gg_graph* g, Window* w) {
       uint8_t* resp = g->h_resp + q0 * rb;
       const int64_t chunk = 512;
       g->pool->parallel_for(ceil_div(nm, chunk), [&](int64_t c) {
-        const int64_t i1 = std::min(nm, (c + 1) * chunk);
-        for (int64_t i = c * chunk; i < i1; ++i)
-          std::memcpy(resp + i * rb, base + (ids[i] - lo) * stride, (size_t)rb);
+        pack_rows(resp, base, ids, lo, stride, rb, c * chunk, std::min(nm, (c + 1) * chunk));
       });
       w->ms_pack += (float)(now_ms() - p0);
       CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));

@@ -67,21 +67,41 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
   if (threadIdx.x == 0) totals[b] = carry_s;
 }
 
-// One 32-key step of the threshold pass: lane evaluates the key of position j (state x =
-// hdst + (j+1)*gamma) and the warp appends the keys that pass to the candidate buffer in
-// ascending position.  Only the key's HIGH word is formed for the test (the low word is
-// finished for the few keys that pass); FULL switches to the exact 64-bit test, which the
-// bisection falls back to only if two thresholds ever share a high word.
-template <bool FULL>
-__device__ __forceinline__ void select_step(uint64_t x, uint32_t j, uint32_t deg, uint64_t T,
-                                            int& cnt, uint64_t* s_key, int32_t* s_pos) {
-  uint64_t z = x;
-  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-  const uint32_t zh = (uint32_t)(z >> 32);
+// ---- the hot loop: one key per lane per step -------------------------------------------------
+// The sampler is bound by the integer ALU pipe (LOP3 / SHF / ISETP issue at half the rate of the
+// FMA pipe that runs IMAD), so the step below is written to keep ALU-pipe instructions per key low:
+//   * the state h + (j+1)*gamma is formed from j with IMAD.WIDE (FMA pipe), not carried adds;
+//   * the high-word halves of the two xor-shifts use mul.hi (x >> s == mulhi(x, 2^(32-s)));
+//   * the final xor-shift is never formed for the test: with an ODD high-word threshold M,
+//     (z_hi ^ (z_hi >> 31)) <= M  <=>  z_hi <= M, because the xor only flips bit 0;
+//   * the compaction (popc, smem stores, finishing the key) runs only when some lane passed.
+__device__ __forceinline__ uint32_t mulhi_u32(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("mul.hi.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));  // opaque to the optimiser: stays an IMAD.HI
+  return r;
+}
+__device__ __forceinline__ uint64_t key_z(uint64_t hdst, uint32_t j) {
+  uint64_t x = hdst + (uint64_t)(j + 1u) * kGamma;
+  uint32_t lo = (uint32_t)x, hi = (uint32_t)(x >> 32);
+  lo ^= __funnelshift_r(lo, hi, 30);
+  hi ^= mulhi_u32(hi, 1u << 2);
+  uint64_t z = (((uint64_t)hi << 32) | lo) * 0xBF58476D1CE4E5B9ull;
+  lo = (uint32_t)z;
+  hi = (uint32_t)(z >> 32);
+  lo ^= __funnelshift_r(lo, hi, 27);
+  hi ^= mulhi_u32(hi, 1u << 5);
+  return (((uint64_t)hi << 32) | lo) * 0x94D049BB133111EBull;  // key = z ^ (z >> 31)
+}
+
+// FULL = exact 64-bit test (only when the bisection can no longer separate on high words).
+template <bool FULL, bool CHECK>
+__device__ __forceinline__ void select_step(uint64_t hdst, uint32_t j, uint32_t deg, uint64_t T,
+                                            uint32_t Modd, int& cnt, uint64_t* s_key, int32_t* s_pos) {
+  const uint64_t z = key_z(hdst, j);
   bool p;
-  if (FULL) p = (j < deg) && ((z ^ (z >> 31)) <= T);
-  else p = (j < deg) && ((zh ^ (zh >> 31)) <= (uint32_t)(T >> 32));
+  if (FULL) p = (z ^ (z >> 31)) <= T;
+  else p = (uint32_t)(z >> 32) <= Modd;
+  if (CHECK) p = p && (j < deg);
   const unsigned m = __ballot_sync(0xffffffffu, p);
   if (m) {
     if (p) {
@@ -99,15 +119,18 @@ template <bool FULL>
 __device__ __forceinline__ int select_pass(uint64_t hdst, uint32_t deg, uint64_t T,
                                            uint64_t* s_key, int32_t* s_pos) {
   const uint32_t lane = threadIdx.x & 31;
+  const uint32_t Modd = (uint32_t)(T >> 32) | 1u;
   int cnt = 0;
-  uint64_t x = hdst + (uint64_t)(lane + 1) * kGamma;
   uint32_t j = lane;
-  // two independent key chains per lane per iteration
-  for (uint32_t j0 = 0; j0 < deg; j0 += 64) {
-    select_step<FULL>(x, j, deg, T, cnt, s_key, s_pos);
-    select_step<FULL>(x + 32 * kGamma, j + 32, deg, T, cnt, s_key, s_pos);
-    x += 64 * kGamma;
-    j += 64;
+  const uint32_t full_end = deg & ~63u;
+  // two independent key chains per lane per iteration; no bound check inside whole 64-key chunks
+  for (; j < full_end; j += 64) {
+    select_step<FULL, false>(hdst, j, deg, T, Modd, cnt, s_key, s_pos);
+    select_step<FULL, false>(hdst, j + 32, deg, T, Modd, cnt, s_key, s_pos);
+  }
+  if (full_end < deg) {
+    select_step<FULL, true>(hdst, j, deg, T, Modd, cnt, s_key, s_pos);
+    select_step<FULL, true>(hdst, j + 32, deg, T, Modd, cnt, s_key, s_pos);
   }
   return cnt;
 }
@@ -134,7 +157,7 @@ __device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int
     // threshold guess: keys are uniform, so the f-th smallest is near f/deg * 2^64.  The
     // threshold only prunes; the exact rank below decides, so its rounding is immaterial.
     uint64_t T = (uint64_t)((float)want / (float)deg * 18446744073709551616.0f);
-    T |= 0xffffffffull;
+    T |= 0x1ffffffffull;  // the test uses the high word made odd: keep T equal to what is tested
     uint64_t lo = 0, hi = ~0ull;  // count(lo) < f known; count(hi) > kCand known once have_hi
     bool have_hi = false, full = false;
     for (;;) {
@@ -149,8 +172,8 @@ __device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int
         have_hi = true;
         T = lo + ((hi - lo) >> 1);
       }
-      if (have_hi && (hi >> 32) == (lo >> 32)) full = true;  // high words can no longer separate
-      if (!full) T |= 0xffffffffull;
+      if (have_hi && (hi >> 32) - (lo >> 32) <= 2) full = true;  // odd high words can no longer separate
+      if (!full) T |= 0x1ffffffffull;
     }
   }
   __syncwarp();
