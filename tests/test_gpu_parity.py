@@ -149,3 +149,28 @@ def test_error_codes(workload, dev):
     with pytest.raises(binding.GreenGNNError) as e:
         binding.Graph(w.indptr.cpu(), w.indices.cpu(), w.part_offsets, 0, w.feat_parts, seed=1)
     assert e.value.status == binding.GG_ERR_INVALID_ARG
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times ---------------------
+def test_products_full_size_first_window_W16(workload, dev):
+    """configs[2] at full size (N=2,449,029, nnz=123.8M, dim 100), B=1024, W=16, n_hot unlimited:
+    the first window (16 mini-batches, ~5.5M sampled nodes) against the oracle, every array."""
+    w = workload("products", dev)
+    s = pu.check_epoch(w, W=16, n_hot=-1, max_batches=16, cache_samples=256)
+    assert s["batches"] == 16 and s["misses"] == 0 and s["rows"] > 16 * 300_000
+
+
+def test_products_full_size_budgeted_two_windows(workload, dev):
+    """Same graph, finite budget = 10 % of the remote nodes, W=2, two windows:
+    exercises threshold selection, carry-over and the miss path at full size."""
+    w = workload("products", dev)
+    n_remote = w.num_nodes - int(w.part_offsets[1] - w.part_offsets[0])
+    s = pu.check_epoch(w, W=2, n_hot=n_remote // 10, max_batches=4, cache_samples=256)
+    assert s["windows"] == 2 and s["misses"] > 0
+
+
+def test_dense_full_size_first_window(workload, dev):
+    """configs[3] at full size (N=232,965, nnz=114.6M, avg degree ~490, rb = 2408 B)."""
+    w = workload("dense", dev)
+    s = pu.check_epoch(w, W=4, n_hot=-1, max_batches=4, cache_samples=128)
+    assert s["batches"] == 4
