@@ -240,6 +240,24 @@ gg_status gg_profile_get(gg_graph* g, gg_profile* out);
 /* number of kernels this library has launched in this process (all graphs) */
 uint64_t gg_launch_count(void);
 
+/* a-1 work counters, cumulative over the process (synchronises the device):
+ *   keys      key evaluations the method asks for = sum of deg over sampled destinations with
+ *             deg > fanout (one 64-bit SplitMix key per edge position, reading S1) -- the
+ *             algorithmic ALU work of the sampler, the unit of bench.py's "alu" roofline;
+ *   rows      destinations that needed a keyed selection (deg > fanout);
+ *   fallbacks of those, rows where the fast selection could not prove its result exact (lane
+ *             list overflow, fewer than fanout candidates under the threshold guess, or a tie in
+ *             the high 32 key bits at the boundary) and the exact ballot/bisection path ran.
+ * Any pointer may be NULL. */
+gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);
+
+/* Test knobs for the fallback logic of the selection kernel (tests/test_gpu_parity.py); results
+ * must stay bit-exact for every setting.  rank_shift in [0,31]: the ranking compares only the
+ * top 32-rank_shift key bits (forces ties); want_add: added to the number of candidates the
+ * threshold guess aims for (large: list overflow; negative: too few candidates).
+ * (0, 0.0f) restores the defaults.  Must not be called while a window is being staged. */
+gg_status gg_debug_sampler(int32_t rank_shift, float want_add);
+
 const char* gg_last_error(void);
 const char* gg_version(void);
 

@@ -72,7 +72,7 @@ PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage
 
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
-           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version"]
+           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler"]
 
 _lib = None
 
@@ -109,6 +109,8 @@ def load_library(path: Optional[str] = None):
     lib.gg_launch_count.restype = u64
     lib.gg_key.argtypes = [u64] * 5
     lib.gg_key.restype = u64
+    lib.gg_sampler_stats.argtypes = [P(u64), P(u64), P(u64)]
+    lib.gg_debug_sampler.argtypes = [i32, C.c_float]
     lib.gg_last_error.restype = C.c_char_p
     lib.gg_version.restype = C.c_char_p
     for s in SYMBOLS:
@@ -121,6 +123,23 @@ def load_library(path: Optional[str] = None):
 
 def launch_count() -> int:
     return int(load_library().gg_launch_count())
+
+
+def _check_global(rc: int):
+    if rc != 0:
+        raise GreenGNNError(rc, (load_library().gg_last_error() or b"").decode())
+
+
+def sampler_stats() -> dict:
+    """Cumulative a-1 counters: keys evaluated (algorithmic), keyed rows, exact-path fallbacks."""
+    k, r, f = u64(0), u64(0), u64(0)
+    _check_global(load_library().gg_sampler_stats(C.byref(k), C.byref(r), C.byref(f)))
+    return {"keys": int(k.value), "rows": int(r.value), "fallbacks": int(f.value)}
+
+
+def debug_sampler(rank_shift: int = 0, want_add: float = 0.0) -> None:
+    """Test knobs of the selection kernel (include/greengnn.h gg_debug_sampler)."""
+    _check_global(load_library().gg_debug_sampler(rank_shift, want_add))
 
 
 def gg_key(seed: int, batch: int, layer: int, dst: int, edge_pos: int) -> int:

@@ -1200,6 +1200,24 @@ gg_status gg_profile_get(gg_graph* g, gg_profile* out) {
 
 uint64_t gg_launch_count(void) { return (uint64_t)g_launches.load(); }
 
+gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks) {
+  CU(cudaDeviceSynchronize());
+  unsigned long long v[3] = {0, 0, 0};
+  sampler_stats(v);
+  CU(cudaGetLastError());
+  if (keys) *keys = v[0];
+  if (rows) *rows = v[1];
+  if (fallbacks) *fallbacks = v[2];
+  return GG_OK;
+}
+
+gg_status gg_debug_sampler(int32_t rank_shift, float want_add) {
+  if (rank_shift < 0 || rank_shift > 31) return fail(GG_ERR_INVALID_ARG, "rank_shift must be in [0, 31]");
+  CU(cudaDeviceSynchronize());
+  CU(sampler_debug(rank_shift, want_add));
+  return GG_OK;
+}
+
 gg_status gg_cache_reset(gg_graph* g) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
   if (g->win[0].live || g->win[1].live || g->win[2].live)

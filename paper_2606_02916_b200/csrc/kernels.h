@@ -31,6 +31,8 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
                        const uint64_t* key_prefix_b, uint8_t* cnt_tmp, int64_t cnt_pitch,
                        int32_t* tile_sums, int max_tiles, int32_t* totals, int32_t* blk_indptr,
                        int32_t* edge_off_out, int32_t* src_global);
+void sampler_stats(unsigned long long out[3]);           // synchronous read of g_sampler_stat
+cudaError_t sampler_debug(int rank_shift, float want_add);  // test knobs, see sample.cu
 // shared by a-1 / a-2: one CTA per batch row, exclusive scan of ceil(n_items[b]/items_per_tile) sums
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
                       int items_per_tile, int32_t* totals);

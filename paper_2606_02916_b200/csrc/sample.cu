@@ -17,6 +17,14 @@
 
 namespace gg {
 
+// cumulative sampler statistics: [0] key evaluations the method asks for (sum of deg over rows
+// with deg > fanout), [1] such rows, [2] rows that took the exact fallback path
+__device__ unsigned long long g_sampler_stat[3];
+// test knobs (gg_debug_sampler): compare only the top 32-shift bits when ranking (forces
+// high-word ties), and add to the candidate target (forces list overflow / too few candidates)
+__constant__ int c_rank_shift = 0;
+__constant__ float c_want_add = 0.0f;
+
 constexpr int kTile = 256;      // destinations per CTA tile
 constexpr int kCand = 256;      // candidate buffer per warp
 constexpr int kWarps = 8;
@@ -31,12 +39,23 @@ k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ n
   if (t * kTile >= nd) return;
   const int i = t * kTile + threadIdx.x;
   int c = 0;
+  unsigned long long keys = 0;
   if (i < nd) {
     const int32_t v = nodes[b * node_pitch + i];
     const int64_t r0 = __ldg(indptr + v), r1 = __ldg(indptr + v + 1);
     const int64_t deg = r1 - r0;
     c = deg < fanout ? (int)deg : fanout;
     cnt_tmp[b * cnt_pitch + i] = (uint8_t)c;
+    if (deg > fanout) keys = (unsigned long long)deg;
+  }
+  {
+    const unsigned rows = __popc(__ballot_sync(0xffffffffu, keys != 0));
+#pragma unroll
+    for (int o = 16; o; o >>= 1) keys += __shfl_xor_sync(0xffffffffu, keys, o);
+    if ((threadIdx.x & 31) == 0 && rows) {
+      atomicAdd(&g_sampler_stat[0], keys);
+      atomicAdd(&g_sampler_stat[1], (unsigned long long)rows);
+    }
   }
   int32_t total;
   block_exclusive_scan<int32_t>(c, sm, &total);
@@ -78,6 +97,11 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
 __device__ __forceinline__ uint32_t mulhi_u32(uint32_t a, uint32_t b) {
   uint32_t r;
   asm("mul.hi.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));  // opaque to the optimiser: stays an IMAD.HI
+  return r;
+}
+__device__ __forceinline__ uint32_t mad_lo_u32(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
   return r;
 }
 __device__ __forceinline__ uint64_t key_z(uint64_t hdst, uint32_t j) {
@@ -198,6 +222,160 @@ __device__ __forceinline__ void warp_select(const int32_t* __restrict__ row, int
   __syncwarp();
 }
 
+// ---- fast path: lane-local candidate lists, high-word ranking ---------------------------------
+// ncu (profiles/r01_b_pipeline.md) showed the ballot-compacted loop above spending half of its
+// issue slots outside the hash (vote, branch, popc, 96-bit ranking of ~40 candidates).  The fast
+// path removes every warp-synchronous operation from the key loop:
+//   * lane l owns the CONTIGUOUS positions [l*K, (l+1)*K), K = deg/32 (the deg%32 tail positions
+//     are handled once at the end), so "lane-major" order is ascending edge position;
+//   * a position passes when the HIGH word of its pre-xorshift key z is <= an odd threshold M
+//     (same test as above); a passing lane appends (z_hi, x_lo) to its OWN list in shared memory
+//     with two predicated stores and one predicated add -- no ballot, no branch.  x_lo is the
+//     low word of the SplitMix state, already in a register; the position is recovered from it
+//     as (x_lo - h_lo) * gamma_lo^-1 - 1 (mod 2^32);
+//   * the <= 128 candidates are compacted lane-major (= ascending position) and ranked on the
+//     high 32 bits of the key only: keep i iff #{c : hi_c < hi_i} < f.  That set always CONTAINS
+//     the true top-f under (key, position) and equals it iff it has exactly f members (a tie in
+//     the high word at the boundary is the only way to get more), so `kept == f` proves exactness
+//     and anything else -- a lane list overflow, fewer than f candidates, more than 128, a
+//     boundary tie -- falls back to warp_select above, which is exact by construction.
+constexpr int kLaneCap = 12;                  // candidate slots per lane
+constexpr int kFastCand = 128;                // compacted candidates
+constexpr int kScratchWords = 1024;           // per-warp scratch, 4 KB
+constexpr uint32_t kGammaLo = 0x7F4A7C15u, kGammaLoInv = 0x9937733Du;  // kGammaLo * kGammaLoInv == 1 (mod 2^32)
+constexpr uint32_t kC1lo = 0x1CE4E5B9u, kC1hi = 0xBF58476Du, kC2lo = 0x133111EBu, kC2hi = 0x94D049BBu;
+
+// high word of z = fmix's value before the last xor-shift, from the state x = {xhi, xlo}
+__device__ __forceinline__ uint32_t key_zhi(uint32_t xlo, uint32_t xhi) {
+  uint32_t lo = xlo ^ __funnelshift_r(xlo, xhi, 30);
+  uint32_t hi = xhi ^ mulhi_u32(xhi, 1u << 2);
+  // {hi,lo} * C1 (low 64 bits) in three FMA-pipe instructions: the cross terms accumulate
+  // straight onto the high half of the wide product
+  const uint64_t p = (uint64_t)lo * kC1lo;
+  hi = mad_lo_u32(lo, kC1hi, mad_lo_u32(hi, kC1lo, (uint32_t)(p >> 32)));
+  lo = (uint32_t)p;
+  lo ^= __funnelshift_r(lo, hi, 27);
+  hi ^= mulhi_u32(hi, 1u << 5);
+  return mulhi_u32(lo, kC2lo) + hi * kC2lo + lo * kC2hi;
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void fast_step(uint64_t x, uint32_t M, uint32_t& a) {
+  const uint32_t xlo = (uint32_t)x;
+  const uint32_t z = key_zhi(xlo, (uint32_t)(x >> 32));
+  if (z <= M) {
+    sts_u32(a, z);
+    sts_u32(a + kLaneCap * 128, xlo);
+    a += 128;
+  }
+}
+
+// Returns true when out[0..f) holds the exact result; false = caller must run warp_select.
+__device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row, uint32_t deg, int f,
+                                                 uint64_t hdst, uint32_t* scratch,
+                                                 int32_t* __restrict__ out) {
+  const uint32_t lane = threadIdx.x & 31;
+  uint32_t* c_hi = scratch + 2 * kLaneCap * 32;   // [kFastCand]
+  uint32_t* c_pos = c_hi + kFastCand;             // [kFastCand]
+  const float wantf = fmaxf((float)f + 2.0f + 2.5f * sqrtf((float)f) + c_want_add, 1.0f);
+  const int rshift = c_rank_shift;
+  int total;
+  if ((float)deg <= wantf && deg <= (uint32_t)kFastCand) {
+    // small row: every position is a candidate, already in position order
+    total = (int)deg;
+    for (uint32_t j = lane; j < deg; j += 32) {
+      const uint64_t x = hdst + (uint64_t)(j + 1u) * kGamma;
+      const uint32_t z = key_zhi((uint32_t)x, (uint32_t)(x >> 32));
+      c_hi[j] = (z ^ (z >> 31)) >> rshift;
+      c_pos[j] = j;
+    }
+  } else {
+    const uint32_t M = (uint32_t)fminf(__fdividef(wantf, (float)deg) * 4294967296.0f, 4294967040.0f) | 1u;
+    const uint32_t K = deg >> 5;
+    const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(scratch) + lane * 4;
+    uint32_t a = a0;
+    const uint32_t a_lim4 = a0 + (kLaneCap - 4) * 128, a_lim1 = a0 + (kLaneCap - 1) * 128;
+    uint64_t x = hdst + (uint64_t)(lane * K + 1u) * kGamma;
+    uint32_t n4 = K >> 2;
+    while (n4 != 0 && a <= a_lim4) {
+      fast_step(x, M, a);
+      fast_step(x + kGamma, M, a);
+      fast_step(x + 2 * kGamma, M, a);
+      fast_step(x + 3 * kGamma, M, a);
+      x += 4 * kGamma;
+      --n4;
+    }
+    uint32_t rem = (K & 3u) + 4u * n4;   // n4 != 0 only when this lane's list is nearly full
+    while (rem != 0 && a <= a_lim1) {
+      fast_step(x, M, a);
+      x += kGamma;
+      --rem;
+    }
+    const bool ovf = rem != 0;
+    // tail positions 32K + lane
+    const uint32_t jt = (K << 5) + lane;
+    uint32_t zt = 0;
+    bool pt = false;
+    if (jt < deg) {
+      const uint64_t xt = hdst + (uint64_t)(jt + 1u) * kGamma;
+      zt = key_zhi((uint32_t)xt, (uint32_t)(xt >> 32));
+      pt = zt <= M;
+    }
+    const unsigned tmask = __ballot_sync(0xffffffffu, pt);
+    const int c = (int)((a - a0) >> 7);
+    const int total_main = __reduce_add_sync(0xffffffffu, c);
+    total = total_main + __popc(tmask);
+    if (__any_sync(0xffffffffu, ovf) || total < f || total > kFastCand) return false;
+    int incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, incl, o);
+      if ((int)lane >= o) incl += y;
+    }
+    const int off = incl - c;
+    const uint32_t hlo = (uint32_t)hdst;
+    for (int s = 0; s < c; ++s) {
+      const uint32_t z = lds_u32(a0 + s * 128);
+      const uint32_t xl = lds_u32(a0 + s * 128 + kLaneCap * 128);
+      c_hi[off + s] = (z ^ (z >> 31)) >> rshift;
+      c_pos[off + s] = (xl - hlo) * kGammaLoInv - 1u;
+    }
+    if (pt) {
+      const int q = total_main + __popc(tmask & lanemask_lt());
+      c_hi[q] = (zt ^ (zt >> 31)) >> rshift;
+      c_pos[q] = jt;
+    }
+  }
+  if (lane < 4 && total + (int)lane < kFastCand) c_hi[total + lane] = 0xffffffffu;  // pad to a multiple of 4
+  __syncwarp();
+  const uint4* c_hi4 = reinterpret_cast<const uint4*>(c_hi);
+  const int n4 = (total + 3) >> 2;
+  int emitted = 0;
+  for (int i0 = 0; i0 < total; i0 += 32) {
+    const int i = i0 + (int)lane;
+    const uint32_t mine = i < total ? c_hi[i] : 0u;
+    int rank = 0;
+    for (int q = 0; q < n4; ++q) {
+      const uint4 v = c_hi4[q];
+      rank += (v.x < mine) + (v.y < mine) + (v.z < mine) + (v.w < mine);
+    }
+    const bool keep = i < total && rank < f;
+    const unsigned m = __ballot_sync(0xffffffffu, keep);
+    const int q = emitted + __popc(m & lanemask_lt());
+    if (keep && q < f) out[q] = __ldg(row + c_pos[i]);
+    emitted += __popc(m);
+  }
+  __syncwarp();
+  return emitted == f;
+}
+
+
 __global__ void __launch_bounds__(kTile)
 k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
                 const int32_t* __restrict__ nodes, int64_t node_pitch, BatchOffsets n_dst,
@@ -209,8 +387,7 @@ k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ 
   __shared__ int32_t sm[33];
   __shared__ int32_t s_off[kTile + 1];
   __shared__ int32_t s_edge_base, s_next;
-  __shared__ uint64_t s_key[kWarps][kCand];
-  __shared__ int32_t s_pos[kWarps][kCand];
+  __shared__ __align__(16) uint32_t s_scratch[kWarps][kScratchWords];
   const int b = blockIdx.y, t = blockIdx.x;
   const int nd = n_dst.v[b];
   if (t * kTile >= nd) return;
@@ -254,12 +431,27 @@ k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ 
     if (deg <= fanout) {
       for (int j = lane; j < deg; j += 32) out[j] = __ldg(indices + r0 + j);
     } else {
-      warp_select(indices + r0, deg, fanout, key_hdst(prefix, (uint64_t)(uint32_t)v),
-                  s_key[wid], s_pos[wid], out);
+      const uint64_t hdst = key_hdst(prefix, (uint64_t)(uint32_t)v);
+      if (!warp_select_fast(indices + r0, (uint32_t)deg, fanout, hdst, s_scratch[wid], out)) {
+        // rare: lane-list overflow, a bad threshold guess or a high-word tie at the boundary
+        if (lane == 0) atomicAdd(&g_sampler_stat[2], 1ull);
+        uint64_t* s_key = reinterpret_cast<uint64_t*>(s_scratch[wid]);
+        int32_t* s_pos = reinterpret_cast<int32_t*>(s_scratch[wid] + 2 * kCand);
+        warp_select(indices + r0, deg, fanout, hdst, s_key, s_pos, out);
+      }
     }
     if (lane == 0) d = atomicAdd(&s_next, 1);
     d = __shfl_sync(0xffffffffu, d, 0);
   }
+}
+
+void sampler_stats(unsigned long long out[3]) {
+  cudaMemcpyFromSymbol(out, g_sampler_stat, 3 * sizeof(unsigned long long));
+}
+cudaError_t sampler_debug(int rank_shift, float want_add) {
+  cudaError_t e = cudaMemcpyToSymbol(c_rank_shift, &rank_shift, sizeof(int));
+  if (e != cudaSuccess) return e;
+  return cudaMemcpyToSymbol(c_want_add, &want_add, sizeof(float));
 }
 
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,

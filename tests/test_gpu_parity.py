@@ -70,6 +70,35 @@ def test_large_mini_directed_bf16(workload, dev):
     pu.check_epoch(w, W=4, n_hot=11250, staging_mode=1)
 
 
+@pytest.mark.parametrize("rank_shift,want_add", [(24, 0.0), (31, 0.0), (0, 400.0), (0, 120.0), (0, -30.0), (20, 40.0)])
+def test_selection_fallback_paths_stay_exact(workload, dev, rank_shift, want_add):
+    """The fast selection proves its own result (kept == fanout) or falls back to the exact path.
+    The knobs force each fallback cause -- ties in the compared key bits, lane-list overflow,
+    more than 128 candidates, fewer than fanout candidates -- and the blocks must not change."""
+    from paper_2606_02916_b200 import binding
+    w = workload("dense_mini", dev)
+    before = binding.sampler_stats()
+    binding.debug_sampler(rank_shift, want_add)
+    try:
+        pu.check_epoch(w, W=2, n_hot=-1, max_batches=2, check_features=False)
+    finally:
+        binding.debug_sampler(0, 0.0)
+    after = binding.sampler_stats()
+    assert after["rows"] > before["rows"] and after["keys"] > before["keys"]
+    assert after["fallbacks"] > before["fallbacks"], "the knob did not reach the fallback path"
+
+
+def test_selection_fallbacks_are_rare_by_default(workload, dev):
+    from paper_2606_02916_b200 import binding
+    w = workload("dense_mini", dev)
+    before = binding.sampler_stats()
+    pu.check_epoch(w, W=4, n_hot=-1, max_batches=4, check_features=False)
+    after = binding.sampler_stats()
+    rows = after["rows"] - before["rows"]
+    assert rows > 1000
+    assert (after["fallbacks"] - before["fallbacks"]) <= 0.03 * rows
+
+
 def test_lookahead_one_is_algorithm_1_literal(workload, dev):
     """stage(k+1) / serve k (Alg. 1) gives the same results as the deeper pipeline."""
     from paper_2606_02916_b200 import epoch as ep
