@@ -226,10 +226,13 @@ uint64_t gg_key(uint64_t seed, uint64_t batch, uint64_t layer, uint64_t dst, uin
  *   SELECT  hot select + delta split;        bytes = 12*n_unique
  *   STAGE_COPY the per-owner bulk transfers; bytes = sum |Delta_m| * row_bytes (host link)
  *   CARRY   carry-over D2D copy;             bytes = 2 * carried * row_bytes
+ *   WAIT    GPU stall at a window boundary: time the caller's stream spends in the wait for the
+ *           window's cache-ready event before its first gather (Alg. 1 l.5)
  * gg_profile_enable(g, on) clears the accumulators; gg_profile_get synchronises the device. */
-#define GG_PROF_KINDS 8
+#define GG_PROF_KINDS 9
 enum { GG_PROF_GATHER = 0, GG_PROF_MISS = 1, GG_PROF_SAMPLE = 2, GG_PROF_FRONTIER = 3,
-       GG_PROF_UNIQUE = 4, GG_PROF_SELECT = 5, GG_PROF_STAGE_COPY = 6, GG_PROF_CARRY = 7 };
+       GG_PROF_UNIQUE = 4, GG_PROF_SELECT = 5, GG_PROF_STAGE_COPY = 6, GG_PROF_CARRY = 7,
+       GG_PROF_WAIT = 8 };
 typedef struct {
   double ms[GG_PROF_KINDS];
   int64_t regions[GG_PROF_KINDS];
@@ -245,9 +248,10 @@ uint64_t gg_launch_count(void);
  *             deg > fanout (one 64-bit SplitMix key per edge position, reading S1) -- the
  *             algorithmic ALU work of the sampler, the unit of bench.py's "alu" roofline;
  *   rows      destinations that needed a keyed selection (deg > fanout);
- *   fallbacks of those, rows where the fast selection could not prove its result exact (lane
- *             list overflow, fewer than fanout candidates under the threshold guess, or a tie in
- *             the high 32 key bits at the boundary) and the exact ballot/bisection path ran.
+ *   fallbacks of those, hand-overs because a fast selection could not prove its result exact
+ *             (candidate list overflow, fewer than fanout candidates under the threshold guess,
+ *             or a tie in the high 32 key bits at the boundary): thread-per-row kernel -> warp
+ *             kernel, plus warp kernel -> exact ballot/bisection path.
  * Any pointer may be NULL. */
 gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);
 

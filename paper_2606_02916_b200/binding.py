@@ -65,10 +65,10 @@ class gg_window_trace(C.Structure):
 
 
 class gg_profile(C.Structure):
-    _fields_ = [("ms", C.c_double * 8), ("regions", i64 * 8), ("bytes", i64 * 8)]
+    _fields_ = [("ms", C.c_double * 9), ("regions", i64 * 9), ("bytes", i64 * 9)]
 
 
-PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage_copy", "carry"]
+PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage_copy", "carry", "wait"]
 
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",

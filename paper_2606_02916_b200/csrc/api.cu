@@ -156,6 +156,11 @@ struct CacheSlot {
   DevBuf<int32_t> hot;
   int64_t n_cached = 0;        // entries of `hot` currently reflected in slot_map
   Window* tenant = nullptr;    // window whose H_k is in here (may already be released)
+  // last gather that read this buffer / slot map.  Kept per cache slot, not only per window
+  // arena: the arena of a released tenant can be re-staged (and its own flag reset) before the
+  // next stage_b on this slot runs.
+  cudaEvent_t gather_done = nullptr;
+  bool gather_recorded = false;
 };
 
 // One of the three window arenas (k being served, k+1 being staged, k+2 being sampled).
@@ -188,6 +193,8 @@ struct Window {
   cudaEvent_t sampled = nullptr;  // phase A complete (stream A)
   cudaEvent_t ready = nullptr;    // cache ready (stream B)
   cudaEvent_t gather_done = nullptr;
+  cudaEvent_t ev_copy[2 * GG_MAX_PARTS + 2] = {nullptr};  // start/stop per bulk copy, last pair = carry
+  bool timing_pending = false;    // ms_h2d / ms_carry not yet read from the events
   bool gather_recorded = false;
   bool enqueued = false;          // phase B finished on the host (or an error was recorded)
   gg_status status = GG_OK;
@@ -270,7 +277,11 @@ struct gg_graph {
   DevBuf<uint32_t> seen, newbits, cnt8;
   DevBuf<int32_t> wprefix, seed_perm, tiles32, totals, stats, hist, err_flag, seeds_dev;
   DevBuf<uint64_t> key_prefix;
-  DevBuf<uint8_t> cnt_tmp;
+  DevBuf<uint8_t> cnt_tmp, samp_plan;
+  DevBuf<uint64_t> it_hdst;
+  DevBuf<int64_t> it_row0;
+  DevBuf<uint32_t> it_deg;
+  DevBuf<int32_t> it_out, it_fb;
   int64_t cnt_words = 0;  // padded words of cnt8
   int64_t planned_t32 = 0, planned_cnt_tmp = 0, planned_miss = 0, planned_t64 = 0;
   // phase B workspaces (stager thread only)
@@ -282,14 +293,17 @@ struct gg_graph {
   int32_t* h_small = nullptr;    // phase A readback scratch
   int32_t* h_small_b = nullptr;  // phase B readback scratch
   int32_t* h_req = nullptr;      // request IDs (device -> host)
-  uint8_t* h_resp = nullptr;     // packed rows (host -> device), mode 0
+  uint8_t* h_resp[2] = {nullptr, nullptr};  // packed rows (host -> device), mode 0, ping-pong
+  cudaEvent_t resp_free[2] = {nullptr, nullptr};  // bulk copies out of h_resp[i] have completed
+  bool resp_used[2] = {false, false};
+  int resp_idx = 0;
   int32_t* h_seeds = nullptr;
-  int64_t h_seeds_cap = 0, h_req_cap = 0, h_resp_cap = 0;
+  int64_t h_seeds_cap = 0, h_req_cap = 0, h_resp_cap[2] = {0, 0};
   uint64_t* h_kp = nullptr;
   // streams / threads
   cudaStream_t side = nullptr;    // phase A: sample, frontier, unique
-  cudaStream_t side_b = nullptr;  // phase B: select, delta, bulk copies, carry
-  cudaEvent_t ev_copy[2 * GG_MAX_PARTS] = {nullptr};
+  cudaStream_t side_b = nullptr;  // phase B: select, delta (the stager thread syncs on it)
+  cudaStream_t side_c = nullptr;  // phase B: bulk copies, carry-over copy, cache-ready event (never waited on by the stager)
   Window win[3];
   CacheSlot cslot[2];
   uint64_t stage_counter = 0;
@@ -382,6 +396,12 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
   }
   ENS(g->tiles32, t32);
   ENS(g->cnt_tmp, cnt_tmp);
+  ENS(g->samp_plan, (int64_t)sample_plan_bytes());
+  ENS(g->it_hdst, cnt_tmp);
+  ENS(g->it_row0, cnt_tmp);
+  ENS(g->it_deg, cnt_tmp);
+  ENS(g->it_out, cnt_tmp);
+  ENS(g->it_fb, cnt_tmp);
   ENS(g->tiles64, t64);
   ENS(g->miss_tmp_pos, mcap);
   ENS(g->miss_tmp_id, mcap);
@@ -419,6 +439,8 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   gg_status rc = alloc_window(g, w);
   if (rc != GG_OK) return rc;
   // the arena's previous tenant may still be read by gathers already enqueued
+  // (and its staging on stream C reads the arena's request / carry lists)
+  CU(cudaStreamWaitEvent(st, w->ready, 0));
   if (w->gather_recorded) CU(cudaStreamWaitEvent(st, w->gather_done, 0));
   w->gather_recorded = false;
 
@@ -455,10 +477,14 @@ static gg_status stage_a(gg_graph* g, Window* w) {
     dst_off.v[W] = H.dst_off[W];
     const int max_tiles = (int)ceil_div(max_nd, 256);
     const int64_t cnt_pitch = max_nd;
+    SampleWork wk;
+    wk.plan = g->samp_plan.p;
+    wk.items.hdst = g->it_hdst.p; wk.items.row0 = g->it_row0.p; wk.items.deg = g->it_deg.p;
+    wk.items.out = g->it_out.p; wk.items.fallback = g->it_fb.p;
     cudaEvent_t pe = g->prof.begin(st);
     launch_sample_hop(st, g->indptr, g->indices, w->nodes.p, w->node_pitch, n_dst, dst_off, W, max_nd,
                       w->fanouts[h], g->key_prefix.p + h * Wmax, g->cnt_tmp.p, cnt_pitch, g->tiles32.p,
-                      max_tiles, edge_totals, H.blk_indptr.p, H.edge_off_dev.p, H.src_global.p);
+                      max_tiles, edge_totals, H.blk_indptr.p, H.edge_off_dev.p, H.src_global.p, wk);
     g->prof.end(st, pe, GG_PROF_SAMPLE, 0);
     const int64_t max_edges = (int64_t)H.dst_off[W] * w->fanouts[h];
     pe = g->prof.begin(st);
@@ -558,7 +584,7 @@ static gg_status stage_b(gg_graph* g, Window* w) {
   }
   const double t0 = now_ms();
   CU(cudaStreamWaitEvent(st, w->sampled, 0));
-  if (cs->tenant && cs->tenant->gather_recorded) CU(cudaStreamWaitEvent(st, cs->tenant->gather_done, 0));
+  if (cs->gather_recorded) CU(cudaStreamWaitEvent(st, cs->gather_done, 0));
   CacheSlot* prev = g->prev_cs;
 
   // a-4 hot set: threshold t and quota of count == t nodes from the histogram
@@ -602,7 +628,12 @@ static gg_status stage_b(gg_graph* g, Window* w) {
   const double t1 = now_ms();
   w->ms_select = (float)(t1 - t0);
 
-  // a-6 staging: one bulk transfer per owner into that owner's contiguous slot range
+  // a-6 staging: one bulk transfer per owner into that owner's contiguous slot range.  The
+  // copies, the carry-over copy and the ready event go to stream C, which this thread never
+  // waits on: while the DMA engine drains window k's responses the thread already selects and
+  // packs window k+1 (two response buffers).  Everything C reads was produced on stream B
+  // before the cudaStreamSynchronize above, and B had waited for the old tenant's gathers.
+  cudaStream_t sc = g->side_c;
   w->bulk_copies = 0;
   w->ms_pack = 0;
   const int64_t rb = g->rb;
@@ -612,11 +643,14 @@ static gg_status stage_b(gg_graph* g, Window* w) {
     rc = ensure_pinned(&pr, &g->h_req_cap, w->n_delta * (int64_t)sizeof(int32_t));
     g->h_req = (int32_t*)pr;
     if (rc != GG_OK) return rc;
-    void* pp = g->h_resp;
-    rc = ensure_pinned(&pp, &g->h_resp_cap, w->n_delta * rb);
-    g->h_resp = (uint8_t*)pp;
-    if (rc != GG_OK) return rc;
     CU(cudaMemcpyAsync(g->h_req, w->req_ids.p, (size_t)w->n_delta * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    const int ri = g->resp_idx;
+    g->resp_idx ^= 1;
+    if (g->resp_used[ri]) CU(cudaEventSynchronize(g->resp_free[ri]));  // its previous copies are done
+    void* pp = g->h_resp[ri];
+    rc = ensure_pinned(&pp, &g->h_resp_cap[ri], w->n_delta * rb);
+    g->h_resp[ri] = (uint8_t*)pp;
+    if (rc != GG_OK) return rc;
     CU(cudaStreamSynchronize(st));
     int64_t q0 = 0;
     for (int m = 0; m < g->R.P; ++m) {
@@ -627,60 +661,64 @@ static gg_status stage_b(gg_graph* g, Window* w) {
       const uint8_t* base = g->store.base[m];
       const int64_t lo = g->R.lo[m], stride = g->store.stride;
       const int32_t* ids = g->h_req + q0;
-      uint8_t* resp = g->h_resp + q0 * rb;
+      uint8_t* resp = g->h_resp[ri] + q0 * rb;
       const int64_t chunk = 512;
       g->pool->parallel_for(ceil_div(nm, chunk), [&](int64_t c) {
         pack_rows(resp, base, ids, lo, stride, rb, c * chunk, std::min(nm, (c + 1) * chunk));
       });
       w->ms_pack += (float)(now_ms() - p0);
-      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));
-      CU(cudaMemcpyAsync(cs->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, st));
-      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies + 1], st));
+      cudaEvent_t pe = g->prof.begin(sc);
+      CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies], sc));
+      CU(cudaMemcpyAsync(cs->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, sc));
+      CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies + 1], sc));
+      g->prof.end(sc, pe, GG_PROF_STAGE_COPY, nm * rb);
       w->bulk_copies += 1;
       q0 += nm;
     }
+    CU(cudaEventRecord(g->resp_free[ri], sc));
+    g->resp_used[ri] = true;
   } else if (w->n_delta > 0) {
     // staging_mode 1: GPU-initiated pull, one launch per owner, no host pack / no ID read-back
     int64_t q0 = 0;
     for (int m = 0; m < g->R.P; ++m) {
       const int64_t nm = w->bulk[m];
       if (nm == 0) continue;
-      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies], st));
-      launch_rows_from_store(st, w->req_ids.p + q0, (int)nm, g->store, g->R, cs->cache, q0, rb, (int)rb);
-      CU(cudaEventRecord(g->ev_copy[2 * w->bulk_copies + 1], st));
+      cudaEvent_t pe = g->prof.begin(sc);
+      CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies], sc));
+      launch_rows_from_store(sc, w->req_ids.p + q0, (int)nm, g->store, g->R, cs->cache, q0, rb, (int)rb);
+      CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies + 1], sc));
+      g->prof.end(sc, pe, GG_PROF_STAGE_COPY, nm * rb);
       w->bulk_copies += 1;
       q0 += nm;
     }
   }
-  // carried rows: D2D out of the previous buffer, after the delta rows
-  pe = g->prof.begin(st);
-  cudaEvent_t carry_a = g->ev_copy[2 * GG_MAX_PARTS - 2], carry_b = g->ev_copy[2 * GG_MAX_PARTS - 1];
-  CU(cudaEventRecord(carry_a, st));
+  // carried rows: D2D out of the previous buffer (filled earlier on the same stream), after the delta rows
+  pe = g->prof.begin(sc);
+  CU(cudaEventRecord(w->ev_copy[2 * GG_MAX_PARTS], sc));
   if (w->n_carry > 0)
-    launch_rows_from_list(st, w->carry_src.p, (int)w->n_carry, prev->cache, rb, cs->cache, w->n_delta, rb, (int)rb);
-  CU(cudaEventRecord(carry_b, st));
-  g->prof.end(st, pe, GG_PROF_CARRY, 2ll * w->n_carry * rb);
-  CU(cudaMemsetAsync(w->counters.p, 0, (size_t)Wmax * (2 + GG_MAX_PARTS) * sizeof(int32_t), st));
-  CU(cudaEventRecord(w->ready, st));
-  CU(cudaEventSynchronize(w->ready));
-  float ms = 0;
-  w->ms_h2d = 0;
-  for (int c = 0; c < w->bulk_copies; ++c) {
-    cudaEventElapsedTime(&ms, g->ev_copy[2 * c], g->ev_copy[2 * c + 1]);
-    w->ms_h2d += ms;
-  }
-  if (g->prof.on && w->n_delta > 0) {
-    std::lock_guard<std::mutex> l(g->prof.m);
-    g->prof.ms[GG_PROF_STAGE_COPY] += w->ms_h2d;
-    g->prof.regions[GG_PROF_STAGE_COPY] += w->bulk_copies;
-    g->prof.bytes[GG_PROF_STAGE_COPY] += w->n_delta * rb;
-  }
-  cudaEventElapsedTime(&ms, carry_a, carry_b);
-  w->ms_carry = ms;
+    launch_rows_from_list(sc, w->carry_src.p, (int)w->n_carry, prev->cache, rb, cs->cache, w->n_delta, rb, (int)rb);
+  CU(cudaEventRecord(w->ev_copy[2 * GG_MAX_PARTS + 1], sc));
+  g->prof.end(sc, pe, GG_PROF_CARRY, 2ll * w->n_carry * rb);
+  CU(cudaMemsetAsync(w->counters.p, 0, (size_t)Wmax * (2 + GG_MAX_PARTS) * sizeof(int32_t), sc));
+  CU(cudaEventRecord(w->ready, sc));
+  w->timing_pending = true;
   CU(cudaGetLastError());
   g->prev_cs = cs;
   w->ms_total = w->ms_sample + w->ms_unique + (float)(now_ms() - t0);
   return GG_OK;
+}
+
+// ms_h2d / ms_carry of a window whose ready event has completed
+static void resolve_timing(Window* w) {
+  if (!w->timing_pending) return;
+  float ms = 0;
+  w->ms_h2d = 0;
+  for (int c = 0; c < w->bulk_copies; ++c)
+    if (cudaEventElapsedTime(&ms, w->ev_copy[2 * c], w->ev_copy[2 * c + 1]) == cudaSuccess) w->ms_h2d += ms;
+  if (cudaEventElapsedTime(&ms, w->ev_copy[2 * GG_MAX_PARTS], w->ev_copy[2 * GG_MAX_PARTS + 1]) == cudaSuccess)
+    w->ms_carry = ms;
+  cudaGetLastError();
+  w->timing_pending = false;
 }
 
 static void finish_job(gg_graph* g, Window* w, gg_status rc) {
@@ -789,10 +827,12 @@ gg_status gg_graph_destroy(gg_graph* g) {
     if (w.sampled) cudaEventDestroy(w.sampled);
     if (w.ready) cudaEventDestroy(w.ready);
     if (w.gather_done) cudaEventDestroy(w.gather_done);
+    for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) if (w.ev_copy[c]) cudaEventDestroy(w.ev_copy[c]);
   }
   for (int s = 0; s < 2; ++s) {
     CacheSlot& c = g->cslot[s];
     c.hot.release();
+    if (c.gather_done) cudaEventDestroy(c.gather_done);
     if (c.cache) cudaFree(c.cache);
     if (c.slot_map) cudaFree(c.slot_map);
   }
@@ -801,17 +841,22 @@ gg_status gg_graph_destroy(gg_graph* g) {
   g->seed_perm.release(); g->tiles32.release(); g->totals.release(); g->stats.release();
   g->hist.release(); g->owner_cnt.release(); g->n_delta_dev.release(); g->err_flag.release();
   g->seeds_dev.release(); g->tiles64.release(); g->total64.release(); g->key_prefix.release();
+  g->samp_plan.release(); g->it_hdst.release(); g->it_row0.release(); g->it_deg.release();
+  g->it_out.release(); g->it_fb.release();
   g->cnt_tmp.release(); g->miss_tmp_pos.release(); g->miss_tmp_id.release(); g->tile_miss.release();
   g->miss_pos.release(); g->miss_id.release(); g->n_miss.release();
   if (g->h_small) cudaFreeHost(g->h_small);
   if (g->h_small_b) cudaFreeHost(g->h_small_b);
   if (g->h_req) cudaFreeHost(g->h_req);
-  if (g->h_resp) cudaFreeHost(g->h_resp);
+  for (int i = 0; i < 2; ++i) {
+    if (g->h_resp[i]) cudaFreeHost(g->h_resp[i]);
+    if (g->resp_free[i]) cudaEventDestroy(g->resp_free[i]);
+  }
   if (g->h_seeds) cudaFreeHost(g->h_seeds);
   if (g->h_kp) cudaFreeHost(g->h_kp);
-  for (int c = 0; c < 2 * GG_MAX_PARTS; ++c) if (g->ev_copy[c]) cudaEventDestroy(g->ev_copy[c]);
   if (g->side) cudaStreamDestroy(g->side);
   if (g->side_b) cudaStreamDestroy(g->side_b);
+  if (g->side_c) cudaStreamDestroy(g->side_c);
   delete g;
   return GG_OK;
 }
@@ -909,9 +954,11 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   CUC(cudaHostAlloc((void**)&g->h_kp, (size_t)GG_MAX_LAYERS * Wmax * sizeof(uint64_t), cudaHostAllocDefault));
   CUC(cudaStreamCreateWithFlags(&g->side, cudaStreamNonBlocking));
   CUC(cudaStreamCreateWithFlags(&g->side_b, cudaStreamNonBlocking));
-  for (int c = 0; c < 2 * GG_MAX_PARTS; ++c) CUC(cudaEventCreate(&g->ev_copy[c]));
+  CUC(cudaStreamCreateWithFlags(&g->side_c, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) CUC(cudaEventCreateWithFlags(&g->resp_free[i], cudaEventDisableTiming));
   for (int s = 0; s < 2; ++s) {
     CacheSlot& c = g->cslot[s];
+    CUC(cudaEventCreateWithFlags(&c.gather_done, cudaEventDisableTiming));
     CUC(cudaMalloc((void**)&c.cache, (size_t)std::max<int64_t>(g->cache_rows, 1) * rb));
     CUC(cudaMalloc((void**)&c.slot_map, (size_t)g->N * sizeof(int32_t)));
     CUC(c.hot.ensure(std::max<int64_t>(g->cache_rows, 1)));
@@ -922,6 +969,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
     CUC(cudaEventCreateWithFlags(&w.sampled, cudaEventDisableTiming));
     CUC(cudaEventCreateWithFlags(&w.ready, cudaEventDefault));
     CUC(cudaEventCreateWithFlags(&w.gather_done, cudaEventDisableTiming));
+    for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) CUC(cudaEventCreate(&w.ev_copy[c]));
   }
   CUC(cudaDeviceSynchronize());
 #undef CUC
@@ -1061,7 +1109,14 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   if (out->features_capacity_rows < n)
     return fail(GG_ERR_CAPACITY, "features_capacity_rows = %lld < n_input = %d", (long long)out->features_capacity_rows, n);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  CU(cudaStreamWaitEvent(st, w->ready, 0));
+  if (!w->gather_recorded) {
+    // first gather of the window: the boundary wait of Alg. 1 l.5, timed on the caller's stream
+    cudaEvent_t pw = g->prof.begin(st);
+    CU(cudaStreamWaitEvent(st, w->ready, 0));
+    g->prof.end(st, pw, GG_PROF_WAIT, 0);
+  } else {
+    CU(cudaStreamWaitEvent(st, w->ready, 0));
+  }
   GatherLaunch G;
   G.nodes = w->nodes.p + (int64_t)b * w->node_pitch; G.n = n; G.slot_of = w->cs->slot_map;
   G.local_base = g->store.base[g->R.local]; G.local_stride = g->store.stride;
@@ -1081,6 +1136,8 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   }
   CU(cudaEventRecord(w->gather_done, st));
   w->gather_recorded = true;
+  CU(cudaEventRecord(w->cs->gather_done, st));
+  w->cs->gather_recorded = true;
   CU(cudaGetLastError());
   fill_batch_out(w, b, out, g);
   return GG_OK;
@@ -1112,6 +1169,7 @@ gg_status gg_trace(gg_graph* g, int64_t window_id, gg_window_trace* out) {
   gg_status rc = wait_enqueued(g, w);
   if (rc != GG_OK) return rc;
   CU(cudaEventSynchronize(w->ready));
+  resolve_timing(w);
   if (w->gather_recorded) CU(cudaEventSynchronize(w->gather_done));
   out->W = w->W; out->num_parts = g->R.P;
   out->n_access = w->n_access; out->n_unique = w->n_unique; out->n_unique_remote = w->n_remote;
@@ -1202,12 +1260,12 @@ uint64_t gg_launch_count(void) { return (uint64_t)g_launches.load(); }
 
 gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks) {
   CU(cudaDeviceSynchronize());
-  unsigned long long v[3] = {0, 0, 0};
+  unsigned long long v[4] = {0, 0, 0, 0};
   sampler_stats(v);
   CU(cudaGetLastError());
   if (keys) *keys = v[0];
   if (rows) *rows = v[1];
-  if (fallbacks) *fallbacks = v[2];
+  if (fallbacks) *fallbacks = v[2] + v[3];
   return GG_OK;
 }
 

@@ -24,14 +24,26 @@ struct FrontierBufs {
   int perm_pitch;      // max_batch
 };
 
-// a-1
+// a-1: work items of one hop, structure of arrays (k_sample_plan writes, the select kernels read)
+struct SampleItems {
+  uint64_t* hdst;     // SplitMix stream seed of the row: sm(prefix(seed, batch, layer) ^ dst)
+  int64_t* row0;      // indptr[dst]
+  uint32_t* deg;
+  int32_t* out;       // final offset of the row's first kept neighbor in src_global
+  int32_t* fallback;  // item indices handed from the thread kernel to the warp kernel
+};
+struct SampleWork {
+  void* plan;         // device, sample_plan_bytes()
+  SampleItems items;  // each array holds at least the hop's destination count
+};
+size_t sample_plan_bytes();
 void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* indices,
                        const int32_t* nodes, int64_t node_pitch, const BatchOffsets& n_dst,
                        const BatchOffsets& dst_off, int W, int max_nd, int fanout,
                        const uint64_t* key_prefix_b, uint8_t* cnt_tmp, int64_t cnt_pitch,
                        int32_t* tile_sums, int max_tiles, int32_t* totals, int32_t* blk_indptr,
-                       int32_t* edge_off_out, int32_t* src_global);
-void sampler_stats(unsigned long long out[3]);           // synchronous read of g_sampler_stat
+                       int32_t* edge_off_out, int32_t* src_global, const SampleWork& wk);
+void sampler_stats(unsigned long long out[4]);           // synchronous read of g_sampler_stat
 cudaError_t sampler_debug(int rank_shift, float want_add);  // test knobs, see sample.cu
 // shared by a-1 / a-2: one CTA per batch row, exclusive scan of ceil(n_items[b]/items_per_tile) sums
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,

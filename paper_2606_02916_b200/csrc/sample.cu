@@ -6,20 +6,29 @@
 // edge position.  The key depends on (seed, batch, layer, dst, j) only -- never on the
 // neighbor id -- so the adjacency row is not read to select; only the <= f chosen entries are.
 //
-// Three launches per hop:
-//   k_sample_count   one thread per destination: c = min(deg, f) -> cnt_tmp, per-tile sums
-//   k_tile_scan      one CTA per batch: exclusive scan of that batch's tile sums, batch total
-//   k_sample_select  one CTA per tile of 256 destinations: in-tile scan -> block indptr and
-//                    final output offsets (no atomics => deterministic), then one WARP PER
-//                    DESTINATION (dynamic in-CTA queue) does the keyed selection.
+// Five launches per hop (the rows of a power-law graph differ in cost by 1000x, so they are
+// binned by degree and each bin gets the granularity that suits it):
+//   k_sample_count   one thread per destination: c = min(deg, f) -> cnt_tmp, per-tile sums,
+//                    histogram of the keyed rows (deg > f) over half-octave degree bins
+//   k_tile_scan      one CTA per batch: exclusive scan of that batch's tile sums, batch total;
+//                    CTA 0 also turns the histogram into bin regions (largest degrees first)
+//   k_sample_plan    one CTA per tile of 256 destinations: in-tile scan -> block indptr and the
+//                    FINAL output offset of every row (no atomics on output order =>
+//                    deterministic); rows with deg <= f are copied; every other row becomes a
+//                    work item {h_dst, row start, deg, output offset} in its bin's region
+//   k_select_thread  bins with deg < kThreadDeg: ONE THREAD PER ROW (32 rows of similar degree
+//                    per warp); rows it cannot prove exact are appended to a fallback list
+//   k_select_warp    bins with deg >= kThreadDeg, then the fallback list: ONE WARP PER ROW,
+//                    largest rows first, dynamic queue
 #include "common.cuh"
 #include "kernels.h"
 
 namespace gg {
 
 // cumulative sampler statistics: [0] key evaluations the method asks for (sum of deg over rows
-// with deg > fanout), [1] such rows, [2] rows that took the exact fallback path
-__device__ unsigned long long g_sampler_stat[3];
+// with deg > fanout), [1] such rows, [2] rows that took the exact ballot/bisection path,
+// [3] rows the thread-per-row kernel handed to the warp kernel
+__device__ unsigned long long g_sampler_stat[4];
 // test knobs (gg_debug_sampler): compare only the top 32-shift bits when ranking (forces
 // high-word ties), and add to the candidate target (forces list overflow / too few candidates)
 __constant__ int c_rank_shift = 0;
@@ -28,15 +37,41 @@ __constant__ float c_want_add = 0.0f;
 constexpr int kTile = 256;      // destinations per CTA tile
 constexpr int kCand = 256;      // candidate buffer per warp
 constexpr int kWarps = 8;
+constexpr int kBins = 64;       // half-octave degree bins: bin = 2*floor(log2 deg) + next bit
+constexpr int kThreadDegLog2 = 10;
+constexpr uint32_t kThreadDeg = 1u << kThreadDegLog2;   // rows below this degree: one thread per row
+constexpr int kThreadMaxFanout = 16;                    // ... when fanout <= this (candidate list in smem)
+
+// device-side plan of one hop (zeroed before k_sample_count)
+struct SamplePlan {
+  int32_t bin_count[kBins];    // keyed rows per bin (k_sample_count)
+  int32_t bin_start[kBins];    // first item of the bin's region, bins in DESCENDING degree order
+  int32_t bin_cursor[kBins];   // items already placed (k_sample_plan)
+  int32_t n_items;             // keyed rows
+  int32_t n_warp_items;        // items [0, n_warp_items) belong to the warp kernel
+  int32_t n_fallback;          // rows the thread kernel handed over
+  int32_t warp_cursor;         // dynamic queue of the warp kernel
+};
+
+__device__ __forceinline__ int deg_bin(uint32_t deg) {   // deg >= 2
+  const int l = 31 - __clz(deg);
+  return 2 * l + (int)((deg >> (l - 1)) & 1u);
+}
 
 __global__ void __launch_bounds__(kTile)
 k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ nodes,
                int64_t node_pitch, BatchOffsets n_dst, int fanout, int max_tiles,
-               uint8_t* __restrict__ cnt_tmp, int64_t cnt_pitch, int32_t* __restrict__ tile_sums) {
+               uint8_t* __restrict__ cnt_tmp, int64_t cnt_pitch, int32_t* __restrict__ tile_sums,
+               SamplePlan* __restrict__ plan) {
   __shared__ int32_t sm[33];
+  __shared__ int32_t s_bin[kBins];
+  __shared__ unsigned long long s_keys;
   const int b = blockIdx.y, t = blockIdx.x;
   const int nd = n_dst.v[b];
   if (t * kTile >= nd) return;
+  if (threadIdx.x < kBins) s_bin[threadIdx.x] = 0;
+  if (threadIdx.x == 0) s_keys = 0;
+  __syncthreads();
   const int i = t * kTile + threadIdx.x;
   int c = 0;
   unsigned long long keys = 0;
@@ -46,26 +81,34 @@ k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ n
     const int64_t deg = r1 - r0;
     c = deg < fanout ? (int)deg : fanout;
     cnt_tmp[b * cnt_pitch + i] = (uint8_t)c;
-    if (deg > fanout) keys = (unsigned long long)deg;
-  }
-  {
-    const unsigned rows = __popc(__ballot_sync(0xffffffffu, keys != 0));
-#pragma unroll
-    for (int o = 16; o; o >>= 1) keys += __shfl_xor_sync(0xffffffffu, keys, o);
-    if ((threadIdx.x & 31) == 0 && rows) {
-      atomicAdd(&g_sampler_stat[0], keys);
-      atomicAdd(&g_sampler_stat[1], (unsigned long long)rows);
+    if (deg > fanout) {
+      keys = (unsigned long long)deg;
+      atomicAdd(&s_bin[deg_bin((uint32_t)deg)], 1);
     }
   }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) keys += __shfl_xor_sync(0xffffffffu, keys, o);
+  if ((threadIdx.x & 31) == 0 && keys) atomicAdd(&s_keys, keys);
   int32_t total;
-  block_exclusive_scan<int32_t>(c, sm, &total);
+  block_exclusive_scan<int32_t>(c, sm, &total);   // contains __syncthreads
   if (threadIdx.x == 0) tile_sums[b * max_tiles + t] = total;
+  int rows = 0;
+  if (threadIdx.x < kBins) {
+    rows = s_bin[threadIdx.x];
+    if (rows) atomicAdd(&plan->bin_count[threadIdx.x], rows);
+  }
+  if (threadIdx.x < 64) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) rows += __shfl_xor_sync(0xffffffffu, rows, o);
+    if ((threadIdx.x & 31) == 0 && rows) atomicAdd(&g_sampler_stat[1], (unsigned long long)rows);
+  }
+  if (threadIdx.x == 0 && s_keys) atomicAdd(&g_sampler_stat[0], s_keys);
 }
 
 // One CTA per batch (row): in-place exclusive scan of row[0..n_tiles[b]) ; totals[b] = sum.
 __global__ void __launch_bounds__(1024)
 k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, int items_per_tile,
-            int32_t* __restrict__ totals) {
+            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int min_warp_bin) {
   __shared__ int32_t sm[33];
   __shared__ int32_t carry_s;
   const int b = blockIdx.x;
@@ -84,6 +127,20 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
     __syncthreads();
   }
   if (threadIdx.x == 0) totals[b] = carry_s;
+  // bin regions of the hop's work items, largest degrees first (the warp kernel's bins lead)
+  if (plan && b == 0 && threadIdx.x == 0) {
+    int32_t acc = 0, n_warp = 0;
+    for (int k = kBins - 1; k >= 0; --k) {
+      plan->bin_start[k] = acc;
+      plan->bin_cursor[k] = 0;
+      acc += plan->bin_count[k];
+      if (k == min_warp_bin) n_warp = acc;
+    }
+    plan->n_items = acc;
+    plan->n_warp_items = min_warp_bin <= 0 ? acc : n_warp;
+    plan->n_fallback = 0;
+    plan->warp_cursor = 0;
+  }
 }
 
 // ---- the hot loop: one key per lane per step -------------------------------------------------
@@ -277,13 +334,15 @@ __device__ __forceinline__ void fast_step(uint64_t x, uint32_t M, uint32_t& a) {
 }
 
 // Returns true when out[0..f) holds the exact result; false = caller must run warp_select.
+__device__ __forceinline__ float want_candidates(int f) {
+  return fmaxf((float)f + 2.0f + 2.5f * sqrtf((float)f) + c_want_add, 1.0f);
+}
 __device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row, uint32_t deg, int f,
-                                                 uint64_t hdst, uint32_t* scratch,
+                                                 float wantf, uint64_t hdst, uint32_t* scratch,
                                                  int32_t* __restrict__ out) {
   const uint32_t lane = threadIdx.x & 31;
   uint32_t* c_hi = scratch + 2 * kLaneCap * 32;   // [kFastCand]
   uint32_t* c_pos = c_hi + kFastCand;             // [kFastCand]
-  const float wantf = fmaxf((float)f + 2.0f + 2.5f * sqrtf((float)f) + c_want_add, 1.0f);
   const int rshift = c_rank_shift;
   int total;
   if ((float)deg <= wantf && deg <= (uint32_t)kFastCand) {
@@ -377,21 +436,22 @@ __device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row
 
 
 __global__ void __launch_bounds__(kTile)
-k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
-                const int32_t* __restrict__ nodes, int64_t node_pitch, BatchOffsets n_dst,
-                BatchOffsets dst_off, int W, int fanout, int max_tiles,
-                const uint64_t* __restrict__ key_prefix_b, const uint8_t* __restrict__ cnt_tmp,
-                int64_t cnt_pitch, const int32_t* __restrict__ tile_sums,
-                const int32_t* __restrict__ totals, int32_t* __restrict__ blk_indptr,
-                int32_t* __restrict__ edge_off_out, int32_t* __restrict__ src_global) {
+k_sample_plan(const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
+              const int32_t* __restrict__ nodes, int64_t node_pitch, BatchOffsets n_dst,
+              BatchOffsets dst_off, int W, int fanout, int max_tiles,
+              const uint64_t* __restrict__ key_prefix_b, const uint8_t* __restrict__ cnt_tmp,
+              int64_t cnt_pitch, const int32_t* __restrict__ tile_sums,
+              const int32_t* __restrict__ totals, int32_t* __restrict__ blk_indptr,
+              int32_t* __restrict__ edge_off_out, int32_t* __restrict__ src_global,
+              SamplePlan* __restrict__ plan, SampleItems items) {
   __shared__ int32_t sm[33];
-  __shared__ int32_t s_off[kTile + 1];
-  __shared__ int32_t s_edge_base, s_next;
-  __shared__ __align__(16) uint32_t s_scratch[kWarps][kScratchWords];
+  __shared__ int32_t s_edge_base;
+  __shared__ int32_t s_bin[kBins], s_base[kBins];
   const int b = blockIdx.y, t = blockIdx.x;
   const int nd = n_dst.v[b];
   if (t * kTile >= nd) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (threadIdx.x < kBins) s_bin[threadIdx.x] = 0;
   // edge offset of this batch = sum of the totals of the batches before it
   if (wid == 0) {
     int32_t s = 0;
@@ -400,7 +460,6 @@ k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ 
     for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == 0) {
       s_edge_base = s;
-      s_next = kWarps;
       if (t == 0) {
         edge_off_out[b] = s;
         if (b == W - 1) edge_off_out[W] = s + totals[b];
@@ -410,43 +469,165 @@ k_sample_select(const int64_t* __restrict__ indptr, const int32_t* __restrict__ 
   const int i = t * kTile + threadIdx.x;
   const int c = i < nd ? cnt_tmp[b * cnt_pitch + i] : 0;
   int32_t tot;
-  const int32_t ex = block_exclusive_scan<int32_t>(c, sm, &tot);
+  const int32_t ex = block_exclusive_scan<int32_t>(c, sm, &tot);   // contains __syncthreads
   const int32_t tile_base = tile_sums[b * max_tiles + t];
-  s_off[threadIdx.x] = tile_base + ex;
   // block indptr (0-based inside the batch's block); batch b's row starts at dst_off[b] + b
   int32_t* ip = blk_indptr + dst_off.v[b] + b;
   if (i < nd) ip[i] = tile_base + ex;
   if (i == nd - 1) ip[nd] = tile_base + ex + c;
-  __syncthreads();
-  const int n_here = min(kTile, nd - t * kTile);
-  const uint64_t prefix = key_prefix_b[b];
-  int32_t* out_b = src_global + s_edge_base;
-  // warp per destination, dynamic queue inside the tile (rows differ in cost by 1000x)
-  int d = wid;
-  while (d < n_here) {
-    const int32_t v = nodes[b * node_pitch + t * kTile + d];
-    const int64_t r0 = __ldg(indptr + v), r1 = __ldg(indptr + v + 1);
-    const int64_t deg = r1 - r0;
-    int32_t* out = out_b + s_off[d];
-    if (deg <= fanout) {
-      for (int j = lane; j < deg; j += 32) out[j] = __ldg(indices + r0 + j);
+  const int32_t out = s_edge_base + tile_base + ex;
+  int bin = -1, rank = 0;
+  int64_t r0 = 0;
+  uint32_t deg = 0;
+  uint64_t hdst = 0;
+  if (i < nd) {
+    const int32_t v = nodes[b * node_pitch + i];
+    r0 = __ldg(indptr + v);
+    const int64_t d64 = __ldg(indptr + v + 1) - r0;
+    deg = (uint32_t)d64;
+    if (d64 <= fanout) {
+      for (int j = 0; j < (int)deg; ++j) src_global[out + j] = __ldg(indices + r0 + j);
     } else {
-      const uint64_t hdst = key_hdst(prefix, (uint64_t)(uint32_t)v);
-      if (!warp_select_fast(indices + r0, (uint32_t)deg, fanout, hdst, s_scratch[wid], out)) {
-        // rare: lane-list overflow, a bad threshold guess or a high-word tie at the boundary
-        if (lane == 0) atomicAdd(&g_sampler_stat[2], 1ull);
-        uint64_t* s_key = reinterpret_cast<uint64_t*>(s_scratch[wid]);
-        int32_t* s_pos = reinterpret_cast<int32_t*>(s_scratch[wid] + 2 * kCand);
-        warp_select(indices + r0, deg, fanout, hdst, s_key, s_pos, out);
-      }
+      hdst = key_hdst(key_prefix_b[b], (uint64_t)(uint32_t)v);
+      bin = deg_bin(deg);
+      rank = atomicAdd(&s_bin[bin], 1);
     }
-    if (lane == 0) d = atomicAdd(&s_next, 1);
-    d = __shfl_sync(0xffffffffu, d, 0);
+  }
+  __syncthreads();
+  if (threadIdx.x < kBins) {
+    const int n = s_bin[threadIdx.x];
+    s_base[threadIdx.x] = n ? plan->bin_start[threadIdx.x] + atomicAdd(&plan->bin_cursor[threadIdx.x], n) : 0;
+  }
+  __syncthreads();
+  if (bin >= 0) {
+    const int q = s_base[bin] + rank;
+    items.hdst[q] = hdst;
+    items.row0[q] = r0;
+    items.deg[q] = deg;
+    items.out[q] = out;
   }
 }
 
-void sampler_stats(unsigned long long out[3]) {
-  cudaMemcpyFromSymbol(out, g_sampler_stat, 3 * sizeof(unsigned long long));
+// ---- one thread per row (deg < kThreadDeg, fanout <= kThreadMaxFanout) -------------------------
+// Same selection as warp_select_fast, serial in one thread: positions are visited in ascending
+// order, a position whose z_hi passes the odd threshold M appends (z_hi, x_lo) to the thread's
+// own list in shared memory (entry s of thread t at s*1024 + t*4, x_lo 512 bytes further: no bank
+// conflicts), the c candidates are ranked on the high key word (c^2 compares, c ~ 12-27), and
+// `kept == fanout` proves the result.  Anything else goes to the warp kernel's fallback list.
+constexpr int kTThreads = 128;
+constexpr uint32_t kTSlot = kTThreads * 8;   // bytes per list entry across the CTA (z | x)
+
+__device__ __forceinline__ void thread_step(uint64_t x, uint32_t M, uint32_t& a) {
+  const uint32_t xlo = (uint32_t)x;
+  const uint32_t z = key_zhi(xlo, (uint32_t)(x >> 32));
+  if (z <= M) {
+    sts_u32(a, z);
+    sts_u32(a + kTThreads * 4, xlo);
+    a += kTSlot;
+  }
+}
+
+__global__ void __launch_bounds__(kTThreads)
+k_select_thread(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
+                SampleItems items, int32_t* __restrict__ src_global) {
+  extern __shared__ __align__(16) uint32_t s_list[];   // [cap][2][kTThreads]
+  const int n_items = plan->n_items, first = plan->n_warp_items;
+  const float wantf = want_candidates(fanout);
+  const int rshift = c_rank_shift;
+  const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(s_list) + threadIdx.x * 4;
+  const uint32_t a_lim4 = a0 + (uint32_t)(cap - 4) * kTSlot, a_lim1 = a0 + (uint32_t)(cap - 1) * kTSlot;
+  for (int q = first + blockIdx.x * kTThreads + threadIdx.x; q < n_items; q += gridDim.x * kTThreads) {
+    const uint64_t hdst = items.hdst[q];
+    const uint32_t deg = items.deg[q];
+    const float fdeg = (float)deg;
+    const uint32_t M = fdeg <= wantf
+                           ? 0xffffffffu
+                           : ((uint32_t)fminf(__fdividef(wantf, fdeg) * 4294967296.0f, 4294967040.0f) | 1u);
+    uint32_t a = a0;
+    uint64_t x = hdst + kGamma;
+    uint32_t n4 = deg >> 2;
+    while (n4 != 0 && a <= a_lim4) {
+      thread_step(x, M, a);
+      thread_step(x + kGamma, M, a);
+      thread_step(x + 2 * kGamma, M, a);
+      thread_step(x + 3 * kGamma, M, a);
+      x += 4 * kGamma;
+      --n4;
+    }
+    uint32_t rem = (deg & 3u) + 4u * n4;
+    while (rem != 0 && a <= a_lim1) {
+      thread_step(x, M, a);
+      x += kGamma;
+      --rem;
+    }
+    const int c = (int)((a - a0) / kTSlot);
+    int kept = -1;
+    if (rem == 0 && c >= fanout) {
+      for (int s = 0; s < c; ++s) {
+        const uint32_t z = lds_u32(a0 + s * kTSlot);
+        sts_u32(a0 + s * kTSlot, (z ^ (z >> 31)) >> rshift);
+      }
+      // keep flags first (one bit per candidate, cap <= 64), then a loop of exactly `fanout`
+      // steps that every lane of the warp runs together
+      unsigned long long keep = 0;
+      for (int i = 0; i < c; ++i) {
+        const uint32_t mine = lds_u32(a0 + i * kTSlot);
+        int rank = 0;
+        for (int s = 0; s < c; ++s) rank += lds_u32(a0 + s * kTSlot) < mine;
+        keep |= (unsigned long long)(rank < fanout) << i;
+      }
+      kept = __popcll(keep);
+      if (kept == fanout) {
+        const uint32_t hlo = (uint32_t)hdst;
+        const int32_t* row = indices + items.row0[q];
+        int32_t* out = src_global + items.out[q];
+        for (int e = 0; e < fanout; ++e) {
+          const int i = __ffsll((long long)keep) - 1;
+          keep &= keep - 1;
+          const uint32_t pos = (lds_u32(a0 + i * kTSlot + kTThreads * 4) - hlo) * kGammaLoInv - 1u;
+          out[e] = __ldg(row + pos);
+        }
+      }
+    }
+    if (kept != fanout) {
+      // list overflow, too few candidates under the threshold guess, or a high-word tie at the
+      // boundary: the warp kernel redoes the row (and overwrites whatever was written above)
+      items.fallback[atomicAdd(&plan->n_fallback, 1)] = q;
+      atomicAdd(&g_sampler_stat[3], 1ull);
+    }
+  }
+}
+
+// ---- one warp per row: bins with deg >= kThreadDeg (largest first), then the fallback list ----
+__global__ void __launch_bounds__(kWarps * 32)
+k_select_warp(const int32_t* __restrict__ indices, int fanout, SamplePlan* __restrict__ plan,
+              SampleItems items, int32_t* __restrict__ src_global) {
+  __shared__ __align__(16) uint32_t s_scratch[kWarps][kScratchWords];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int n_warp = plan->n_warp_items, n_total = n_warp + plan->n_fallback;
+  const float wantf = want_candidates(fanout);
+  for (;;) {
+    int w = 0;
+    if (lane == 0) w = atomicAdd(&plan->warp_cursor, 1);
+    w = __shfl_sync(0xffffffffu, w, 0);
+    if (w >= n_total) break;
+    const int q = w < n_warp ? w : items.fallback[w - n_warp];
+    const uint64_t hdst = items.hdst[q];
+    const uint32_t deg = items.deg[q];
+    const int32_t* row = indices + items.row0[q];
+    int32_t* out = src_global + items.out[q];
+    if (!warp_select_fast(row, deg, fanout, wantf, hdst, s_scratch[wid], out)) {
+      // rare: lane-list overflow, a bad threshold guess or a high-word tie at the boundary
+      if (lane == 0) atomicAdd(&g_sampler_stat[2], 1ull);
+      uint64_t* s_key = reinterpret_cast<uint64_t*>(s_scratch[wid]);
+      int32_t* s_pos = reinterpret_cast<int32_t*>(s_scratch[wid] + 2 * kCand);
+      warp_select(row, (int64_t)deg, fanout, hdst, s_key, s_pos, out);
+    }
+  }
+}
+
+void sampler_stats(unsigned long long out[4]) {
+  cudaMemcpyFromSymbol(out, g_sampler_stat, 4 * sizeof(unsigned long long));
 }
 cudaError_t sampler_debug(int rank_shift, float want_add) {
   cudaError_t e = cudaMemcpyToSymbol(c_rank_shift, &rank_shift, sizeof(int));
@@ -456,25 +637,47 @@ cudaError_t sampler_debug(int rank_shift, float want_add) {
 
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
                       int items_per_tile, int32_t* totals) {
-  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals);
+  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals, nullptr, 0);
   count_launches(1);
 }
+
+size_t sample_plan_bytes() { return sizeof(SamplePlan); }
 
 void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* indices,
                        const int32_t* nodes, int64_t node_pitch, const BatchOffsets& n_dst,
                        const BatchOffsets& dst_off, int W, int max_nd, int fanout,
                        const uint64_t* key_prefix_b, uint8_t* cnt_tmp, int64_t cnt_pitch,
                        int32_t* tile_sums, int max_tiles, int32_t* totals, int32_t* blk_indptr,
-                       int32_t* edge_off_out, int32_t* src_global) {
+                       int32_t* edge_off_out, int32_t* src_global, const SampleWork& wk) {
   const int tiles = (max_nd + kTile - 1) / kTile;
   dim3 grid(tiles, W);
-  count_launches(3);
+  SamplePlan* plan = static_cast<SamplePlan*>(wk.plan);
+  const bool thread_path = fanout <= kThreadMaxFanout;
+  const int min_warp_bin = thread_path ? 2 * kThreadDegLog2 : 0;
+  cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
+  count_launches(thread_path ? 5 : 4);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
-                                         cnt_tmp, cnt_pitch, tile_sums);
-  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals);
-  k_sample_select<<<grid, kTile, 0, st>>>(indptr, indices, nodes, node_pitch, n_dst, dst_off, W,
-                                          fanout, max_tiles, key_prefix_b, cnt_tmp, cnt_pitch,
-                                          tile_sums, totals, blk_indptr, edge_off_out, src_global);
+                                         cnt_tmp, cnt_pitch, tile_sums, plan);
+  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, min_warp_bin);
+  k_sample_plan<<<grid, kTile, 0, st>>>(indptr, indices, nodes, node_pitch, n_dst, dst_off, W,
+                                        fanout, max_tiles, key_prefix_b, cnt_tmp, cnt_pitch,
+                                        tile_sums, totals, blk_indptr, edge_off_out, src_global,
+                                        plan, wk.items);
+  if (thread_path) {
+    // candidate list capacity: target + 4.5 sigma of a Poisson count, multiple of 4
+    const float want = (float)fanout + 2.0f + 2.5f * sqrtf((float)fanout);
+    const int cap = ((int)ceilf(want + 4.5f * sqrtf(want)) + 3) & ~3;
+    const size_t smem = (size_t)cap * kTSlot;
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaFuncSetAttribute(k_select_thread, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+      attr_set = true;
+    }
+    int per_sm = (int)((220 * 1024) / (smem + 1024));
+    per_sm = per_sm < 1 ? 1 : (per_sm > 12 ? 12 : per_sm);
+    k_select_thread<<<148 * per_sm, kTThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
+  }
+  k_select_warp<<<148 * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
 }
 
 }  // namespace gg
