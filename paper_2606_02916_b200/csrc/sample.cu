@@ -20,6 +20,8 @@
 //                    per warp); rows it cannot prove exact are appended to a fallback list
 //   k_select_warp    bins with deg >= kThreadDeg, then the fallback list: ONE WARP PER ROW,
 //                    largest rows first, dynamic queue
+#include <cstdlib>
+
 #include "common.cuh"
 #include "kernels.h"
 
@@ -38,7 +40,7 @@ constexpr int kTile = 256;      // destinations per CTA tile
 constexpr int kCand = 256;      // candidate buffer per warp
 constexpr int kWarps = 8;
 constexpr int kBins = 64;       // half-octave degree bins: bin = 2*floor(log2 deg) + next bit
-constexpr int kThreadDegLog2 = 10;
+constexpr int kThreadDegLog2 = 9;
 constexpr uint32_t kThreadDeg = 1u << kThreadDegLog2;   // rows below this degree: one thread per row
 constexpr int kThreadMaxFanout = 16;                    // ... when fanout <= this (candidate list in smem)
 
@@ -362,6 +364,10 @@ __device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row
     const uint32_t a_lim4 = a0 + (kLaneCap - 4) * 128, a_lim1 = a0 + (kLaneCap - 1) * 128;
     uint64_t x = hdst + (uint64_t)(lane * K + 1u) * kGamma;
     uint32_t n4 = K >> 2;
+    // The ALU pipe (IADD3 / SHF / LOP3 / ISETP, one warp instruction per 2 clocks) carries half
+    // of this loop (43 of 84 instructions per 4 keys) and is its limiter.  Moving the state
+    // updates to the FMA pipe (IMAD.WIDE with a 64-bit addend) was tried three ways; ptxas splits
+    // the addend back into IADD3 + IMAD.X every time, so the carried adds stay.
     while (n4 != 0 && a <= a_lim4) {
       fast_step(x, M, a);
       fast_step(x + kGamma, M, a);
@@ -511,30 +517,42 @@ k_sample_plan(const int64_t* __restrict__ indptr, const int32_t* __restrict__ in
 // ---- one thread per row (deg < kThreadDeg, fanout <= kThreadMaxFanout) -------------------------
 // Same selection as warp_select_fast, serial in one thread: positions are visited in ascending
 // order, a position whose z_hi passes the odd threshold M appends (z_hi, x_lo) to the thread's
-// own list in shared memory (entry s of thread t at s*1024 + t*4, x_lo 512 bytes further: no bank
-// conflicts), the c candidates are ranked on the high key word (c^2 compares, c ~ 12-27), and
+// own list in shared memory (entry s of thread t: z at s*768 + t*4, the low half of x_lo at
+// s*768 + 512 + t*2: no bank conflicts), the c candidates are ranked on the high key word (c^2 compares, c ~ 12-27), and
 // `kept == fanout` proves the result.  Anything else goes to the warp kernel's fallback list.
 constexpr int kTThreads = 128;
-constexpr uint32_t kTSlot = kTThreads * 8;   // bytes per list entry across the CTA (z | x)
+constexpr uint32_t kTSlot = kTThreads * 6;   // bytes per list entry across the CTA (z u32 | x u16)
 
-__device__ __forceinline__ void thread_step(uint64_t x, uint32_t M, uint32_t& a) {
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
+  unsigned short v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
+  return v;
+}
+// a: address of the thread's next z slot, ax: of its next x slot (low 16 bits of the state's low
+// word are enough to recover a position < 65536)
+__device__ __forceinline__ void thread_step(uint64_t x, uint32_t M, uint32_t& a, uint32_t& ax) {
   const uint32_t xlo = (uint32_t)x;
   const uint32_t z = key_zhi(xlo, (uint32_t)(x >> 32));
   if (z <= M) {
     sts_u32(a, z);
-    sts_u32(a + kTThreads * 4, xlo);
+    sts_u16(ax, xlo);
     a += kTSlot;
+    ax += kTSlot;
   }
 }
 
 __global__ void __launch_bounds__(kTThreads)
 k_select_thread(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
                 SampleItems items, int32_t* __restrict__ src_global) {
-  extern __shared__ __align__(16) uint32_t s_list[];   // [cap][2][kTThreads]
+  extern __shared__ __align__(16) uint32_t s_list[];   // [cap]{z u32[kTThreads], x u16[kTThreads]}
   const int n_items = plan->n_items, first = plan->n_warp_items;
   const float wantf = want_candidates(fanout);
   const int rshift = c_rank_shift;
   const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(s_list) + threadIdx.x * 4;
+  const uint32_t ax0 = (uint32_t)__cvta_generic_to_shared(s_list) + kTThreads * 4 + threadIdx.x * 2;
   const uint32_t a_lim4 = a0 + (uint32_t)(cap - 4) * kTSlot, a_lim1 = a0 + (uint32_t)(cap - 1) * kTSlot;
   for (int q = first + blockIdx.x * kTThreads + threadIdx.x; q < n_items; q += gridDim.x * kTThreads) {
     const uint64_t hdst = items.hdst[q];
@@ -543,39 +561,55 @@ k_select_thread(const int32_t* __restrict__ indices, int fanout, int cap, Sample
     const uint32_t M = fdeg <= wantf
                            ? 0xffffffffu
                            : ((uint32_t)fminf(__fdividef(wantf, fdeg) * 4294967296.0f, 4294967040.0f) | 1u);
-    uint32_t a = a0;
+    uint32_t a = a0, ax = ax0;
     uint64_t x = hdst + kGamma;
     uint32_t n4 = deg >> 2;
     while (n4 != 0 && a <= a_lim4) {
-      thread_step(x, M, a);
-      thread_step(x + kGamma, M, a);
-      thread_step(x + 2 * kGamma, M, a);
-      thread_step(x + 3 * kGamma, M, a);
+      thread_step(x, M, a, ax);
+      thread_step(x + kGamma, M, a, ax);
+      thread_step(x + 2 * kGamma, M, a, ax);
+      thread_step(x + 3 * kGamma, M, a, ax);
       x += 4 * kGamma;
       --n4;
     }
     uint32_t rem = (deg & 3u) + 4u * n4;
     while (rem != 0 && a <= a_lim1) {
-      thread_step(x, M, a);
+      thread_step(x, M, a, ax);
       x += kGamma;
       --rem;
     }
     const int c = (int)((a - a0) / kTSlot);
     int kept = -1;
     if (rem == 0 && c >= fanout) {
+      // final key word of every candidate; pad to a multiple of 4 with all-ones (cap is one)
       for (int s = 0; s < c; ++s) {
         const uint32_t z = lds_u32(a0 + s * kTSlot);
         sts_u32(a0 + s * kTSlot, (z ^ (z >> 31)) >> rshift);
       }
-      // keep flags first (one bit per candidate, cap <= 64), then a loop of exactly `fanout`
-      // steps that every lane of the warp runs together
-      unsigned long long keep = 0;
-      for (int i = 0; i < c; ++i) {
-        const uint32_t mine = lds_u32(a0 + i * kTSlot);
-        int rank = 0;
-        for (int s = 0; s < c; ++s) rank += lds_u32(a0 + s * kTSlot) < mine;
-        keep |= (unsigned long long)(rank < fanout) << i;
+      const int c4 = (c + 3) & ~3;
+      for (int s = c; s < c4; ++s) sts_u32(a0 + s * kTSlot, 0xffffffffu);
+      // the fanout-th smallest DISTINCT value, one round per rank: each round takes the minimum
+      // of (v - last - 1) mod 2^32, which orders the values above `last` before everything else
+      uint32_t lastp1 = 0, thr = 0;
+      bool wrapped = false;
+      for (int r = 0; r < fanout; ++r) {
+        wrapped = wrapped || (r > 0 && lastp1 == 0);
+        uint32_t best = 0xffffffffu;
+        for (int s = 0; s < c4; s += 4) {
+          const uint32_t w0 = lds_u32(a0 + s * kTSlot) - lastp1;
+          const uint32_t w1 = lds_u32(a0 + (s + 1) * kTSlot) - lastp1;
+          const uint32_t w2 = lds_u32(a0 + (s + 2) * kTSlot) - lastp1;
+          const uint32_t w3 = lds_u32(a0 + (s + 3) * kTSlot) - lastp1;
+          best = min(min(best, w0), min(w1, min(w2, w3)));
+        }
+        thr = best + lastp1;
+        lastp1 = thr + 1u;
       }
+      // keep flags (one bit per candidate, cap <= 64): fewer than `fanout` distinct values or a
+      // tie at or below the threshold gives kept != fanout
+      unsigned long long keep = 0;
+      for (int i = 0; i < c; ++i) keep |= (unsigned long long)(lds_u32(a0 + i * kTSlot) <= thr) << i;
+      if (wrapped) keep = 0;
       kept = __popcll(keep);
       if (kept == fanout) {
         const uint32_t hlo = (uint32_t)hdst;
@@ -584,7 +618,7 @@ k_select_thread(const int32_t* __restrict__ indices, int fanout, int cap, Sample
         for (int e = 0; e < fanout; ++e) {
           const int i = __ffsll((long long)keep) - 1;
           keep &= keep - 1;
-          const uint32_t pos = (lds_u32(a0 + i * kTSlot + kTThreads * 4) - hlo) * kGammaLoInv - 1u;
+          const uint32_t pos = ((lds_u16(ax0 + i * kTSlot) - hlo) * kGammaLoInv - 1u) & 0xffffu;
           out[e] = __ldg(row + pos);
         }
       }
@@ -653,7 +687,13 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
   dim3 grid(tiles, W);
   SamplePlan* plan = static_cast<SamplePlan*>(wk.plan);
   const bool thread_path = fanout <= kThreadMaxFanout;
-  const int min_warp_bin = thread_path ? 2 * kThreadDegLog2 : 0;
+  static int deg_log2 = -1;
+  if (deg_log2 < 0) {
+    const char* e = getenv("GG_THREAD_DEG_LOG2");
+    deg_log2 = e ? atoi(e) : kThreadDegLog2;
+    if (deg_log2 > 16) deg_log2 = 16;
+  }
+  const int min_warp_bin = thread_path ? 2 * deg_log2 : 0;
   cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
   count_launches(thread_path ? 5 : 4);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
