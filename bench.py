@@ -54,14 +54,48 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic():
-    """dram read+write bytes per k_gather launch from the committed ncu --set full summary."""
-    p = os.path.join(ROOT, "profiles", "r01_gather_ncu_summary.txt")
+def ncu_traffic(name):
+    """dram read+write bytes per launch from a committed ncu --set full summary under profiles/."""
+    p = os.path.join(ROOT, "profiles", name)
     if os.path.exists(p):
         for line in open(p):
             if line.startswith("traffic_bytes_per_launch:"):
                 return float(line.split(":")[1])
     return None
+
+
+# Issue slots the key loop of k_select_warp / k_select_thread spends per key (84 SASS
+# instructions per 4 keys: DESIGN.md Sec. 6); the ALU roofline is one warp instruction per clock
+# per SM sub-partition.
+KEY_ISSUE_SLOTS = 21.0
+SM_COUNT, SMSP_PER_SM = 148, 4
+
+
+def alu_peak_gkeys(sm_mhz):
+    return SM_COUNT * SMSP_PER_SM * 32 * sm_mhz * 1e6 / KEY_ISSUE_SLOTS / 1e9
+
+
+class EnergyMeter:
+    """NVML total-energy counter (mJ) around the timed region (north star: NVML energy per epoch)."""
+
+    def __init__(self, index):
+        self.h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.nv.nvmlDeviceGetTotalEnergyConsumption(self.h)
+        except Exception:
+            self.h = None
+
+    def read_mj(self):
+        if self.h is None:
+            return None
+        try:
+            return float(self.nv.nvmlDeviceGetTotalEnergyConsumption(self.h))
+        except Exception:
+            return None
 
 
 class ClockSampler:
@@ -226,6 +260,7 @@ def run_ours(args):
     # (long-running, ALU-bound) sampling kernels whenever an SM has room for both
     stream = torch.cuda.Stream(dev, priority=-1)
     torch.cuda.set_stream(stream)
+    energy = EnergyMeter(local_rank)
     link_peak = host_link_peak(dev)
 
     # size the output buffer from the first window (|N_b| varies little between batches)
@@ -263,6 +298,8 @@ def run_ours(args):
         gdist.barrier()
         if clocks:
             clocks.start()
+        s0 = binding.sampler_stats() if profile else None
+        mj0 = energy.read_mj() if profile else None
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
         e0.record(stream)
@@ -271,13 +308,18 @@ def run_ours(args):
         e1.record(stream)
         torch.cuda.synchronize(dev)
         wall = time.perf_counter() - t0
+        mj1 = energy.read_mj() if profile else None
+        s1 = binding.sampler_stats() if profile else None
         gdist.barrier()
         ck = clocks.stop() if clocks else None
         sec = e0.elapsed_time(e1) / 1e3
         prof = g.profile_get() if profile else None
         if profile:
             g.profile_enable(False)
-        return dict(sec=sec, wall=wall, launches=binding.launch_count() - l0, prof=prof, clocks=ck)
+        samp = {k: s1[k] - s0[k] for k in s0} if profile else None
+        joules = (mj1 - mj0) / 1e3 if (mj0 is not None and mj1 is not None) else None
+        return dict(sec=sec, wall=wall, launches=binding.launch_count() - l0, prof=prof, clocks=ck,
+                    sampler=samp, joules=joules)
 
     # ---- headline: device-resident inputs --------------------------------------------------
     main = timed(W, args.steps, args.warmup, profile=True, clocks=ClockSampler(local_rank))
@@ -322,15 +364,31 @@ def run_ours(args):
 
     if rank != 0:
         return
-    # ---- roofline of the dominant kernel (slot-map gather) ------------------------------------
+    # ---- rooflines: the dominant kernel group (a-1 sampling, ALU-bound) and the gather (HBM) ----
     peak, peak_src = measured_peaks()
     pg = main["prof"]["gather"]
     ach = pg["bytes"] / (pg["ms"] * 1e-3) / 1e9 if pg["ms"] > 0 else 0.0
-    roof = {"bound": "hbm", "kernel": "k_gather", "achieved": ach, "peak": peak, "unit": "GB/s",
-            "frac": ach / peak, "traffic": ncu_traffic(), "peak_source": peak_src,
-            "launches": pg["regions"], "avg_launch_us": 1e3 * pg["ms"] / max(pg["regions"], 1),
-            "algorithmic_bytes_per_launch": pg["bytes"] / max(pg["regions"], 1),
-            "share_of_step": pg["ms"] * 1e-3 / main["sec"]}
+    roof_gather = {"bound": "hbm", "kernel": "k_gather", "achieved": ach, "peak": peak, "unit": "GB/s",
+                   "frac": ach / peak, "traffic": ncu_traffic("r01_gather_ncu_summary.txt"), "peak_source": peak_src,
+                   "launches": pg["regions"], "avg_launch_us": 1e3 * pg["ms"] / max(pg["regions"], 1),
+                   "algorithmic_bytes_per_launch": pg["bytes"] / max(pg["regions"], 1),
+                   "share_of_step": pg["ms"] * 1e-3 / main["sec"],
+                   "note": "live: shares the SMs with the sampler on the side stream; alone it runs at the ncu time in profiles/"}
+    ps = main["prof"]["sample"]
+    sm_mhz = (main["clocks"] or {}).get("sm_max_mhz") or 1965.0
+    keys = main["sampler"]["keys"]
+    gk = keys / (ps["ms"] * 1e-3) / 1e9 if ps["ms"] > 0 else 0.0
+    gk_peak = alu_peak_gkeys(sm_mhz)
+    roof = {"bound": "alu", "kernel": "a-1 sampling (k_sample_count/plan + k_select_thread + k_select_warp per hop)",
+            "achieved": gk, "peak": gk_peak, "unit": "Gkey/s", "frac": gk / gk_peak,
+            "traffic": ncu_traffic("r01_sample_ncu_summary.txt"),
+            "peak_source": "derived: %d SMs x %d sub-partitions x 1 warp instruction/clk x 32 lanes x %.0f MHz / %.0f issue "
+                           "slots per key (DESIGN.md Sec. 6)" % (SM_COUNT, SMSP_PER_SM, sm_mhz, KEY_ISSUE_SLOTS),
+            "launches": ps["regions"], "avg_launch_us": 1e3 * ps["ms"] / max(ps["regions"], 1),
+            "algorithmic_keys_per_launch": keys / max(ps["regions"], 1),
+            "keyed_rows_per_step": main["sampler"]["rows"] / args.steps,
+            "fallback_rows_per_step": main["sampler"]["fallbacks"] / args.steps,
+            "share_of_step": ps["ms"] * 1e-3 / main["sec"]}
     stages = {}
     for k, v in main["prof"].items():
         if v["regions"]:
@@ -353,7 +411,11 @@ def run_ours(args):
                          % (w.num_nodes * w.row_bytes / 1e6, tr_acc["n_access"] / n_b * w.row_bytes / 1e6)},
         "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
-        "roofline": roof, "stages": stages, "vs_W": vs_w,
+        "roofline": roof, "roofline_gather": roof_gather, "stages": stages, "vs_W": vs_w,
+        "gpu_stall_ms_per_step": (main["prof"]["wait"]["ms"] / args.steps) if "wait" in main["prof"] else None,
+        "energy": {"J_per_step": (main["joules"] / args.steps) if main["joules"] is not None else None,
+                   "avg_W": (main["joules"] / main["wall"]) if main["joules"] is not None else None,
+                   "source": "NVML total energy counter over the timed region"},
         "staging": {"host_link_bytes_per_step": int(tr_acc["bulk_bytes"]), "bulk_copies_per_step": tr_acc["bulk_copies"],
                     "h2d_GB/s": tr_acc["bulk_bytes"] / (tr_acc["h2d_ms"] * 1e-3) / 1e9 if tr_acc["h2d_ms"] > 0 else None,
                     "host_link_peak_GB/s": link_peak,
