@@ -407,6 +407,8 @@ def make_workload(name: str, device="cpu", pin: Optional[bool] = None,
             else:
                 feature_rows(lo, hi - lo, cfg["dim"], dtype, fseed, "cpu", out=host)
             parts.append(host)
+    if torch.device(device).type == "cuda":
+        torch.cuda.empty_cache()    # the generator's sort temporaries (tens of GB for "large")
     batches = train_batches(n, cfg["n_train"], cfg["batch"], substream(ms, 300))
     if cfg["max_batches"]:
         batches = batches[:cfg["max_batches"]]

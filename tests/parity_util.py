@@ -7,17 +7,22 @@ from paper_2606_02916_b200 import epoch as ep
 
 
 def oracle_parts(w):
-    feat = w.host_features()
-    po = w.part_offsets
-    return feat, [np.ascontiguousarray(feat[po[m]:po[m + 1]]) for m in range(len(po) - 1)]
+    """Per-owner [rows, row_bytes] uint8 host views of the feature store (no concatenation:
+    the Large config's store is 28 GB)."""
+    parts = []
+    for p in w.feat_parts:
+        h = p if p.device.type == "cpu" else p.cpu()
+        parts.append(h.contiguous().view(torch.uint8).view(h.shape[0], -1).numpy())
+    return parts
 
 
 def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, max_cache_rows=0,
-                check_features=True, cache_samples=64, host_threads=0):
+                check_features=True, cache_samples=64, host_threads=0, oracle_threads=1, host_graph=None,
+                parts=None):
     """Runs one epoch on the GPU and on the oracle; asserts bit-exact agreement everywhere.
     Returns a small summary dict."""
     batches = w.batches if max_batches is None else w.batches[:max_batches]
-    indptr, indices = w.host_graph()
+    indptr, indices = host_graph if host_graph is not None else w.host_graph()
     og = ggo.Graph(indptr, indices)
     po = w.part_offsets
     P = len(po) - 1
@@ -25,7 +30,8 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
     cache_rows = min(max_cache_rows, n_remote_nodes) if max_cache_rows > 0 else n_remote_nodes
     eff = cache_rows if n_hot < 0 else min(n_hot, cache_rows)        # reading S9
     ostate = ggo.State(og.n, po, w.local_part, eff, carry_over)
-    feat, parts = oracle_parts(w) if check_features else (None, None)
+    if parts is None and check_features:
+        parts = oracle_parts(w)
 
     g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=carry_over, max_window=max(W, 1),
                                staging_mode=staging_mode, max_cache_rows=max_cache_rows,
@@ -40,6 +46,15 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
         if bi not in obatches:
             obatches[bi] = ggo.Batch(og, batches[bi], w.fanouts, w.seed, bi)
         return obatches[bi]
+
+    if oracle_threads > 1:
+        # the oracle's batches are independent calls (ctypes releases the GIL): run them side by
+        # side; the oracle itself is unchanged and single-threaded per batch
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(oracle_threads) as ex:
+            for bi, ob in zip(range(len(batches)),
+                              ex.map(lambda bi: ggo.Batch(og, batches[bi], w.fanouts, w.seed, bi), range(len(batches)))):
+                obatches[bi] = ob
 
     # the oracle advances its cache window by window in the same order
     for k, win in enumerate(wins):
@@ -91,7 +106,10 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
         assert np.array_equal(t["miss"], np.stack(ow.miss)), "per-owner miss counts"
         if check_features and len(ow.hot) and cache_samples:
             ids = ow.hot[np.linspace(0, len(ow.hot) - 1, min(cache_samples, len(ow.hot))).astype(np.int64)]
-            assert np.array_equal(g.cache_read(wid, ids), np.take(feat, ids, axis=0)), "cache rows"
+            want = ggo.gather(ids, po, parts, w.row_bytes)
+            got = g.cache_read(wid, ids)
+            got = np.ascontiguousarray(got).view(np.uint8).reshape(len(ids), -1)
+            assert np.array_equal(got, want), "cache rows"
         stats["windows"] += 1
 
     ep.run_epoch(g, batches, w.fanouts, W, features, on_batch=on_batch, on_window=on_window)

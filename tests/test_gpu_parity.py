@@ -203,3 +203,32 @@ def test_dense_full_size_first_window(workload, dev):
     w = workload("dense", dev)
     s = pu.check_epoch(w, W=4, n_hot=-1, max_batches=4, cache_samples=128)
     assert s["batches"] == 4
+
+
+def test_large_full_size_first_windows(dev):
+    """configs[4] at full size: R-MAT, N = 111,000,000, 1.6 B directed edges (int64 offsets),
+    dim 128 bf16, 83 M remote rows in pinned host memory.  The first 8 windows at W=4 (32
+    mini-batches) and the same batches as 2 windows at W=16 with a finite budget, every array
+    against the oracle (its 32 batches are sampled once, 16 at a time on the host cores)."""
+    import os
+    from paper_2606_02916_b200 import inputs
+    free_b, _ = torch.cuda.mem_get_info()
+    try:
+        host_gb = os.sysconf("SC_PHYS_PAGES") * os.sysconf("SC_PAGE_SIZE") / 1e9
+    except (ValueError, OSError):
+        host_gb = 0.0
+    if free_b < 120e9 or host_gb < 100:
+        pytest.skip("needs ~120 GB of HBM and ~100 GB of host memory")
+    w = inputs.make_workload("large", device=dev)
+    assert w.num_nodes == 111_000_000 and w.indices.numel() == 1_600_000_000
+    hg = w.host_graph()
+    parts = pu.oracle_parts(w)
+    thr = min(16, os.cpu_count() or 1)
+    s = pu.check_epoch(w, W=4, n_hot=-1, max_batches=32, cache_samples=64, oracle_threads=thr,
+                       host_graph=hg, parts=parts)
+    assert s["windows"] == 8 and s["batches"] == 32 and s["misses"] == 0
+    s = pu.check_epoch(w, W=16, n_hot=200_000, max_batches=32, cache_samples=64, oracle_threads=thr,
+                       host_graph=hg, parts=parts)
+    assert s["windows"] == 2 and s["misses"] > 0
+    del w, hg, parts
+    torch.cuda.empty_cache()
