@@ -341,6 +341,25 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     g.cache_reset()
 
+    # ---- the same kernels with the pipeline switched off: sample+stage a window, wait, then
+    # serve it, so no two of the library's streams compete for the SMs (one epoch, untimed as a
+    # whole; only the per-kernel event pairs are read).  Says what the kernels do alone; the
+    # live fractions above say what they do inside the overlapped step.
+    g.profile_enable(True)
+    s0 = binding.sampler_stats()
+    for k, win in enumerate(ep.windows_of(n_b, W)):
+        g.window_stage(7 * 10 ** 6 + k, win.start, [batches[i] for i in win], w.fanouts)
+        g.batch_info(7 * 10 ** 6 + k, 0)
+        g.trace(7 * 10 ** 6 + k, len(win))           # synchronises the window's staging
+        for j in range(len(win)):
+            g.batch_gather(7 * 10 ** 6 + k, j, feats, stream)
+        torch.cuda.synchronize(dev)
+        g.window_release(7 * 10 ** 6 + k)
+    serial_prof = g.profile_get()
+    serial_keys = binding.sampler_stats()["keys"] - s0["keys"]
+    g.profile_enable(False)
+    g.cache_reset()
+
     # ---- end to end: results read back to pinned host buffers every batch -------------------
     e2e = None
     if not args.no_e2e:
@@ -389,6 +408,19 @@ def run_ours(args):
             "keyed_rows_per_step": main["sampler"]["rows"] / args.steps,
             "fallback_rows_per_step": main["sampler"]["fallbacks"] / args.steps,
             "share_of_step": ps["ms"] * 1e-3 / main["sec"]}
+    sp_s, sp_g = serial_prof["sample"], serial_prof["gather"]
+    serial = {
+        "what": "same epoch with the pipeline off (stage a window, wait, serve it): kernels run without SM contention",
+        "sample_Gkey/s": serial_keys / (sp_s["ms"] * 1e-3) / 1e9 if sp_s["ms"] > 0 else None,
+        "sample_frac_of_alu_peak": (serial_keys / (sp_s["ms"] * 1e-3) / 1e9 / gk_peak) if sp_s["ms"] > 0 else None,
+        "gather_GB/s": sp_g["bytes"] / (sp_g["ms"] * 1e-3) / 1e9 if sp_g["ms"] > 0 else None,
+        "gather_frac_of_hbm_peak": (sp_g["bytes"] / (sp_g["ms"] * 1e-3) / 1e9 / peak) if sp_g["ms"] > 0 else None,
+        "h2d_GB/s": (serial_prof["stage_copy"]["bytes"] / (serial_prof["stage_copy"]["ms"] * 1e-3) / 1e9)
+        if serial_prof["stage_copy"]["ms"] > 0 else None,
+        "ms_per_epoch": {k: round(v["ms"], 3) for k, v in serial_prof.items() if v["regions"]},
+    }
+    if serial["h2d_GB/s"]:
+        serial["h2d_frac_of_link_peak"] = serial["h2d_GB/s"] / link_peak
     stages = {}
     for k, v in main["prof"].items():
         if v["regions"]:
@@ -411,7 +443,7 @@ def run_ours(args):
                          % (w.num_nodes * w.row_bytes / 1e6, tr_acc["n_access"] / n_b * w.row_bytes / 1e6)},
         "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
-        "roofline": roof, "roofline_gather": roof_gather, "stages": stages, "vs_W": vs_w,
+        "roofline": roof, "roofline_gather": roof_gather, "kernels_alone": serial, "stages": stages, "vs_W": vs_w,
         "gpu_stall_ms_per_step": (main["prof"]["wait"]["ms"] / args.steps) if "wait" in main["prof"] else None,
         "energy": {"J_per_step": (main["joules"] / args.steps) if main["joules"] is not None else None,
                    "avg_W": (main["joules"] / main["wall"]) if main["joules"] is not None else None,
