@@ -262,6 +262,49 @@ gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);
  * (0, 0.0f) restores the defaults.  Must not be called while a window is being staged. */
 gg_status gg_debug_sampler(int32_t rank_shift, float want_add);
 
+/* ---- NEXT-1: trace simulator + analytical energy model ----
+ * Coefficients of PAPER.md:128 (the energy profiler's output), per owner m:
+ *   eps_init[m] J per transfer; eps_payload(m,x) = eps_pay_a[m] + eps_pay_b[m]*x J for x > 0 rows
+ *   and 0 for x = 0 ("a linear fit ... as a function of transfer size"; DESIGN.md
+ *   reading S24); lam_* the latency surrogates in seconds, same form; bw_bytes_per_s the
+ *   aggregate bandwidth ceiling; p_idle_w the accelerator's idle power.  Entries of the local
+ *   owner are never used. */
+typedef struct {
+  double eps_init[GG_MAX_PARTS], eps_pay_a[GG_MAX_PARTS], eps_pay_b[GG_MAX_PARTS];
+  double lam_init[GG_MAX_PARTS], lam_pay_a[GG_MAX_PARTS], lam_pay_b[GG_MAX_PARTS];
+  double bw_bytes_per_s, p_idle_w;
+} gg_energy_model;
+
+/* One candidate W: event tallies of the single pass over the trace and Eqs. (1)-(3).
+ *   rebuild_events = sum_k sum_m I[Delta_{k,m} != {}], rebuild_rows = sum |Delta_{k,m}|   (Eq. 1)
+ *   miss_events    = sum_b sum_m I[M_{b,m} != {}],     miss_rows    = sum |M_{b,m}|       (Eq. 2)
+ *   t_stall = sum over rebuild and miss events of max(slowest single-owner transfer,
+ *             event bytes / BW) (Eq. 3 prose, reading S20); e_stall = p_idle * t_stall
+ *   e_phy = (e_rebuild + e_miss) + e_stall; hit_ratio = hit_cache / (hit_cache + miss_rows)
+ * z(W) of PAPER.md:182 = (rebuild_events, miss_events, t_stall, hit_ratio). */
+typedef struct {
+  int32_t W, n_windows;
+  int64_t rebuild_events, miss_events, rebuild_rows, miss_rows;
+  int64_t n_access, n_remote_access, hit_local, hit_cache;
+  double e_rebuild, e_miss, t_stall, e_stall, e_phy, hit_ratio;
+} gg_sim_result;
+
+/* Samples the epoch's B mini-batches once (a-1/a-2; batch i keyed with first_batch_index+i),
+ * keeps the trace T in HBM, and replays it for each candidate window size Ws[0..nW) with the
+ * graph's n_hot / carry_over / owner map: window unique+count, hot-set select, rebuild delta
+ * against the previous cache state (C_0 = {}), per-batch hit / miss classification -- no
+ * feature row is moved.  out[i] receives candidate i; *best = index of the smallest e_phy
+ * (W* = argmin, PAPER.md:186 with L(W) = 0; ties -> the earlier candidate).
+ * Optional parity exports (host, may be NULL): delta_out[(sum of windows over candidates) * P]
+ * = |Delta_{k,m}| candidate-major; miss_out[nW * B * P] = |M_{b,m}|.
+ * seeds / batch_offsets / fanouts / Ws / model / out: host.  Synchronous; requires that no
+ * window is live (GG_ERR_STATE otherwise) and leaves the cache state empty.
+ * Errors: as gg_window_stage for the batch arguments; Ws[i] outside [1, max_window]. */
+gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_t* batch_offsets, int32_t B,
+                      uint64_t first_batch_index, const int32_t* fanouts, int32_t num_layers,
+                      const int32_t* Ws, int32_t nW, const gg_energy_model* model,
+                      gg_sim_result* out, int32_t* best, int64_t* delta_out, int64_t* miss_out);
+
 const char* gg_last_error(void);
 const char* gg_version(void);
 

@@ -68,11 +68,24 @@ class gg_profile(C.Structure):
     _fields_ = [("ms", C.c_double * 9), ("regions", i64 * 9), ("bytes", i64 * 9)]
 
 
+class gg_energy_model(C.Structure):
+    _fields_ = [(n, C.c_double * GG_MAX_PARTS) for n in
+                ("eps_init", "eps_pay_a", "eps_pay_b", "lam_init", "lam_pay_a", "lam_pay_b")] + \
+               [("bw_bytes_per_s", C.c_double), ("p_idle_w", C.c_double)]
+
+
+class gg_sim_result(C.Structure):
+    _fields_ = [("W", i32), ("n_windows", i32)] + \
+               [(n, i64) for n in ("rebuild_events", "miss_events", "rebuild_rows", "miss_rows",
+                                   "n_access", "n_remote_access", "hit_local", "hit_cache")] + \
+               [(n, C.c_double) for n in ("e_rebuild", "e_miss", "t_stall", "e_stall", "e_phy", "hit_ratio")]
+
+
 PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage_copy", "carry", "wait"]
 
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
-           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler"]
+           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_simulate"]
 
 _lib = None
 
@@ -111,6 +124,8 @@ def load_library(path: Optional[str] = None):
     lib.gg_key.restype = u64
     lib.gg_sampler_stats.argtypes = [P(u64), P(u64), P(u64)]
     lib.gg_debug_sampler.argtypes = [i32, C.c_float]
+    lib.gg_simulate.argtypes = [vp, vp, vp, i32, u64, vp, i32, vp, i32, P(gg_energy_model), P(gg_sim_result),
+                                P(i32), vp, vp]
     lib.gg_last_error.restype = C.c_char_p
     lib.gg_version.restype = C.c_char_p
     for s in SYMBOLS:
@@ -219,6 +234,43 @@ class Graph:
         fo = np.ascontiguousarray(fanouts, dtype=np.int32)
         self._check(self.lib.gg_window_stage(self.h, window_id, first_batch_index, seeds.ctypes.data,
                                              off.ctypes.data, len(batches), fo.ctypes.data, len(fo)))
+
+    # -- gg_simulate (NEXT-1) ----------------------------------------------------------------
+    def simulate(self, batches: Sequence[np.ndarray], fanouts: Sequence[int], candidates: Sequence[int],
+                 model: Dict, first_batch_index: int = 0, export: bool = False) -> Dict:
+        """Trace simulator + Eqs. (1)-(3) for every candidate W.  `model`: dict with per-owner
+        lists eps_init, eps_pay_a, eps_pay_b, lam_init, lam_pay_a, lam_pay_b and scalars bw, p_idle.
+        Returns {"best": W*, "results": [dict per candidate]} (+ "delta"/"miss" arrays if export)."""
+        seeds = np.ascontiguousarray(np.concatenate([np.asarray(b, dtype=np.int32) for b in batches]), dtype=np.int32)
+        off = np.zeros(len(batches) + 1, dtype=np.int64)
+        off[1:] = np.cumsum([len(b) for b in batches])
+        fo = np.ascontiguousarray(fanouts, dtype=np.int32)
+        ws = np.ascontiguousarray(candidates, dtype=np.int32)
+        em = gg_energy_model()
+        for name in ("eps_init", "eps_pay_a", "eps_pay_b", "lam_init", "lam_pay_a", "lam_pay_b"):
+            arr = getattr(em, name)
+            for m, v in enumerate(model[name]):
+                arr[m] = float(v)
+        em.bw_bytes_per_s, em.p_idle_w = float(model["bw"]), float(model["p_idle"])
+        B, nW = len(batches), len(ws)
+        res = (gg_sim_result * nW)()
+        best = i32(0)
+        Ks = [-(-B // int(W)) for W in ws]
+        d_out = np.zeros(sum(Ks) * self.P, dtype=np.int64) if export else None
+        m_out = np.zeros(nW * B * self.P, dtype=np.int64) if export else None
+        self._check(self.lib.gg_simulate(self.h, seeds.ctypes.data, off.ctypes.data, B, first_batch_index,
+                                         fo.ctypes.data, len(fo), ws.ctypes.data, nW, C.byref(em), res,
+                                         C.byref(best), d_out.ctypes.data if export else None,
+                                         m_out.ctypes.data if export else None))
+        out = {"best": int(ws[best.value]),
+               "results": [{n: getattr(r, n) for n, _ in gg_sim_result._fields_} for r in res]}
+        if export:
+            out["delta"], c = [], 0
+            for K in Ks:
+                out["delta"].append(d_out[c:c + K * self.P].reshape(K, self.P))
+                c += K * self.P
+            out["miss"] = m_out.reshape(nW, B, self.P)
+        return out
 
     # -- gg_batch_info / gg_batch_gather -----------------------------------------------------
     def _unpack(self, o: gg_batch_out) -> Dict:

@@ -1297,3 +1297,202 @@ gg_status gg_cache_reset(gg_graph* g) {
 }
 
 }  // extern "C"
+
+// =============================== NEXT-1: gg_simulate =========================================
+namespace gg {
+// hot-set threshold t and quota of count == t nodes from the histogram of remote counts (a-4)
+static void hot_threshold(const int32_t* hist, int64_t n_remote, int64_t n_hot_eff, int64_t* n_hot,
+                          int32_t* thr, uint32_t* quota) {
+  *thr = 0;
+  *quota = 0;
+  if (n_remote <= n_hot_eff) {
+    *n_hot = n_remote;
+    return;
+  }
+  *n_hot = n_hot_eff;
+  int64_t above = 0;
+  int t;
+  for (t = 255; t >= 1; --t) {
+    if (above + hist[t] > *n_hot) break;
+    above += hist[t];
+  }
+  *thr = t;
+  *quota = (uint32_t)(*n_hot - above);
+}
+}  // namespace gg
+
+extern "C" gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_t* batch_offsets, int32_t B,
+                                 uint64_t first_batch_index, const int32_t* fanouts, int32_t num_layers,
+                                 const int32_t* Ws, int32_t nW, const gg_energy_model* model,
+                                 gg_sim_result* out, int32_t* best, int64_t* delta_out, int64_t* miss_out) {
+  if (!g || !seeds || !batch_offsets || !fanouts || !Ws || !model || !out)
+    return fail(GG_ERR_INVALID_ARG, "null argument");
+  if (B < 1 || nW < 1) return fail(GG_ERR_INVALID_ARG, "B and nW must be >= 1");
+  if (num_layers < 1 || num_layers > g->cfg.max_layers)
+    return fail(GG_ERR_INVALID_ARG, "num_layers = %d outside [1, max_layers = %d]", num_layers, g->cfg.max_layers);
+  for (int h = 0; h < num_layers; ++h)
+    if (fanouts[h] < 1 || fanouts[h] > GG_MAX_FANOUT)
+      return fail(GG_ERR_INVALID_ARG, "fanouts[%d] = %d outside [1, %d]", h, fanouts[h], GG_MAX_FANOUT);
+  for (int i = 0; i < nW; ++i)
+    if (Ws[i] < 1 || Ws[i] > g->cfg.max_window)
+      return fail(GG_ERR_INVALID_ARG, "Ws[%d] = %d outside [1, max_window = %d]", i, Ws[i], g->cfg.max_window);
+  if (batch_offsets[0] != 0) return fail(GG_ERR_INVALID_ARG, "batch_offsets[0] must be 0");
+  for (int b = 0; b < B; ++b) {
+    const int64_t n = batch_offsets[b + 1] - batch_offsets[b];
+    if (n < 1 || n > g->cfg.max_batch)
+      return fail(GG_ERR_INVALID_ARG, "batch %d has %lld seeds; must be in [1, max_batch = %d]", b, (long long)n, g->cfg.max_batch);
+  }
+  for (int64_t i = 0; i < batch_offsets[B]; ++i)
+    if (seeds[i] < 0 || seeds[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "seed %lld = %d outside [0, N)", (long long)i, seeds[i]);
+  if (g->win[0].live || g->win[1].live || g->win[2].live)
+    return fail(GG_ERR_STATE, "release every window before gg_simulate");
+  {
+    std::unique_lock<std::mutex> l(g->mu);
+    g->cv_done.wait(l, [&] { return g->busy == 0; });
+  }
+  CU(cudaSetDevice(g->device));
+  CU(cudaDeviceSynchronize());
+  const int Wc = g->cfg.max_window, L = num_layers, P = g->R.P;
+  gg_status rc = ensure_shared(g, Wc, L, fanouts, nullptr);
+  if (rc != GG_OK) return rc;
+
+  // ---- the trace: every batch sampled once, N_b lists kept in HBM -------------------------
+  Window* w = &g->win[0];
+  DevBuf<int32_t> db;
+  std::vector<int64_t> off((size_t)B + 1, 0);
+  for (int c0 = 0; c0 < B; c0 += Wc) {
+    const int wc = std::min(Wc, B - c0);
+    w->id = -1; w->W = wc; w->L = L; w->first_batch = first_batch_index + (uint64_t)c0;
+    for (int h = 0; h < L; ++h) w->fanouts[h] = fanouts[h];
+    w->seeds.assign(seeds + batch_offsets[c0], seeds + batch_offsets[c0 + wc]);
+    w->boff.resize((size_t)wc + 1);
+    for (int b = 0; b <= wc; ++b) w->boff[b] = batch_offsets[c0 + b] - batch_offsets[c0];
+    rc = stage_a(g, w);
+    if (rc != GG_OK) { db.release(); return rc; }
+    for (int b = 0; b < wc; ++b) off[c0 + b + 1] = off[c0 + b] + w->n_front[L][b];
+    const int64_t need = off[c0 + wc];
+    if (need > db.n) {
+      // grow: estimate the whole epoch from what has been seen, copy what is already there
+      const int64_t est = (int64_t)((double)need / (c0 + wc) * B * 1.1) + 4096;
+      int32_t* np_ = nullptr;
+      if (cudaMalloc((void**)&np_, (size_t)std::max(est, need) * sizeof(int32_t)) != cudaSuccess) {
+        cudaGetLastError();
+        db.release();
+        return fail(GG_ERR_OOM, "device allocation of the trace (%lld ids) failed", (long long)std::max(est, need));
+      }
+      if (db.p && off[c0] > 0) cudaMemcpyAsync(np_, db.p, (size_t)off[c0] * sizeof(int32_t), cudaMemcpyDeviceToDevice, g->side);
+      cudaStreamSynchronize(g->side);
+      db.release();
+      db.p = np_;
+      db.n = std::max(est, need);
+    }
+    for (int b = 0; b < wc; ++b)
+      CU(cudaMemcpyAsync(db.p + off[c0 + b], w->nodes.p + (int64_t)b * w->node_pitch,
+                         (size_t)w->n_front[L][b] * sizeof(int32_t), cudaMemcpyDeviceToDevice, g->side));
+    CU(cudaStreamSynchronize(g->side));
+  }
+  int64_t max_n = 0;
+  for (int b = 0; b < B; ++b) max_n = std::max(max_n, off[b + 1] - off[b]);
+
+  // ---- replay per candidate W ---------------------------------------------------------------
+  cudaStream_t st = g->side_b;
+  int Kmax = 0;
+  for (int i = 0; i < nW; ++i) Kmax = std::max(Kmax, (B + Ws[i] - 1) / Ws[i]);
+  DevBuf<int64_t> off_dev;
+  DevBuf<int32_t> delta_dev, counters_dev;
+  DevBuf<gg_sim_result> res_dev;
+  auto cleanup = [&]() { db.release(); off_dev.release(); delta_dev.release(); counters_dev.release(); res_dev.release(); };
+  const int64_t n_cnt = (int64_t)B * (2 + GG_MAX_PARTS), n_del = (int64_t)Kmax * GG_MAX_PARTS;
+  if (off_dev.ensure(B + 1) != cudaSuccess || delta_dev.ensure(n_del) != cudaSuccess ||
+      counters_dev.ensure(n_cnt) != cudaSuccess || res_dev.ensure(nW) != cudaSuccess) {
+    cudaGetLastError();
+    cleanup();
+    return fail(GG_ERR_OOM, "device allocation of the simulator's tallies failed");
+  }
+#define CUS(call)                                                                         \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      cleanup();                                                                          \
+      return fail(GG_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+    }                                                                                     \
+  } while (0)
+  CUS(cudaMemcpyAsync(off_dev.p, off.data(), (size_t)(B + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+  std::vector<int32_t> h_cnt((size_t)n_cnt), h_del((size_t)n_del);
+  int64_t delta_cursor = 0;
+  for (int i = 0; i < nW; ++i) {
+    const int W = Ws[i], K = (B + W - 1) / W;
+    for (int s = 0; s < 2; ++s) {
+      CacheSlot& c = g->cslot[s];
+      launch_slots_clear(st, c.hot.p, (int)c.n_cached, c.slot_map);
+      c.n_cached = 0;
+      c.tenant = nullptr;
+    }
+    CUS(cudaMemsetAsync(counters_dev.p, 0, (size_t)n_cnt * sizeof(int32_t), st));
+    CUS(cudaMemsetAsync(delta_dev.p, 0, (size_t)n_del * sizeof(int32_t), st));
+    CacheSlot* prev = nullptr;
+    for (int k = 0; k < K; ++k) {
+      const int b0 = k * W, b1 = std::min(B, b0 + W);
+      // a-3 over the window's slice of the trace
+      launch_count_db(st, db.p, off[b0], off[b1], g->cnt8.p);
+      launch_unique_count(st, g->cnt8.p, g->cnt_words, g->R, g->tiles32.p, g->stats.p, g->hist.p, w->uniq.p, w->cnt.p);
+      CUS(cudaMemcpyAsync(g->h_small, g->stats.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      CUS(cudaMemcpyAsync(g->h_small + 1, g->hist.p, 256 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      CUS(cudaStreamSynchronize(st));
+      const int64_t n_unique = g->h_small[0];
+      int64_t n_remote = 0, n_hot = 0;
+      for (int c = 1; c < 256; ++c) n_remote += g->h_small[1 + c];
+      int32_t thr;
+      uint32_t quota;
+      hot_threshold(g->h_small + 1, n_remote, g->n_hot_eff, &n_hot, &thr, &quota);
+      // a-4 / a-5 against the previous cache state
+      CacheSlot* cs = &g->cslot[k & 1];
+      launch_slots_clear(st, cs->hot.p, (int)cs->n_cached, cs->slot_map);
+      cs->n_cached = 0;
+      if (n_hot > 0) {
+        launch_hot_select(st, w->uniq.p, w->cnt.p, (int)n_unique, g->R, thr, quota, g->tiles64.p, g->total64.p, cs->hot.p);
+        const int carry = (g->cfg.carry_over && prev) ? 1 : 0;
+        launch_delta_split(st, cs->hot.p, (int)n_hot, g->R, prev ? prev->slot_map : nullptr, carry, g->tiles32_b.p,
+                           g->n_delta_dev.p, g->owner_cnt.p, cs->slot_map, w->req_ids.p, w->carry_src.p, w->carry_ids.p);
+        cs->n_cached = n_hot;
+        CUS(cudaMemcpyAsync(delta_dev.p + (int64_t)k * GG_MAX_PARTS, g->owner_cnt.p + GG_MAX_PARTS,
+                            GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+      }
+      // Alg. 1 l.11-12 as counts
+      launch_classify(st, db.p, off_dev.p, b0, b1 - b0, max_n, cs->slot_map, g->R, counters_dev.p);
+      prev = cs;
+    }
+    launch_sim_events(st, delta_dev.p, counters_dev.p, K, B, W, *model, P, g->rb, res_dev.p + i);
+    if (delta_out) {
+      CUS(cudaMemcpyAsync(h_del.data(), delta_dev.p, (size_t)K * GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      CUS(cudaStreamSynchronize(st));
+      for (int k = 0; k < K; ++k)
+        for (int m = 0; m < P; ++m) delta_out[delta_cursor + (int64_t)k * P + m] = h_del[(size_t)k * GG_MAX_PARTS + m];
+    }
+    delta_cursor += (int64_t)K * P;
+    if (miss_out) {
+      CUS(cudaMemcpyAsync(h_cnt.data(), counters_dev.p, (size_t)n_cnt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      CUS(cudaStreamSynchronize(st));
+      for (int b = 0; b < B; ++b)
+        for (int m = 0; m < P; ++m)
+          miss_out[((int64_t)i * B + b) * P + m] = h_cnt[(size_t)b * (2 + GG_MAX_PARTS) + 2 + m];
+    }
+  }
+  CUS(cudaMemcpyAsync(out, res_dev.p, (size_t)nW * sizeof(gg_sim_result), cudaMemcpyDeviceToHost, st));
+  for (int s = 0; s < 2; ++s) {
+    CacheSlot& c = g->cslot[s];
+    launch_slots_clear(st, c.hot.p, (int)c.n_cached, c.slot_map);
+    c.n_cached = 0;
+    c.tenant = nullptr;
+  }
+  g->prev_cs = nullptr;
+  CUS(cudaStreamSynchronize(st));
+  CUS(cudaGetLastError());
+#undef CUS
+  cleanup();
+  int bi = 0;
+  for (int i = 1; i < nW; ++i)
+    if (out[i].e_phy < out[bi].e_phy) bi = i;
+  if (best) *best = bi;
+  return GG_OK;
+}

@@ -105,4 +105,11 @@ void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const St
                             const OwnerRanges& R, uint8_t* dst_base, int64_t dst_row0,
                             int64_t dst_stride, int rb);
 
+// NEXT-1 trace simulator (simulate.cu)
+void launch_count_db(cudaStream_t st, const int32_t* db_nodes, int64_t begin, int64_t end, uint32_t* cnt8);
+void launch_classify(cudaStream_t st, const int32_t* db_nodes, const int64_t* db_off, int b0, int nb,
+                     int64_t max_n, const int32_t* slot_of, const OwnerRanges& R, int32_t* counters);
+void launch_sim_events(cudaStream_t st, const int32_t* delta, const int32_t* counters, int K, int B, int W,
+                       const gg_energy_model& E, int P, int64_t row_bytes, gg_sim_result* out_dev);
+
 }  // namespace gg

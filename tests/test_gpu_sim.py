@@ -1,0 +1,105 @@
+"""GPU parity of gg_simulate (NEXT-1: trace simulator + Eqs. 1-3) against oracle/sim.py.
+Integers bit-exact; the energies are IEEE doubles formed by the same operations in the same order
+on both sides (no FMA contraction on the device), so they are compared for equality too."""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+from oracle import ggo, sim  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return "cuda:0"
+
+
+def make_model(P, rb, seed=5, bw=5.0e10):
+    rng = np.random.default_rng(seed)
+    f = lambda lo, hi: rng.uniform(lo, hi, P).tolist()
+    d = dict(eps_init=f(1e-3, 5e-3), eps_pay_a=f(0, 1e-4), eps_pay_b=f(1e-7, 5e-7),
+             lam_init=f(1e-5, 5e-5), lam_pay_a=f(0, 1e-6), lam_pay_b=f(1e-9, 9e-9), bw=bw, p_idle=140.0)
+    om = sim.EnergyModel(row_bytes=rb, **d)
+    return d, om
+
+
+INT_KEYS = ("n_windows", "rebuild_events", "miss_events", "rebuild_rows", "miss_rows", "n_access",
+            "n_remote_access", "hit_local", "hit_cache")
+F64_KEYS = ("e_rebuild", "e_miss", "t_stall", "e_stall", "e_phy", "hit_ratio")
+
+
+def check(w, dev, candidates, n_hot, carry, batches=None, bw=5.0e10):
+    from paper_2606_02916_b200 import epoch as ep
+    batches = w.batches if batches is None else batches
+    og = ggo.Graph(*w.host_graph())
+    trace = [ggo.Batch(og, b, w.fanouts, w.seed, i).nodes for i, b in enumerate(batches)]
+    d, om = make_model(len(w.part_offsets) - 1, w.row_bytes, bw=bw)
+    g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=carry, max_window=max(candidates))
+    got = g.simulate(batches, w.fanouts, candidates, d, export=True)
+    want_best, want = sim.select_window(trace, w.part_offsets, w.local_part, n_hot, candidates, om, carry_over=carry)
+    for i, (gr, wr) in enumerate(zip(got["results"], want)):
+        assert gr["W"] == candidates[i]
+        for k in INT_KEYS:
+            assert gr[k] == int(np.sum(wr[k])), (candidates[i], k, gr[k], wr[k])   # per-batch arrays are summed
+        assert np.array_equal(got["delta"][i], wr["delta"]), "per-owner |Delta| (W=%d)" % candidates[i]
+        assert np.array_equal(got["miss"][i], wr["miss"]), "per-owner |M| (W=%d)" % candidates[i]
+        for k in F64_KEYS:
+            assert gr[k] == wr[k], (candidates[i], k, gr[k], wr[k])       # same bits
+    assert got["best"] == want_best
+    # the simulator leaves the graph usable and the cache empty: a normal epoch still matches
+    from tests import parity_util as pu
+    g.close()
+    return got
+
+
+def test_tiny_all_budgets(workload, dev):
+    w = workload("tiny", dev)
+    check(w, dev, [1, 2, 3, 4], -1, 1)
+    check(w, dev, [1, 2, 4], 200, 1)
+    check(w, dev, [1, 2, 4], 200, 0)
+    check(w, dev, [4, 1], 0, 1)
+
+
+def test_small_full_epoch_candidates(workload, dev):
+    w = workload("small", dev)
+    r = check(w, dev, [1, 2, 4, 8], 7500, 1)
+    assert r["results"][0]["rebuild_events"] >= r["results"][3]["rebuild_events"]
+    check(w, dev, [1, 4, 8], -1, 1, bw=1.0e6)          # a slow link: the bandwidth ceiling sets every event time
+
+
+def test_products_mini_and_large_mini(workload, dev):
+    check(workload("products_mini", dev), dev, [1, 4, 16], 4500, 1)
+    check(workload("large_mini", dev), dev, [2, 8], 11250, 1)
+
+
+def test_simulate_then_run_epoch(workload, dev):
+    """gg_simulate leaves the cache state empty and the pipeline usable."""
+    from paper_2606_02916_b200 import epoch as ep
+    from tests import parity_util as pu
+    w = workload("tiny", dev)
+    g = ep.graph_from_workload(w, n_hot=200, max_window=4)
+    d, _ = make_model(4, w.row_bytes)
+    a = g.simulate(w.batches, w.fanouts, [1, 4], d)
+    b = g.simulate(w.batches, w.fanouts, [1, 4], d)
+    assert a == b
+    g.close()
+    pu.check_epoch(w, W=4, n_hot=200)
+
+
+def test_simulate_errors(workload, dev):
+    from paper_2606_02916_b200 import binding, epoch as ep
+    w = workload("tiny", dev)
+    g = ep.graph_from_workload(w, max_window=4)
+    d, _ = make_model(4, w.row_bytes)
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.simulate(w.batches, w.fanouts, [8], d)                      # candidate above max_window
+    assert e.value.status == binding.GG_ERR_INVALID_ARG
+    g.window_stage(0, 0, w.batches[:2], w.fanouts)
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.simulate(w.batches, w.fanouts, [2], d)                      # a window is live
+    assert e.value.status == binding.GG_ERR_STATE
+    g.window_release(0)
+    g.close()
