@@ -37,6 +37,10 @@ def parse_args():
     ap.add_argument("--window", type=int, default=16)
     ap.add_argument("--n-hot", type=int, default=-1)
     ap.add_argument("--staging-mode", type=int, default=0)
+    ap.add_argument("--lookahead", type=int, default=6,
+                    help="windows staged ahead of the one being served (sampling runs that far ahead; "
+                         "the cache is always built one window ahead)")
+    ap.add_argument("--host-threads", type=int, default=0)
     ap.add_argument("--no-sweep", action="store_true", help="skip the W sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -255,7 +259,9 @@ def run_ours(args):
     W = args.window
     sweep_ws = [] if args.no_sweep or world > 1 else [x for x in w.cfg["windows"] if x != W]
     g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
-                               staging_mode=args.staging_mode)
+                               staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
+                               host_threads=args.host_threads)
+    LA = args.lookahead
     # gathers run on a high-priority stream so their CTAs are scheduled ahead of the library's
     # (long-running, ALU-bound) sampling kernels whenever an SM has room for both
     stream = torch.cuda.Stream(dev, priority=-1)
@@ -272,15 +278,15 @@ def run_ours(args):
 
     def one_epoch(Wx, sink=None, wid0=0):
         if sink is None:
-            ep.run_epoch(g, batches, w.fanouts, Wx, feats, stream=stream, first_window_id=wid0)
+            ep.run_epoch(g, batches, w.fanouts, Wx, feats, stream=stream, first_window_id=wid0, lookahead=LA)
         else:
             wins = ep.windows_of(n_b, Wx)
-            for k in range(min(2, len(wins))):
+            for k in range(min(LA, len(wins))):
                 g.window_stage(wid0 + k, wins[k].start, [batches[i] for i in wins[k]], w.fanouts)
             for k, win in enumerate(wins):
-                if k + 2 < len(wins):
-                    nxt = wins[k + 2]
-                    g.window_stage(wid0 + k + 2, nxt.start, [batches[i] for i in nxt], w.fanouts)
+                if k + LA < len(wins):
+                    nxt = wins[k + LA]
+                    g.window_stage(wid0 + k + LA, nxt.start, [batches[i] for i in nxt], w.fanouts)
                 for j, _bi in enumerate(win):
                     sink.consume(g.batch_gather(wid0 + k, j, sink.buffer(), stream))
                 g.window_release(wid0 + k)
@@ -337,7 +343,8 @@ def run_ours(args):
         tr_acc["h2d_ms"] += t["ms_h2d"]
         tr_acc["n_access"] += t["n_access"]
 
-    ep.run_epoch(g, batches, w.fanouts, W, feats, on_window=on_window, stream=stream, first_window_id=5 * 10 ** 6)
+    ep.run_epoch(g, batches, w.fanouts, W, feats, on_window=on_window, stream=stream, first_window_id=5 * 10 ** 6,
+                 lookahead=LA)
     torch.cuda.synchronize(dev)
     g.cache_reset()
 
@@ -413,6 +420,16 @@ def run_ours(args):
                     "PAPER.md:345 Kendall tau 0.62-1.00 on its cluster",
         }
 
+    # ---- variant (NEXT-2): GPU-initiated pull staging instead of host pack + cudaMemcpyAsync ----
+    variants = {}
+    if not args.no_sweep and world == 1 and args.staging_mode == 0:
+        g.close()
+        g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws), staging_mode=1,
+                                   max_live_windows=args.lookahead + 1)
+        r = timed(W, 3, 2)
+        variants["staging_mode_1_gpu_pull"] = {"value": 3 * n_b / r["sec"], "unit": UNIT,
+                                               "note": "k_rows<.,1> reads the owners' pinned rows over PCIe (12 CTAs), no host pack, no ID read-back"}
+
     if rank != 0:
         return
     # ---- rooflines: the dominant kernel group (a-1 sampling, ALU-bound) and the gather (HBM) ----
@@ -469,14 +486,14 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "u8 rows / int32 ids / uint64 keys",
         "data": "synthetic",
         "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot,
-                   "staging_mode": args.staging_mode, "carry_over": 1,
+                   "staging_mode": args.staging_mode, "carry_over": 1, "lookahead_windows": LA,
                    "step": "one epoch = %d mini-batches in %d windows, cache reset per epoch" % (n_b, -(-n_b // W)),
                    "l2": "inputs larger than L2 (feature store %.0f MB, X_b %.0f MB per batch)"
                          % (w.num_nodes * w.row_bytes / 1e6, tr_acc["n_access"] / n_b * w.row_bytes / 1e6)},
         "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
         "roofline": roof, "roofline_gather": roof_gather, "kernels_alone": serial, "stages": stages, "vs_W": vs_w,
-        "J_per_epoch_vs_W": j_w, "simulator": simulator,
+        "J_per_epoch_vs_W": j_w, "simulator": simulator, "variants": variants,
         "gpu_stall_ms_per_step": (main["prof"]["wait"]["ms"] / args.steps) if "wait" in main["prof"] else None,
         "energy": {"J_per_step": (main["joules"] / args.steps) if main["joules"] is not None else None,
                    "avg_W": (main["joules"] / main["wall"]) if main["joules"] is not None else None,

@@ -40,11 +40,14 @@
  *    hop whose n_src = n_input.  fanouts[h] belongs to hop h counted outward (reading S2).
  *  - Every function returns a gg_status; none aborts or throws; on error no output is
  *    partially valid.  gg_last_error() gives the text for the calling thread's last failure.
- *  - One caller thread per gg_graph.  At most THREE windows are live: k being served, k+1
- *    whose cache is being staged, k+2 being sampled (the two prefetch phases run on two library
- *    threads and two side streams).  There are two cache buffers: window k+2's cache is built
- *    only after window k is released, so asking for k+2's batches while k is live is
- *    GG_ERR_STATE.  Staging one window ahead (the literal loop of Alg. 1) is equally valid.
+ *  - One caller thread per gg_graph.  At most gg_config.max_live_windows (default 3) windows are
+ *    live: k being served, k+1 whose cache is being staged, k+2 .. being sampled ahead (the two
+ *    prefetch phases run on two library threads and their side streams; sampling does not depend
+ *    on the cache, so it may run as far ahead as there are arenas -- on a short epoch that fills
+ *    the GPU while the cold first window crosses the host link).  There are two cache buffers:
+ *    window k+2's cache is built only after window k is released, so asking for k+2's batches
+ *    while k is live is GG_ERR_STATE.  Staging one window ahead (the literal loop of Alg. 1) is
+ *    equally valid.
  */
 #ifndef GREENGNN_H_
 #define GREENGNN_H_
@@ -58,6 +61,7 @@ extern "C" {
 #define GG_MAX_LAYERS 8
 #define GG_MAX_PARTS 16
 #define GG_MAX_FANOUT 96   /* selection candidate buffer is 256 entries; see DESIGN.md a-1 */
+#define GG_MAX_LIVE_WINDOWS 16
 #define GG_MAX_WINDOW 255  /* access counts are 8-bit lanes of a packed counter; W in {1..64} in PAPER.md:130 */
 
 typedef struct gg_graph gg_graph; /* opaque */
@@ -108,6 +112,10 @@ typedef struct {
                              owner (BASELINE.json:north_star (d));
                              1 = one GPU-initiated pull kernel per owner reading the pinned store */
   int32_t host_threads;   /* owner-service pack threads; <= 0 = min(16, hardware threads) */
+  int32_t max_live_windows; /* window arenas = how far gg_window_stage may run ahead of the window
+                               being served: k served, k+1 staged, k+2 .. k+n-1 sampled ahead (their
+                               cache is still built one window ahead, Alg. 1 l.8); <= 0 = 3,
+                               clamped to [3, GG_MAX_LIVE_WINDOWS] */
 } gg_config;
 
 /* Builds the handle.  Borrows indptr / indices / part_base pointers (caller keeps them alive
@@ -127,7 +135,7 @@ gg_status gg_graph_destroy(gg_graph* g);
  *                  keyed with first_batch_index+i (reading S7: epoch is not hashed)
  *   fanouts        host int32 [num_layers], hop order outward from the seeds, 1..GG_MAX_FANOUT
  * Errors: INVALID_ARG (nulls, W<1 or >max_window, L<1 or >max_layers, a batch larger than
- * max_batch or empty window, seed outside [0,N)), STATE (three windows already live, or
+ * max_batch or empty window, seed outside [0,N)), STATE (max_live_windows already live, or
  * window_id already live), CAPACITY (caps derived from fanouts exceed int32 indexing). */
 gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_index,
                           const int32_t* seeds, const int64_t* batch_offsets, int32_t W,

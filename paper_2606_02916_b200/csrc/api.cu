@@ -163,7 +163,7 @@ struct CacheSlot {
   bool gather_recorded = false;
 };
 
-// One of the three window arenas (k being served, k+1 being staged, k+2 being sampled).
+// One of the n_win window arenas (k being served, k+1 being staged, k+2 .. k+n_win-1 sampled ahead).
 struct Window {
   // identity / arguments
   int64_t id = -1;
@@ -304,7 +304,8 @@ struct gg_graph {
   cudaStream_t side = nullptr;    // phase A: sample, frontier, unique
   cudaStream_t side_b = nullptr;  // phase B: select, delta (the stager thread syncs on it)
   cudaStream_t side_c = nullptr;  // phase B: bulk copies, carry-over copy, cache-ready event (never waited on by the stager)
-  Window win[3];
+  Window win[GG_MAX_LIVE_WINDOWS];
+  int n_win = 3;
   CacheSlot cslot[2];
   uint64_t stage_counter = 0;
   CacheSlot* prev_cs = nullptr;   // holds C_{k-1} for the next phase B (stager thread)
@@ -816,7 +817,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
   cudaDeviceSynchronize();
   delete g->pool;
   g->prof.destroy();
-  for (int s = 0; s < 3; ++s) {
+  for (int s = 0; s < g->n_win; ++s) {
     Window& w = g->win[s];
     w.nodes.release(); w.n_front_dev.release(); w.uniq.release(); w.cnt.release();
     w.req_ids.release(); w.carry_src.release(); w.carry_ids.release(); w.counters.release();
@@ -909,6 +910,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   for (int m = 0; m < GG_MAX_PARTS; ++m) g->store.base[m] = m < P ? (const uint8_t*)store->part_base[m] : nullptr;
   g->store.stride = store->row_stride_bytes;
   g->dim = store->dim; g->rb = (int)rb; g->dtype = store->dtype; g->cfg = *cfg;
+  g->n_win = cfg->max_live_windows <= 0 ? 3 : std::min(std::max(cfg->max_live_windows, 3), GG_MAX_LIVE_WINDOWS);
   cudaGetDevice(&g->device);
   const int64_t n_remote_nodes = g->N - (g->R.lo[g->R.local + 1] - g->R.lo[g->R.local]);
   g->cache_rows = cfg->max_cache_rows > 0 ? std::min<int64_t>(cfg->max_cache_rows, n_remote_nodes) : n_remote_nodes;
@@ -953,7 +955,13 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   CUC(cudaHostAlloc((void**)&g->h_seeds, (size_t)Wmax * cfg->max_batch * sizeof(int32_t), cudaHostAllocDefault));
   CUC(cudaHostAlloc((void**)&g->h_kp, (size_t)GG_MAX_LAYERS * Wmax * sizeof(uint64_t), cudaHostAllocDefault));
   CUC(cudaStreamCreateWithFlags(&g->side, cudaStreamNonBlocking));
-  CUC(cudaStreamCreateWithFlags(&g->side_b, cudaStreamNonBlocking));
+  {
+    // the stager's kernels are tiny but sit on the critical path to the host link (the thread
+    // waits for |Delta_m| before it can pack): run them ahead of the sampler's long kernels
+    int lo_pri = 0, hi_pri = 0;
+    CUC(cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri));
+    CUC(cudaStreamCreateWithPriority(&g->side_b, cudaStreamNonBlocking, hi_pri));
+  }
   CUC(cudaStreamCreateWithFlags(&g->side_c, cudaStreamNonBlocking));
   for (int i = 0; i < 2; ++i) CUC(cudaEventCreateWithFlags(&g->resp_free[i], cudaEventDisableTiming));
   for (int s = 0; s < 2; ++s) {
@@ -964,7 +972,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
     CUC(c.hot.ensure(std::max<int64_t>(g->cache_rows, 1)));
     launch_fill_i32(0, c.slot_map, g->N, -1);
   }
-  for (int s = 0; s < 3; ++s) {
+  for (int s = 0; s < g->n_win; ++s) {
     Window& w = g->win[s];
     CUC(cudaEventCreateWithFlags(&w.sampled, cudaEventDisableTiming));
     CUC(cudaEventCreateWithFlags(&w.ready, cudaEventDefault));
@@ -985,7 +993,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
 
 namespace gg {
 static Window* find_window(gg_graph* g, int64_t id) {
-  for (int s = 0; s < 3; ++s)
+  for (int s = 0; s < g->n_win; ++s)
     if (g->win[s].live && g->win[s].id == id) return &g->win[s];
   return nullptr;
 }
@@ -996,7 +1004,7 @@ static gg_status wait_enqueued(gg_graph* g, Window* w) {
   if (!w->enqueued) {
     // window k+2's cache buffer is window k's: it cannot be built before k is released
     Window* t = w->cs ? w->cs->tenant : nullptr;
-    for (int s = 0; s < 3; ++s) {
+    for (int s = 0; s < g->n_win; ++s) {
       Window* o = &g->win[s];
       if (o != w && o->live && o->seq + 2 == w->seq)
         return fail(GG_ERR_STATE, "window %lld shares its cache buffer with live window %lld: release that one first",
@@ -1053,8 +1061,8 @@ gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_i
   for (int64_t i = 0; i < S; ++i)
     if (seeds[i] < 0 || seeds[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "seed %lld = %d outside [0, N)", (long long)i, seeds[i]);
   if (find_window(g, window_id)) return fail(GG_ERR_STATE, "window %lld is already live", (long long)window_id);
-  Window* w = &g->win[g->stage_counter % 3];
-  if (w->live) return fail(GG_ERR_STATE, "three windows are live; release window %lld first", (long long)w->id);
+  Window* w = &g->win[g->stage_counter % g->n_win];
+  if (w->live) return fail(GG_ERR_STATE, "%d windows are live; release window %lld first", g->n_win, (long long)w->id);
   // shared scratch sized by (W, fanouts): grow only with both pipeline threads idle
   bool need_drain = false;
   gg_status rc = ensure_shared(g, W, num_layers, fanouts, &need_drain);
@@ -1152,7 +1160,7 @@ gg_status gg_window_release(gg_graph* g, int64_t window_id) {
     std::unique_lock<std::mutex> l(g->mu);
     bool blocked = false;
     if (!w->enqueued)
-      for (int s = 0; s < 3; ++s)
+      for (int s = 0; s < g->n_win; ++s)
         if (&g->win[s] != w && g->win[s].live && g->win[s].seq + 2 == w->seq) blocked = true;
     if (blocked) return fail(GG_ERR_STATE, "release the older live window first");
     g->cv_done.wait(l, [&] { return w->enqueued; });
@@ -1278,8 +1286,8 @@ gg_status gg_debug_sampler(int32_t rank_shift, float want_add) {
 
 gg_status gg_cache_reset(gg_graph* g) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
-  if (g->win[0].live || g->win[1].live || g->win[2].live)
-    return fail(GG_ERR_STATE, "release every window before gg_cache_reset");
+  for (int s = 0; s < g->n_win; ++s)
+    if (g->win[s].live) return fail(GG_ERR_STATE, "release every window before gg_cache_reset");
   {
     std::unique_lock<std::mutex> l(g->mu);
     g->cv_done.wait(l, [&] { return g->busy == 0; });
@@ -1344,8 +1352,8 @@ extern "C" gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_
   }
   for (int64_t i = 0; i < batch_offsets[B]; ++i)
     if (seeds[i] < 0 || seeds[i] >= g->N) return fail(GG_ERR_INVALID_ARG, "seed %lld = %d outside [0, N)", (long long)i, seeds[i]);
-  if (g->win[0].live || g->win[1].live || g->win[2].live)
-    return fail(GG_ERR_STATE, "release every window before gg_simulate");
+  for (int s = 0; s < g->n_win; ++s)
+    if (g->win[s].live) return fail(GG_ERR_STATE, "release every window before gg_simulate");
   {
     std::unique_lock<std::mutex> l(g->mu);
     g->cv_done.wait(l, [&] { return g->busy == 0; });

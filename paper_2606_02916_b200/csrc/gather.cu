@@ -37,16 +37,16 @@ __device__ __forceinline__ void st_stream(uint8_t* p, typename VecT<VEC>::type v
 
 // Copies the tile's rows.  s_src[r] == nullptr means "skip row r".  If DENSE_DST the tile's
 // destination is one contiguous run starting at dst0.
-template <int VEC, bool DENSE_DST>
+template <int VEC, bool DENSE_DST, int UNROLL = kUnroll>
 __device__ __forceinline__ void copy_tile(const uint8_t* const* s_src, uint8_t* const* s_dst,
                                           uint8_t* dst0, int rows, int cpr /*chunks per row*/) {
   const int total = rows * cpr;
-  for (int c0 = threadIdx.x; c0 < total; c0 += kThreads * kUnroll) {
-    typename VecT<VEC>::type v[kUnroll];
-    int row[kUnroll], col[kUnroll];
-    bool ok[kUnroll];
+  for (int c0 = threadIdx.x; c0 < total; c0 += kThreads * UNROLL) {
+    typename VecT<VEC>::type v[UNROLL];
+    int row[UNROLL], col[UNROLL];
+    bool ok[UNROLL];
 #pragma unroll
-    for (int k = 0; k < kUnroll; ++k) {
+    for (int k = 0; k < UNROLL; ++k) {
       const int c = c0 + k * kThreads;
       row[k] = c / cpr;
       col[k] = c - row[k] * cpr;
@@ -54,7 +54,7 @@ __device__ __forceinline__ void copy_tile(const uint8_t* const* s_src, uint8_t* 
       if (ok[k]) v[k] = ld_stream<VEC>(s_src[row[k]] + (int64_t)col[k] * VEC);
     }
 #pragma unroll
-    for (int k = 0; k < kUnroll; ++k) {
+    for (int k = 0; k < UNROLL; ++k) {
       if (ok[k]) {
         uint8_t* d = DENSE_DST ? dst0 + (int64_t)(c0 + k * kThreads) * VEC
                                : s_dst[row[k]] + (int64_t)col[k] * VEC;
@@ -210,7 +210,9 @@ __global__ void __launch_bounds__(kThreads) k_rows(RowsArgs A) {
       s_dst[r] = dst;
     }
     __syncthreads();
-    copy_tile<VEC, false>(s_src, s_dst, nullptr, rows, A.rb / VEC);
+    // rows that come over the host link (MODE 1) keep twice as many loads in flight per thread:
+    // a few CTAs then saturate PCIe and the rest of the GPU stays with the sampler
+    copy_tile<VEC, false, MODE == 1 ? 2 * kUnroll : kUnroll>(s_src, s_dst, nullptr, rows, A.rb / VEC);
   }
 }
 
@@ -296,7 +298,12 @@ void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const St
     ok8 = ok8 && (uintptr_t)store.base[m] % 8 == 0;
   }
   int grid = (n + kRows - 1) / kRows;
-  if (grid > 148 * 8) grid = 148 * 8;
+  // Rows cross the host link here: 12 CTAs with 8 16-byte loads in flight per thread already
+  // saturate PCIe (41 GB/s); a wider grid only takes SMs and memory-system queue slots away from
+  // the sampler (measured, products W=16: 12 / 16 / 24 / 32 / 1184 CTAs -> 3903 / 3657 / 3340 /
+  // 3184 / 2607 mini-batches/s).
+  constexpr int kPullCtas = 12;
+  if (grid > kPullCtas) grid = kPullCtas;
   if (ok16) k_rows<16, 1><<<grid, kThreads, 0, st>>>(A);
   else if (ok8) k_rows<8, 1><<<grid, kThreads, 0, st>>>(A);
   else k_rows<4, 1><<<grid, kThreads, 0, st>>>(A);

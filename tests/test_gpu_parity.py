@@ -100,12 +100,13 @@ def test_selection_fallbacks_are_rare_by_default(workload, dev):
 
 
 def test_lookahead_one_is_algorithm_1_literal(workload, dev):
-    """stage(k+1) / serve k (Alg. 1) gives the same results as the deeper pipeline."""
+    """stage(k+1) / serve k (Alg. 1) gives the same results as the deeper pipelines
+    (sampling 2 and 5 windows ahead; the cache is always built one window ahead)."""
     from paper_2606_02916_b200 import epoch as ep
     w = workload("small", dev)
     outs = []
-    for la in (1, 2):
-        g = ep.graph_from_workload(w, n_hot=7500, max_window=4)
+    for la in (1, 2, 5):
+        g = ep.graph_from_workload(w, n_hot=7500, max_window=4, max_live_windows=la + 1)
         feats = torch.empty(w.num_nodes, w.dim, dtype=w.dtype, device=dev)
         got = []
         ep.run_epoch(g, w.batches, w.fanouts, 4, feats, lookahead=la,
@@ -113,8 +114,9 @@ def test_lookahead_one_is_algorithm_1_literal(workload, dev):
                                                               r["features"].cpu().clone(), g.misses(r)[0].copy())))
         outs.append(got)
         g.close()
-    for a, b in zip(*outs):
+    for a, b, c in zip(*outs):
         assert np.array_equal(a[0], b[0]) and torch.equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+        assert np.array_equal(a[0], c[0]) and torch.equal(a[1], c[1]) and np.array_equal(a[2], c[2])
 
 
 def test_determinism_two_epochs_identical(workload, dev):
