@@ -44,9 +44,9 @@
  *    live: k being served, k+1 whose cache is being staged, k+2 .. being sampled ahead (the two
  *    prefetch phases run on two library threads and their side streams; sampling does not depend
  *    on the cache, so it may run as far ahead as there are arenas -- on a short epoch that fills
- *    the GPU while the cold first window crosses the host link).  There are two cache buffers:
- *    window k+2's cache is built only after window k is released, so asking for k+2's batches
- *    while k is live is GG_ERR_STATE.  Staging one window ahead (the literal loop of Alg. 1) is
+ *    the GPU while the cold first window crosses the host link).  There are n = cache_buffers
+ *    cache buffers: window k+n's cache is built only after window k is released, so asking for
+ *    k+n's batches while k is live is GG_ERR_STATE.  Staging one window ahead (the literal loop of Alg. 1) is
  *    equally valid.
  */
 #ifndef GREENGNN_H_
@@ -62,6 +62,7 @@ extern "C" {
 #define GG_MAX_PARTS 16
 #define GG_MAX_FANOUT 96   /* selection candidate buffer is 256 entries; see DESIGN.md a-1 */
 #define GG_MAX_LIVE_WINDOWS 16
+#define GG_MAX_CACHE_BUFFERS 4
 #define GG_MAX_WINDOW 255  /* access counts are 8-bit lanes of a packed counter; W in {1..64} in PAPER.md:130 */
 
 typedef struct gg_graph gg_graph; /* opaque */
@@ -112,6 +113,11 @@ typedef struct {
                              owner (BASELINE.json:north_star (d));
                              1 = one GPU-initiated pull kernel per owner reading the pinned store */
   int32_t host_threads;   /* owner-service pack threads; <= 0 = min(16, hardware threads) */
+  int32_t cache_buffers;  /* HBM cache buffers (+ slot maps) in rotation, window k uses k mod n.  2 = the
+                             ping-pong a literal Alg. 1 needs; with 2, window k's hot set can only be
+                             selected after window k-2's gathers have finished, and that chain
+                             (gathers -> select -> pack -> copy) sets the pace; 3 takes it off the
+                             critical path (measured: ~2 % on the products epoch).  <= 0 = 2, clamped to [2, GG_MAX_CACHE_BUFFERS] */
   int32_t max_live_windows; /* window arenas = how far gg_window_stage may run ahead of the window
                                being served: k served, k+1 staged, k+2 .. k+n-1 sampled ahead (their
                                cache is still built one window ahead, Alg. 1 l.8); <= 0 = 3,

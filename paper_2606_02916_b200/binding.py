@@ -40,7 +40,7 @@ class gg_feature_store(C.Structure):
 class gg_config(C.Structure):
     _fields_ = [("seed", u64), ("n_hot", i64), ("carry_over", i32), ("max_layers", i32),
                 ("max_window", i32), ("max_batch", i32), ("max_cache_rows", i64),
-                ("max_input_nodes", i64), ("staging_mode", i32), ("host_threads", i32), ("max_live_windows", i32)]
+                ("max_input_nodes", i64), ("staging_mode", i32), ("host_threads", i32), ("cache_buffers", i32), ("max_live_windows", i32)]
 
 
 class gg_block(C.Structure):
@@ -182,7 +182,7 @@ class Graph:
                  local_part: int, feat_parts: List[torch.Tensor], seed: int, n_hot: int = -1,
                  carry_over: int = 1, max_layers: int = 3, max_window: int = 32, max_batch: int = 1024,
                  max_cache_rows: int = 0, max_input_nodes: int = 0, staging_mode: int = 0,
-                 host_threads: int = 0, max_live_windows: int = 0):
+                 host_threads: int = 0, max_live_windows: int = 0, cache_buffers: int = 0):
         self.lib = load_library()
         assert indptr.dtype == torch.int64 and indices.dtype == torch.int32
         self._keep = (indptr, indices, feat_parts)
@@ -201,7 +201,7 @@ class Graph:
         fs = gg_feature_store(self.dim, {torch.float32: 0, torch.bfloat16: 1}[self.feat_dtype],
                               strides.pop(), C.cast(bases, vp))
         cfg = gg_config(seed & ((1 << 64) - 1), n_hot, carry_over, max_layers, max_window, max_batch,
-                        max_cache_rows, max_input_nodes, staging_mode, host_threads, max_live_windows)
+                        max_cache_rows, max_input_nodes, staging_mode, host_threads, cache_buffers, max_live_windows)
         h = vp()
         ctx = torch.cuda.device(self.device) if self.device.type == "cuda" else contextlib.nullcontext()
         with ctx:

@@ -47,6 +47,11 @@ static gg_status fail(gg_status s, const char* fmt, ...) {
       return fail(GG_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
   } while (0)
 
+static bool g_timeline = getenv("GG_TIMELINE") != nullptr;
+static double now_ms();
+static void tl(const char* what, long long wid, double extra = 0) {
+  if (g_timeline) fprintf(stderr, "TL %.3f %s %lld %.3f\n", now_ms(), what, wid, extra);
+}
 static double now_ms() {
   using namespace std::chrono;
   return duration<double, std::milli>(steady_clock::now().time_since_epoch()).count();
@@ -195,6 +200,10 @@ struct Window {
   cudaEvent_t gather_done = nullptr;
   cudaEvent_t ev_copy[2 * GG_MAX_PARTS + 2] = {nullptr};  // start/stop per bulk copy, last pair = carry
   bool timing_pending = false;    // ms_h2d / ms_carry not yet read from the events
+  int32_t* h_req = nullptr;       // pinned: this window's request IDs (device -> host), mode 0
+  int64_t h_req_cap = 0;
+  CacheSlot* prev_cs = nullptr;   // C_{k-1}'s buffer: source of the carry-over copy
+  double t_b0 = 0;                // start of phase B on the host
   bool gather_recorded = false;
   bool enqueued = false;          // phase B finished on the host (or an error was recorded)
   gg_status status = GG_OK;
@@ -292,13 +301,12 @@ struct gg_graph {
   // pinned
   int32_t* h_small = nullptr;    // phase A readback scratch
   int32_t* h_small_b = nullptr;  // phase B readback scratch
-  int32_t* h_req = nullptr;      // request IDs (device -> host)
   uint8_t* h_resp[2] = {nullptr, nullptr};  // packed rows (host -> device), mode 0, ping-pong
   cudaEvent_t resp_free[2] = {nullptr, nullptr};  // bulk copies out of h_resp[i] have completed
   bool resp_used[2] = {false, false};
   int resp_idx = 0;
   int32_t* h_seeds = nullptr;
-  int64_t h_seeds_cap = 0, h_req_cap = 0, h_resp_cap[2] = {0, 0};
+  int64_t h_seeds_cap = 0, h_resp_cap[2] = {0, 0};
   uint64_t* h_kp = nullptr;
   // streams / threads
   cudaStream_t side = nullptr;    // phase A: sample, frontier, unique
@@ -306,13 +314,14 @@ struct gg_graph {
   cudaStream_t side_c = nullptr;  // phase B: bulk copies, carry-over copy, cache-ready event (never waited on by the stager)
   Window win[GG_MAX_LIVE_WINDOWS];
   int n_win = 3;
-  CacheSlot cslot[2];
+  CacheSlot cslot[GG_MAX_CACHE_BUFFERS];
+  int n_cs = 2;                   // cache buffers in rotation (window k uses buffer k mod n_cs)
   uint64_t stage_counter = 0;
   CacheSlot* prev_cs = nullptr;   // holds C_{k-1} for the next phase B (stager thread)
-  std::thread worker_a, worker_b;
+  std::thread worker_a, worker_b, worker_c;
   std::mutex mu;
-  std::condition_variable cv_a, cv_b, cv_done;
-  std::deque<Window*> jobs_a, jobs_b;
+  std::condition_variable cv_a, cv_b, cv_c, cv_done;
+  std::deque<Window*> jobs_a, jobs_b, jobs_c;
   int busy = 0;                   // jobs queued or in flight
   bool stop = false;
   Pool* pool = nullptr;
@@ -436,6 +445,7 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
   cudaStream_t st = g->side;
   const double t0 = now_ms();
+  tl("a_start", w->id);
   CU(cudaSetDevice(g->device));
   gg_status rc = alloc_window(g, w);
   if (rc != GG_OK) return rc;
@@ -453,8 +463,8 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   for (int h = 0; h < L; ++h)
     for (int b = 0; b < W; ++b)
       g->h_kp[h * Wmax + b] = key_prefix(g->cfg.seed, w->first_batch + (uint64_t)b, (uint64_t)h);
-  CU(cudaMemcpyAsync(g->seeds_dev.p, g->h_seeds, (size_t)S * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  CU(cudaMemcpyAsync(g->key_prefix.p, g->h_kp, (size_t)L * Wmax * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
+  launch_copy_words(st, g->seeds_dev.p, g->h_seeds, S);
+  launch_copy_words(st, g->key_prefix.p, g->h_kp, 2ll * L * Wmax);
   CU(cudaMemsetAsync(g->err_flag.p, 0, sizeof(int32_t), st));
 
   // a-1 / a-2, hop by hop over the whole window
@@ -494,9 +504,9 @@ static gg_status stage_a(gg_graph* g, Window* w) {
                         Wmax, g->tiles32.p, new_totals, g->err_flag.p, H.src_local.p);
     g->prof.end(st, pe, GG_PROF_FRONTIER, 0);
     // sizes of the next frontier and of this hop's blocks -> host
-    CU(cudaMemcpyAsync(g->h_small, w->n_front_dev.p + (h + 1) * Wmax, W * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(g->h_small + Wmax, H.edge_off_dev.p, (W + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(g->h_small + 2 * Wmax + 2, g->err_flag.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    launch_copy_words(st, g->h_small, w->n_front_dev.p + (h + 1) * Wmax, W);
+    launch_copy_words(st, g->h_small + Wmax, H.edge_off_dev.p, W + 1);
+    launch_copy_words(st, g->h_small + 2 * Wmax + 2, g->err_flag.p, 1);
     CU(cudaStreamSynchronize(st));
     if (g->h_small[2 * Wmax + 2])
       return fail(GG_ERR_CAPACITY, "hop %d: a batch's frontier exceeds max_input_nodes = %lld", h,
@@ -525,8 +535,8 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   cudaEvent_t pe = g->prof.begin(st);
   launch_unique_count(st, g->cnt8.p, g->cnt_words, g->R, g->tiles32.p, g->stats.p, g->hist.p, w->uniq.p, w->cnt.p);
   g->prof.end(st, pe, GG_PROF_UNIQUE, 0);
-  CU(cudaMemcpyAsync(g->h_small, g->stats.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-  CU(cudaMemcpyAsync(g->h_small + 1, g->hist.p, 256 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  launch_copy_words(st, g->h_small, g->stats.p, 1);
+  launch_copy_words(st, g->h_small + 1, g->hist.p, 256);
   CU(cudaEventRecord(w->sampled, st));
   CU(cudaStreamSynchronize(st));
   w->n_unique = g->h_small[0];
@@ -538,6 +548,7 @@ static gg_status stage_a(gg_graph* g, Window* w) {
     g->prof.bytes[GG_PROF_UNIQUE] += 4ll * w->n_access + 8ll * w->n_unique;
   }
   w->ms_unique = (float)(now_ms() - t1);
+  tl("a_end", w->id);
   CU(cudaGetLastError());
   return GG_OK;
 }
@@ -567,8 +578,11 @@ static void pack_rows(uint8_t* resp, const uint8_t* base, const int32_t* ids, in
   if (nt) _mm_sfence();
 }
 
-// ---- phase B (stager thread, stream `side_b`): a-4, a-5, a-6 --------------------------------
-static gg_status stage_b(gg_graph* g, Window* w) {
+// ---- phase B1 (selector thread, stream `side_b`): a-4, a-5 and the request IDs to the host ----
+// ---- phase B2 (stager thread, stream `side_c`): a-6 -------------------------------------------
+// Two threads so that window k+1's hot set, delta and request lists are already on the host when
+// the stager finishes packing window k: the host link then never waits for a kernel round trip.
+static gg_status stage_b1(gg_graph* g, Window* w) {
   const int Wmax = g->cfg.max_window;
   cudaStream_t st = g->side_b;
   CU(cudaSetDevice(g->device));
@@ -579,11 +593,13 @@ static gg_status stage_b(gg_graph* g, Window* w) {
     std::unique_lock<std::mutex> l(g->mu);
     g->cv_done.wait(l, [&] {
       Window* t = cs->tenant;
-      return g->stop || !t || t->seq + 2 != w->seq || !t->live;
+      return g->stop || !t || t->seq + (uint64_t)g->n_cs != w->seq || !t->live;
     });
     if (g->stop) return fail(GG_ERR_STATE, "graph is being destroyed");
   }
   const double t0 = now_ms();
+  w->t_b0 = t0;
+  tl("b1_start", w->id);
   CU(cudaStreamWaitEvent(st, w->sampled, 0));
   if (cs->gather_recorded) CU(cudaStreamWaitEvent(st, cs->gather_done, 0));
   CacheSlot* prev = g->prev_cs;
@@ -617,34 +633,56 @@ static gg_status stage_b(gg_graph* g, Window* w) {
   cs->tenant = w;
   g->prof.end(st, pe, GG_PROF_SELECT, 12ll * w->n_unique);
   int32_t* hs = g->h_small_b;
-  CU(cudaMemcpyAsync(hs, g->owner_cnt.p, 2 * GG_MAX_PARTS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-  CU(cudaMemcpyAsync(hs + 2 * GG_MAX_PARTS, g->n_delta_dev.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  launch_copy_words(st, hs, g->owner_cnt.p, 2 * GG_MAX_PARTS);
+  launch_copy_words(st, hs + 2 * GG_MAX_PARTS, g->n_delta_dev.p, 1);
+  tl("b1_launched", w->id);
   CU(cudaStreamSynchronize(st));
+  tl("b1_counts", w->id);
   w->n_delta = w->n_hot > 0 ? hs[2 * GG_MAX_PARTS] : 0;
   w->n_carry = w->n_hot - w->n_delta;
   for (int m = 0; m < GG_MAX_PARTS; ++m) {
     w->staged[m] = w->n_hot > 0 ? hs[m] : 0;
     w->bulk[m] = w->n_hot > 0 ? hs[GG_MAX_PARTS + m] : 0;
   }
-  const double t1 = now_ms();
-  w->ms_select = (float)(t1 - t0);
+  // request IDs of the bulk transfers -> this window's pinned buffer (mode 0)
+  if (g->cfg.staging_mode == 0 && w->n_delta > 0) {
+    void* pr = w->h_req;
+    // sized once for the largest request this graph can make (bounded at 32 MB up front): growing
+    // a pinned buffer frees and re-pins, which synchronises the device under the sampler
+    const int64_t want_b = std::max<int64_t>(w->n_delta * (int64_t)sizeof(int32_t),
+                                             std::min<int64_t>(g->cache_rows * (int64_t)sizeof(int32_t), 32ll << 20));
+    gg_status rc = ensure_pinned(&pr, &w->h_req_cap, want_b);
+    w->h_req = (int32_t*)pr;
+    if (rc != GG_OK) return rc;
+    tl("b1_pinned", w->id);
+    launch_copy_words(st, w->h_req, w->req_ids.p, w->n_delta);
+    CU(cudaStreamSynchronize(st));
+  }
+  w->prev_cs = prev;
+  g->prev_cs = cs;
+  w->ms_select = (float)(now_ms() - t0);
+  tl("b1_end", w->id, (double)w->n_delta);
+  CU(cudaGetLastError());
+  return GG_OK;
+}
 
+static gg_status stage_b2(gg_graph* g, Window* w) {
+  const int Wmax = g->cfg.max_window;
+  tl("b2_start", w->id);
+  CU(cudaSetDevice(g->device));
+  CacheSlot* cs = w->cs;
+  CacheSlot* prev = w->prev_cs;
   // a-6 staging: one bulk transfer per owner into that owner's contiguous slot range.  The
   // copies, the carry-over copy and the ready event go to stream C, which this thread never
-  // waits on: while the DMA engine drains window k's responses the thread already selects and
-  // packs window k+1 (two response buffers).  Everything C reads was produced on stream B
-  // before the cudaStreamSynchronize above, and B had waited for the old tenant's gathers.
+  // waits on: while the DMA engine drains window k's responses the thread already packs window
+  // k+1 (two response buffers).  Everything C reads was produced on stream B before phase B1's
+  // cudaStreamSynchronize, and B had waited for the old tenant's gathers.
   cudaStream_t sc = g->side_c;
   w->bulk_copies = 0;
   w->ms_pack = 0;
   const int64_t rb = g->rb;
   gg_status rc;
   if (g->cfg.staging_mode == 0 && w->n_delta > 0) {
-    void* pr = g->h_req;
-    rc = ensure_pinned(&pr, &g->h_req_cap, w->n_delta * (int64_t)sizeof(int32_t));
-    g->h_req = (int32_t*)pr;
-    if (rc != GG_OK) return rc;
-    CU(cudaMemcpyAsync(g->h_req, w->req_ids.p, (size_t)w->n_delta * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     const int ri = g->resp_idx;
     g->resp_idx ^= 1;
     if (g->resp_used[ri]) CU(cudaEventSynchronize(g->resp_free[ri]));  // its previous copies are done
@@ -652,7 +690,6 @@ static gg_status stage_b(gg_graph* g, Window* w) {
     rc = ensure_pinned(&pp, &g->h_resp_cap[ri], w->n_delta * rb);
     g->h_resp[ri] = (uint8_t*)pp;
     if (rc != GG_OK) return rc;
-    CU(cudaStreamSynchronize(st));
     int64_t q0 = 0;
     for (int m = 0; m < g->R.P; ++m) {
       const int64_t nm = w->bulk[m];
@@ -661,13 +698,14 @@ static gg_status stage_b(gg_graph* g, Window* w) {
       const double p0 = now_ms();
       const uint8_t* base = g->store.base[m];
       const int64_t lo = g->R.lo[m], stride = g->store.stride;
-      const int32_t* ids = g->h_req + q0;
+      const int32_t* ids = w->h_req + q0;
       uint8_t* resp = g->h_resp[ri] + q0 * rb;
       const int64_t chunk = 512;
       g->pool->parallel_for(ceil_div(nm, chunk), [&](int64_t c) {
         pack_rows(resp, base, ids, lo, stride, rb, c * chunk, std::min(nm, (c + 1) * chunk));
       });
       w->ms_pack += (float)(now_ms() - p0);
+      tl("pack_done", w->id, now_ms() - p0);
       cudaEvent_t pe = g->prof.begin(sc);
       CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies], sc));
       CU(cudaMemcpyAsync(cs->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, sc));
@@ -694,7 +732,7 @@ static gg_status stage_b(gg_graph* g, Window* w) {
     }
   }
   // carried rows: D2D out of the previous buffer (filled earlier on the same stream), after the delta rows
-  pe = g->prof.begin(sc);
+  cudaEvent_t pe = g->prof.begin(sc);
   CU(cudaEventRecord(w->ev_copy[2 * GG_MAX_PARTS], sc));
   if (w->n_carry > 0)
     launch_rows_from_list(sc, w->carry_src.p, (int)w->n_carry, prev->cache, rb, cs->cache, w->n_delta, rb, (int)rb);
@@ -704,8 +742,8 @@ static gg_status stage_b(gg_graph* g, Window* w) {
   CU(cudaEventRecord(w->ready, sc));
   w->timing_pending = true;
   CU(cudaGetLastError());
-  g->prev_cs = cs;
-  w->ms_total = w->ms_sample + w->ms_unique + (float)(now_ms() - t0);
+  w->ms_total = w->ms_sample + w->ms_unique + (float)(now_ms() - w->t_b0);
+  tl("b2_end", w->id);
   return GG_OK;
 }
 
@@ -768,7 +806,31 @@ static void worker_b_main(gg_graph* g) {
       w = g->jobs_b.front();
       g->jobs_b.pop_front();
     }
-    finish_job(g, w, stage_b(g, w));
+    gg_status rc = stage_b1(g, w);
+    if (rc != GG_OK) {
+      finish_job(g, w, rc);
+      continue;
+    }
+    {
+      std::lock_guard<std::mutex> l(g->mu);
+      g->jobs_c.push_back(w);
+    }
+    g->cv_c.notify_one();
+  }
+}
+
+static void worker_c_main(gg_graph* g) {
+  cudaSetDevice(g->device);
+  for (;;) {
+    Window* w;
+    {
+      std::unique_lock<std::mutex> l(g->mu);
+      g->cv_c.wait(l, [&] { return g->stop || !g->jobs_c.empty(); });
+      if (g->jobs_c.empty()) return;
+      w = g->jobs_c.front();
+      g->jobs_c.pop_front();
+    }
+    finish_job(g, w, stage_b2(g, w));
   }
 }
 
@@ -810,9 +872,11 @@ gg_status gg_graph_destroy(gg_graph* g) {
   }
   g->cv_a.notify_all();
   g->cv_b.notify_all();
+  g->cv_c.notify_all();
   g->cv_done.notify_all();
   if (g->worker_a.joinable()) g->worker_a.join();
   if (g->worker_b.joinable()) g->worker_b.join();
+  if (g->worker_c.joinable()) g->worker_c.join();
   cudaSetDevice(g->device);
   cudaDeviceSynchronize();
   delete g->pool;
@@ -828,9 +892,10 @@ gg_status gg_graph_destroy(gg_graph* g) {
     if (w.sampled) cudaEventDestroy(w.sampled);
     if (w.ready) cudaEventDestroy(w.ready);
     if (w.gather_done) cudaEventDestroy(w.gather_done);
+    if (w.h_req) cudaFreeHost(w.h_req);
     for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) if (w.ev_copy[c]) cudaEventDestroy(w.ev_copy[c]);
   }
-  for (int s = 0; s < 2; ++s) {
+  for (int s = 0; s < g->n_cs; ++s) {
     CacheSlot& c = g->cslot[s];
     c.hot.release();
     if (c.gather_done) cudaEventDestroy(c.gather_done);
@@ -848,7 +913,6 @@ gg_status gg_graph_destroy(gg_graph* g) {
   g->miss_pos.release(); g->miss_id.release(); g->n_miss.release();
   if (g->h_small) cudaFreeHost(g->h_small);
   if (g->h_small_b) cudaFreeHost(g->h_small_b);
-  if (g->h_req) cudaFreeHost(g->h_req);
   for (int i = 0; i < 2; ++i) {
     if (g->h_resp[i]) cudaFreeHost(g->h_resp[i]);
     if (g->resp_free[i]) cudaEventDestroy(g->resp_free[i]);
@@ -910,6 +974,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   for (int m = 0; m < GG_MAX_PARTS; ++m) g->store.base[m] = m < P ? (const uint8_t*)store->part_base[m] : nullptr;
   g->store.stride = store->row_stride_bytes;
   g->dim = store->dim; g->rb = (int)rb; g->dtype = store->dtype; g->cfg = *cfg;
+  g->n_cs = cfg->cache_buffers <= 0 ? 2 : std::min(std::max(cfg->cache_buffers, 2), GG_MAX_CACHE_BUFFERS);
   g->n_win = cfg->max_live_windows <= 0 ? 3 : std::min(std::max(cfg->max_live_windows, 3), GG_MAX_LIVE_WINDOWS);
   cudaGetDevice(&g->device);
   const int64_t n_remote_nodes = g->N - (g->R.lo[g->R.local + 1] - g->R.lo[g->R.local]);
@@ -964,7 +1029,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   }
   CUC(cudaStreamCreateWithFlags(&g->side_c, cudaStreamNonBlocking));
   for (int i = 0; i < 2; ++i) CUC(cudaEventCreateWithFlags(&g->resp_free[i], cudaEventDisableTiming));
-  for (int s = 0; s < 2; ++s) {
+  for (int s = 0; s < g->n_cs; ++s) {
     CacheSlot& c = g->cslot[s];
     CUC(cudaEventCreateWithFlags(&c.gather_done, cudaEventDisableTiming));
     CUC(cudaMalloc((void**)&c.cache, (size_t)std::max<int64_t>(g->cache_rows, 1) * rb));
@@ -985,6 +1050,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   g->pool = new Pool(nt > 1 ? nt : 0);
   g->worker_a = std::thread(worker_a_main, g);
   g->worker_b = std::thread(worker_b_main, g);
+  g->worker_c = std::thread(worker_c_main, g);
   *out = g;
   return GG_OK;
 }
@@ -1006,7 +1072,7 @@ static gg_status wait_enqueued(gg_graph* g, Window* w) {
     Window* t = w->cs ? w->cs->tenant : nullptr;
     for (int s = 0; s < g->n_win; ++s) {
       Window* o = &g->win[s];
-      if (o != w && o->live && o->seq + 2 == w->seq)
+      if (o != w && o->live && o->seq + (uint64_t)g->n_cs == w->seq)
         return fail(GG_ERR_STATE, "window %lld shares its cache buffer with live window %lld: release that one first",
                     (long long)w->id, (long long)o->id);
     }
@@ -1078,11 +1144,12 @@ gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_i
   }
   w->id = window_id; w->live = true; w->W = W; w->L = num_layers; w->first_batch = first_batch_index;
   w->seq = g->stage_counter;
-  w->cs = &g->cslot[g->stage_counter & 1];
+  w->cs = &g->cslot[g->stage_counter % (uint64_t)g->n_cs];
   for (int h = 0; h < num_layers; ++h) w->fanouts[h] = fanouts[h];
   w->seeds.assign(seeds, seeds + S);
   w->boff.assign(batch_offsets, batch_offsets + W + 1);
   w->ms_wait = 0;
+  tl("stage_call", window_id);
   {
     std::lock_guard<std::mutex> l(g->mu);
     w->enqueued = false; w->status = GG_OK; w->error.clear();
@@ -1113,6 +1180,7 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   if (!out->features || ((uintptr_t)out->features & 3)) return fail(GG_ERR_INVALID_ARG, "features must be a 4-byte aligned device buffer");
   gg_status rc = wait_enqueued(g, w);
   if (rc != GG_OK) return rc;
+  if (b == 0) tl("gather0_call", window_id);
   const int n = w->n_front[w->L][b];
   if (out->features_capacity_rows < n)
     return fail(GG_ERR_CAPACITY, "features_capacity_rows = %lld < n_input = %d", (long long)out->features_capacity_rows, n);
@@ -1161,12 +1229,13 @@ gg_status gg_window_release(gg_graph* g, int64_t window_id) {
     bool blocked = false;
     if (!w->enqueued)
       for (int s = 0; s < g->n_win; ++s)
-        if (&g->win[s] != w && g->win[s].live && g->win[s].seq + 2 == w->seq) blocked = true;
+        if (&g->win[s] != w && g->win[s].live && g->win[s].seq + (uint64_t)g->n_cs == w->seq) blocked = true;
     if (blocked) return fail(GG_ERR_STATE, "release the older live window first");
     g->cv_done.wait(l, [&] { return w->enqueued; });
     w->live = false;
   }
   g->cv_done.notify_all();
+  tl("release", window_id);
   return GG_OK;
 }
 
@@ -1293,7 +1362,7 @@ gg_status gg_cache_reset(gg_graph* g) {
     g->cv_done.wait(l, [&] { return g->busy == 0; });
   }
   CU(cudaDeviceSynchronize());
-  for (int s = 0; s < 2; ++s) {
+  for (int s = 0; s < g->n_cs; ++s) {
     CacheSlot& c = g->cslot[s];
     launch_slots_clear(g->side_b, c.hot.p, (int)c.n_cached, c.slot_map);
     c.n_cached = 0;
@@ -1444,8 +1513,8 @@ extern "C" gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_
       // a-3 over the window's slice of the trace
       launch_count_db(st, db.p, off[b0], off[b1], g->cnt8.p);
       launch_unique_count(st, g->cnt8.p, g->cnt_words, g->R, g->tiles32.p, g->stats.p, g->hist.p, w->uniq.p, w->cnt.p);
-      CUS(cudaMemcpyAsync(g->h_small, g->stats.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-      CUS(cudaMemcpyAsync(g->h_small + 1, g->hist.p, 256 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      launch_copy_words(st, g->h_small, g->stats.p, 1);
+      launch_copy_words(st, g->h_small + 1, g->hist.p, 256);
       CUS(cudaStreamSynchronize(st));
       const int64_t n_unique = g->h_small[0];
       int64_t n_remote = 0, n_hot = 0;

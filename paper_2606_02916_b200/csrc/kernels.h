@@ -73,6 +73,8 @@ void launch_delta_split(cudaStream_t st, const int32_t* hot, int n_hot, const Ow
                         int32_t* carry_src, int32_t* carry_ids);
 void launch_slots_clear(cudaStream_t st, const int32_t* ids, int n, int32_t* slot_map);
 void launch_fill_i32(cudaStream_t st, int32_t* p, int64_t n, int32_t v);
+// 32-bit words between device and pinned host memory by a kernel (not by a copy engine)
+void launch_copy_words(cudaStream_t st, void* dst, const void* src, int64_t n_words);
 
 // a-6 .. a-8
 struct GatherLaunch {

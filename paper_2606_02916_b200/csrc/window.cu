@@ -279,6 +279,22 @@ void launch_slots_clear(cudaStream_t st, const int32_t* ids, int n, int32_t* slo
   count_launches(1);
 }
 
+// Control-plane words (sizes, histograms, seeds, request IDs) between device memory and PINNED
+// host memory, moved by a kernel through the unified address space instead of the copy engines:
+// a cudaMemcpyAsync of a few bytes queues behind whatever bulk transfer occupies that engine
+// (a 181 MB staging copy holds the H2D engine for 3.8 ms), which stalled the sampler thread.
+__global__ void __launch_bounds__(256) k_copy_words(uint32_t* __restrict__ dst, const uint32_t* __restrict__ src, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    dst[i] = src[i];
+}
+void launch_copy_words(cudaStream_t st, void* dst, const void* src, int64_t n_words) {
+  if (n_words <= 0) return;
+  int64_t g = (n_words + 255) / 256;
+  if (g > 64) g = 64;
+  k_copy_words<<<(int)g, 256, 0, st>>>((uint32_t*)dst, (const uint32_t*)src, n_words);
+  count_launches(1);
+}
+
 void launch_fill_i32(cudaStream_t st, int32_t* p, int64_t n, int32_t v) {
   if (n <= 0) return;
   int64_t g = (n + 255) / 256;
