@@ -232,7 +232,9 @@ uint64_t gg_key(uint64_t seed, uint64_t batch, uint64_t layer, uint64_t dst, uin
 /* Live measurement support (bench.py roofline leg).  When enabled, the library brackets its own
  * kernel groups with CUDA events ON THE STREAM THEY ARE LAUNCHED ON (caller's stream for the
  * gather and miss path, the side stream for everything else) and counts algorithmic bytes:
- *   GATHER  one k_gather launch per region; bytes = |N_b| * (2*row_bytes + 8)
+ *   GATHER  one k_gather launch per region (one launch in four is bracketed when W >= 4, so that
+ *           the timing events do not serialise the caller's stream); bytes = |N_b| * (2*row_bytes + 8)
+ *           of the bracketed launches
  *   MISS    miss compaction + fill;          bytes = misses * 2*row_bytes   (counted at gg_trace time: 0 here)
  *   SAMPLE  count + scan + select of a hop;  bytes = 24*n_dst + 8*n_edge
  *   FRONTIER mark + word scan + emit + relabel of a hop; bytes = 8*n_edge + 4*n_new
