@@ -18,7 +18,7 @@ def oracle_parts(w):
 
 def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, max_cache_rows=0,
                 check_features=True, cache_samples=64, host_threads=0, oracle_threads=1, host_graph=None,
-                parts=None):
+                parts=None, cache_buffers=0, lookahead=2):
     """Runs one epoch on the GPU and on the oracle; asserts bit-exact agreement everywhere.
     Returns a small summary dict."""
     batches = w.batches if max_batches is None else w.batches[:max_batches]
@@ -35,7 +35,8 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
 
     g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=carry_over, max_window=max(W, 1),
                                staging_mode=staging_mode, max_cache_rows=max_cache_rows,
-                               host_threads=host_threads)
+                               host_threads=host_threads, cache_buffers=cache_buffers,
+                               max_live_windows=lookahead + 1)
     obatches = {}
     owin = {}
     stats = dict(batches=0, misses=0, windows=0, rows=0, edges=0)
@@ -112,7 +113,7 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
             assert np.array_equal(got, want), "cache rows"
         stats["windows"] += 1
 
-    ep.run_epoch(g, batches, w.fanouts, W, features, on_batch=on_batch, on_window=on_window)
+    ep.run_epoch(g, batches, w.fanouts, W, features, on_batch=on_batch, on_window=on_window, lookahead=lookahead)
     torch.cuda.synchronize()
     g.close()
     return stats

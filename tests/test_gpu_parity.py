@@ -42,6 +42,14 @@ def test_small_full_epoch(workload, dev, W, n_hot):
     assert s["batches"] == 10 and s["windows"] == -(-10 // W)
 
 
+@pytest.mark.parametrize("cache_buffers,lookahead", [(3, 2), (3, 5), (4, 6), (2, 4)])
+def test_small_more_cache_buffers_and_deeper_lookahead(workload, dev, cache_buffers, lookahead):
+    """cache_buffers > 2 and sampling several windows ahead change the schedule, not the results."""
+    w = workload("small", dev)
+    pu.check_epoch(w, W=1, n_hot=7500, cache_buffers=cache_buffers, lookahead=lookahead)
+    pu.check_epoch(w, W=2, n_hot=-1, carry_over=1, cache_buffers=cache_buffers, lookahead=lookahead)
+
+
 def test_small_no_carry_and_pull_mode(workload, dev):
     w = workload("small", dev)
     pu.check_epoch(w, W=4, n_hot=-1, carry_over=0)

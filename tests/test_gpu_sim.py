@@ -31,11 +31,16 @@ INT_KEYS = ("n_windows", "rebuild_events", "miss_events", "rebuild_rows", "miss_
 F64_KEYS = ("e_rebuild", "e_miss", "t_stall", "e_stall", "e_phy", "hit_ratio")
 
 
-def check(w, dev, candidates, n_hot, carry, batches=None, bw=5.0e10):
+def check(w, dev, candidates, n_hot, carry, batches=None, bw=5.0e10, oracle_threads=1):
     from paper_2606_02916_b200 import epoch as ep
     batches = w.batches if batches is None else batches
     og = ggo.Graph(*w.host_graph())
-    trace = [ggo.Batch(og, b, w.fanouts, w.seed, i).nodes for i, b in enumerate(batches)]
+    if oracle_threads > 1:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(oracle_threads) as ex:
+            trace = list(ex.map(lambda ib: ggo.Batch(og, ib[1], w.fanouts, w.seed, ib[0]).nodes, enumerate(batches)))
+    else:
+        trace = [ggo.Batch(og, b, w.fanouts, w.seed, i).nodes for i, b in enumerate(batches)]
     d, om = make_model(len(w.part_offsets) - 1, w.row_bytes, bw=bw)
     g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=carry, max_window=max(candidates))
     got = g.simulate(batches, w.fanouts, candidates, d, export=True)
@@ -73,6 +78,17 @@ def test_small_full_epoch_candidates(workload, dev):
 def test_products_mini_and_large_mini(workload, dev):
     check(workload("products_mini", dev), dev, [1, 4, 16], 4500, 1)
     check(workload("large_mini", dev), dev, [2, 8], 11250, 1)
+
+
+def test_products_full_size_first_32_batches(workload, dev):
+    """configs[2] at full size: the first 32 mini-batches of the epoch as the trace, budget = 10 %
+    of the remote nodes, candidates 4, 16, 32."""
+    import os
+    w = workload("products", dev)
+    n_remote = w.num_nodes - int(w.part_offsets[1] - w.part_offsets[0])
+    r = check(w, dev, [4, 16, 32], n_remote // 10, 1, batches=w.batches[:32],
+              oracle_threads=min(16, os.cpu_count() or 1))
+    assert r["results"][0]["miss_rows"] > 0 and r["results"][2]["n_windows"] == 1
 
 
 def test_simulate_then_run_epoch(workload, dev):
