@@ -96,6 +96,27 @@ def test_selection_fallback_paths_stay_exact(workload, dev, rank_shift, want_add
     assert after["fallbacks"] > before["fallbacks"], "the knob did not reach the fallback path"
 
 
+@pytest.mark.parametrize("fanouts", [[96, 40], [1, 1, 1], [16, 17], [3]])
+def test_extreme_fanouts(workload, dev, fanouts):
+    """GG_MAX_FANOUT (every row takes the warp kernel, ~122 candidates of the 128 the fast path
+    holds), fanout 1, the thread/warp cut-over at fanout 16 / 17, and a single layer."""
+    import dataclasses
+    w = dataclasses.replace(workload("dense_mini", dev), fanouts=list(fanouts))
+    pu.check_epoch(w, W=2, n_hot=-1, max_batches=2, check_features=False)
+    pu.check_epoch(w, W=1, n_hot=300, max_batches=2)
+
+
+def test_single_seed_batches_and_partial_last_window(workload, dev):
+    """Batches of one seed, a window of one batch, and a last window shorter than W."""
+    import dataclasses
+    w0 = workload("small", dev)
+    batches = [w0.batches[0][:1], w0.batches[1][:1], w0.batches[2][:7], w0.batches[3][:1], w0.batches[4][:2]]
+    w = dataclasses.replace(w0, batches=batches)
+    pu.check_epoch(w, W=2, n_hot=-1)
+    pu.check_epoch(w, W=4, n_hot=50)
+    pu.check_epoch(w, W=1, n_hot=0)
+
+
 def test_selection_fallbacks_are_rare_by_default(workload, dev):
     from paper_2606_02916_b200 import binding
     w = workload("dense_mini", dev)
