@@ -422,6 +422,7 @@ def run_ours(args):
                              "eps_init_J": max(model["eps_init"]), "eps_payload_J_per_row": max(model["eps_pay_b"]),
                              "bw_GB/s": model["bw"] / 1e9, "p_idle_W": model["p_idle"], "p_active_W": p_active,
                              "probes_bytes_s": probes},
+            "calibration": calibrate(sim["results"], meas_j),
             "note": "coefficients probed on this box (pinned H2D copies + NVML power); PAPER.md:186 reports < 5 s for the offline phase, "
                     "PAPER.md:345 Kendall tau 0.62-1.00 on its cluster",
         }
@@ -550,6 +551,22 @@ def run_ours(args):
     }
     print(json.dumps(out))
     g.close()
+
+
+def calibrate(results, meas_j):
+    """NEXT-3 (Eq. 5): rank calibration of S(W) = beta^T z(W) + gamma_W against the measured J/epoch
+    of the sweep, on the device (gg_rank_calibrate); z columns scaled to unit max."""
+    if any(x is None for x in meas_j):
+        return None
+    from paper_2606_02916_b200 import binding
+    Z = np.array([[r["rebuild_events"], r["miss_events"], r["t_stall"], r["hit_ratio"]] for r in results], dtype=np.float64)
+    Z = Z / np.maximum(np.abs(Z).max(axis=0), 1e-300)
+    e = np.array(meas_j, dtype=np.float64)
+    beta, gamma, loss = binding.rank_calibrate(Z, e, 0.1, 0.05, 2000)
+    S = Z @ beta + gamma
+    return {"beta": beta.tolist(), "gamma": gamma.tolist(), "loss": loss,
+            "kendall_tau_S_vs_measured_J": kendall_tau(S.tolist(), meas_j),
+            "features": ["rebuild_events", "miss_events", "t_stall", "hit_ratio"], "lambda": 0.1, "lr": 0.05, "iters": 2000}
 
 
 def kendall_tau(a, b):

@@ -321,6 +321,18 @@ gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_t* batch_of
                       const int32_t* Ws, int32_t nW, const gg_energy_model* model,
                       gg_sim_result* out, int32_t* best, int64_t* delta_out, int64_t* miss_out);
 
+/* ---- NEXT-3: rank calibration (Eq. 5) ------------------------------------------
+ * Fits S(W) = beta^T z(W) + gamma_W to the measured order of n calibration window sizes by
+ * fixed-step gradient descent (reading S26: the paper names no optimiser) from beta = gamma = 0 on
+ *   L = sum_{i<j} log(1 + exp(-sigma_ij (S(W_j) - S(W_i)))) + lambda ||beta||^2,
+ *   sigma_ij = sign(E_GT(W_j) - E_GT(W_i)) (pairs with equal E_GT contribute nothing).
+ * z: host [n][F] row-major (the simulator's z(W), scaled by the caller), e_gt: host [n] measured
+ * energies, iters steps of size lr.  Outputs (host): beta[F], gamma[n], *loss = L at the result.
+ * L(W) of Eq. 4 is beta^T z(W) + gamma_W; E_net(W) = E_phy(W) + L(W).
+ * Errors: INVALID_ARG for nulls, n outside [1,64], F outside [0,16], iters < 0. */
+gg_status gg_rank_calibrate(const double* z, const double* e_gt, int32_t n, int32_t F, double lambda_,
+                            double lr, int32_t iters, double* beta, double* gamma, double* loss);
+
 const char* gg_last_error(void);
 const char* gg_version(void);
 

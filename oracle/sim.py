@@ -152,3 +152,57 @@ def select_window(trace, part_offsets, local, n_hot, candidates: Sequence[int], 
         if res[i]["e_phy"] < res[best]["e_phy"]:
             best = i
     return candidates[best], res
+
+
+# ---- NEXT-3: rank calibration (Eq. 5) ------------------------------------------
+def rank_loss(beta: np.ndarray, gamma: np.ndarray, Z: np.ndarray, e_gt: np.ndarray, lam: float) -> float:
+    """Eq. (5): sum_{i<j} log(1 + exp(-sigma_ij (S_j - S_i))) + lam * ||beta||^2 with
+    S(W) = beta^T z(W) + gamma_W and sigma_ij = sign(E_GT(W_j) - E_GT(W_i))."""
+    n = len(e_gt)
+    S = [float(np.dot(beta, Z[i])) + float(gamma[i]) for i in range(n)]
+    loss = 0.0
+    for i in range(n):
+        for j in range(i + 1, n):
+            d = e_gt[j] - e_gt[i]
+            sg = 1.0 if d > 0 else (-1.0 if d < 0 else 0.0)
+            loss += float(np.log1p(np.exp(-sg * (S[j] - S[i]))))
+    return loss + lam * float(np.dot(beta, beta))
+
+
+def fit_rank_calibration(Z: np.ndarray, e_gt: np.ndarray, lam: float, lr: float, iters: int):
+    """Plain gradient descent on Eq. (5) from beta = 0, gamma = 0 ("optimization is lightweight ...
+    a linear model over a handful of features and seven candidates").  The paper
+    does not name the optimiser: fixed-step gradient descent is this build's reading (S26).
+    Every step: S_i, then for each pair i<j in order g = -sigma / (1 + exp(sigma (S_j - S_i))),
+    accumulated into dS_j (+g) and dS_i (-g); d beta = sum_i dS_i z_i + 2 lam beta; d gamma = dS.
+    Returns (beta, gamma, final loss)."""
+    Z = np.asarray(Z, dtype=np.float64)
+    e_gt = np.asarray(e_gt, dtype=np.float64)
+    n, F = Z.shape
+    beta = np.zeros(F)
+    gamma = np.zeros(n)
+    for _ in range(iters):
+        S = np.zeros(n)
+        for i in range(n):
+            acc = 0.0
+            for f in range(F):
+                acc = acc + beta[f] * Z[i, f]
+            S[i] = acc + gamma[i]
+        dS = np.zeros(n)
+        for i in range(n):
+            for j in range(i + 1, n):
+                d = e_gt[j] - e_gt[i]
+                sg = 1.0 if d > 0 else (-1.0 if d < 0 else 0.0)
+                if sg == 0.0:
+                    continue
+                g = -sg / (1.0 + float(np.exp(sg * (S[j] - S[i]))))
+                dS[j] = dS[j] + g
+                dS[i] = dS[i] - g
+        for f in range(F):
+            acc = 0.0
+            for i in range(n):
+                acc = acc + dS[i] * Z[i, f]
+            beta[f] = beta[f] - lr * (acc + (2.0 * lam) * beta[f])
+        for i in range(n):
+            gamma[i] = gamma[i] - lr * dS[i]
+    return beta, gamma, rank_loss(beta, gamma, Z, e_gt, lam)

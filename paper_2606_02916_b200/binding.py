@@ -85,7 +85,7 @@ PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage
 
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
-           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_simulate"]
+           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_simulate", "gg_rank_calibrate"]
 
 _lib = None
 
@@ -126,6 +126,7 @@ def load_library(path: Optional[str] = None):
     lib.gg_debug_sampler.argtypes = [i32, C.c_float]
     lib.gg_simulate.argtypes = [vp, vp, vp, i32, u64, vp, i32, vp, i32, P(gg_energy_model), P(gg_sim_result),
                                 P(i32), vp, vp]
+    lib.gg_rank_calibrate.argtypes = [vp, vp, i32, i32, C.c_double, C.c_double, i32, vp, vp, vp]
     lib.gg_last_error.restype = C.c_char_p
     lib.gg_version.restype = C.c_char_p
     for s in SYMBOLS:
@@ -155,6 +156,17 @@ def sampler_stats() -> dict:
 def debug_sampler(rank_shift: int = 0, want_add: float = 0.0) -> None:
     """Test knobs of the selection kernel (include/greengnn.h gg_debug_sampler)."""
     _check_global(load_library().gg_debug_sampler(rank_shift, want_add))
+
+
+def rank_calibrate(Z: np.ndarray, e_gt: np.ndarray, lam: float, lr: float, iters: int):
+    """Eq. (5) fit on the device (gg_rank_calibrate).  Returns (beta[F], gamma[n], loss)."""
+    Z = np.ascontiguousarray(Z, dtype=np.float64)
+    e = np.ascontiguousarray(e_gt, dtype=np.float64)
+    n, F = Z.shape
+    beta, gamma, loss = np.zeros(max(F, 1)), np.zeros(n), np.zeros(1)
+    _check_global(load_library().gg_rank_calibrate(Z.ctypes.data, e.ctypes.data, n, F, lam, lr, iters,
+                                                   beta.ctypes.data, gamma.ctypes.data, loss.ctypes.data))
+    return beta[:F], gamma, float(loss[0])
 
 
 def gg_key(seed: int, batch: int, layer: int, dst: int, edge_pos: int) -> int:

@@ -1575,3 +1575,12 @@ extern "C" gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_
   if (best) *best = bi;
   return GG_OK;
 }
+
+extern "C" gg_status gg_rank_calibrate(const double* z, const double* e_gt, int32_t n, int32_t F, double lambda_,
+                                       double lr, int32_t iters, double* beta, double* gamma, double* loss) {
+  if (!e_gt || !gamma || !loss || (F > 0 && (!z || !beta))) return fail(GG_ERR_INVALID_ARG, "null argument");
+  if (n < 1 || n > 64 || F < 0 || F > 16 || iters < 0)
+    return fail(GG_ERR_INVALID_ARG, "n must be in [1,64], F in [0,16], iters >= 0");
+  CU(rank_calibrate(z, e_gt, n, F, lambda_, lr, iters, beta, gamma, loss));
+  return GG_OK;
+}

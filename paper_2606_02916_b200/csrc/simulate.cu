@@ -124,6 +124,79 @@ __global__ void k_sim_events(const int32_t* __restrict__ delta, const int32_t* _
   out->hit_ratio = remote ? __ddiv_rn((double)hit_cache, (double)remote) : 1.0;
 }
 
+// ---- NEXT-3: rank calibration, Eq. (5) of PAPER.md:226-237 ----------------------------------------
+// S(W) = beta^T z(W) + gamma_W; L = sum_{i<j} log(1 + exp(-sigma_ij (S_j - S_i))) + lambda ||beta||^2.
+// Seven candidates and a handful of features: one thread walks the pairs in a fixed order, so
+// the only difference from a CPU run of the same steps is the last ulp of exp().
+constexpr int kCalMaxN = 64, kCalMaxF = 16;
+__global__ void k_rank_calibrate(const double* __restrict__ Z, const double* __restrict__ e_gt, int n, int F,
+                                 double lam, double lr, int iters, double* __restrict__ beta_out,
+                                 double* __restrict__ gamma_out, double* __restrict__ loss_out) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  double beta[kCalMaxF], gamma[kCalMaxN], S[kCalMaxN], dS[kCalMaxN];
+  for (int f = 0; f < F; ++f) beta[f] = 0.0;
+  for (int i = 0; i < n; ++i) gamma[i] = 0.0;
+  for (int it = 0; it <= iters; ++it) {
+    for (int i = 0; i < n; ++i) {
+      double acc = 0.0;
+      for (int f = 0; f < F; ++f) acc = __dadd_rn(acc, __dmul_rn(beta[f], Z[i * F + f]));
+      S[i] = __dadd_rn(acc, gamma[i]);
+      dS[i] = 0.0;
+    }
+    if (it == iters) break;
+    for (int i = 0; i < n; ++i)
+      for (int j = i + 1; j < n; ++j) {
+        const double d = e_gt[j] - e_gt[i];
+        const double sg = d > 0 ? 1.0 : (d < 0 ? -1.0 : 0.0);
+        if (sg == 0.0) continue;
+        const double g = __ddiv_rn(-sg, __dadd_rn(1.0, exp(__dmul_rn(sg, __dadd_rn(S[j], -S[i])))));
+        dS[j] = __dadd_rn(dS[j], g);
+        dS[i] = __dadd_rn(dS[i], -g);
+      }
+    for (int f = 0; f < F; ++f) {
+      double acc = 0.0;
+      for (int i = 0; i < n; ++i) acc = __dadd_rn(acc, __dmul_rn(dS[i], Z[i * F + f]));
+      beta[f] = __dadd_rn(beta[f], -__dmul_rn(lr, __dadd_rn(acc, __dmul_rn(__dmul_rn(2.0, lam), beta[f]))));
+    }
+    for (int i = 0; i < n; ++i) gamma[i] = __dadd_rn(gamma[i], -__dmul_rn(lr, dS[i]));
+  }
+  double loss = 0.0;
+  for (int i = 0; i < n; ++i)
+    for (int j = i + 1; j < n; ++j) {
+      const double d = e_gt[j] - e_gt[i];
+      const double sg = d > 0 ? 1.0 : (d < 0 ? -1.0 : 0.0);
+      loss += log1p(exp(-sg * (S[j] - S[i])));
+    }
+  double b2 = 0.0;
+  for (int f = 0; f < F; ++f) b2 += beta[f] * beta[f];
+  *loss_out = loss + lam * b2;
+  for (int f = 0; f < F; ++f) beta_out[f] = beta[f];
+  for (int i = 0; i < n; ++i) gamma_out[i] = gamma[i];
+}
+
+cudaError_t rank_calibrate(const double* z_host, const double* e_host, int n, int F, double lam, double lr,
+                           int iters, double* beta_host, double* gamma_host, double* loss_host) {
+  if (n < 1 || n > kCalMaxN || F < 0 || F > kCalMaxF) return cudaErrorInvalidValue;
+  double* d = nullptr;
+  const size_t nz = (size_t)n * (F > 0 ? F : 1);
+  cudaError_t e = cudaMalloc((void**)&d, (nz + 2 * n + kCalMaxF + 1) * sizeof(double));
+  if (e != cudaSuccess) return e;
+  double *dZ = d, *dE = d + nz, *dB = dE + n, *dG = dB + kCalMaxF, *dL = dG + n;
+  if (F > 0) cudaMemcpy(dZ, z_host, (size_t)n * F * sizeof(double), cudaMemcpyHostToDevice);
+  cudaMemcpy(dE, e_host, (size_t)n * sizeof(double), cudaMemcpyHostToDevice);
+  k_rank_calibrate<<<1, 32>>>(dZ, dE, n, F, lam, lr, iters, dB, dG, dL);
+  count_launches(1);
+  e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) {
+    if (F > 0) cudaMemcpy(beta_host, dB, (size_t)F * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaMemcpy(gamma_host, dG, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaMemcpy(loss_host, dL, sizeof(double), cudaMemcpyDeviceToHost);
+    e = cudaGetLastError();
+  }
+  cudaFree(d);
+  return e;
+}
+
 void launch_count_db(cudaStream_t st, const int32_t* db_nodes, int64_t begin, int64_t end, uint32_t* cnt8) {
   if (end <= begin) return;
   const int64_t n = end - begin;

@@ -119,3 +119,22 @@ def test_simulate_errors(workload, dev):
     assert e.value.status == binding.GG_ERR_STATE
     g.window_release(0)
     g.close()
+
+
+def test_rank_calibration_eq5(dev):
+    """gg_rank_calibrate against oracle/sim.fit_rank_calibration: same steps in the same order;
+    the device exp() may differ from libm's in the last ulp, which 3000 contracting gradient
+    steps do not amplify: relative tolerance 1e-9 on beta, gamma and the loss."""
+    from paper_2606_02916_b200 import binding
+    rng = np.random.default_rng(2)
+    for n, F, lam, lr, iters in [(7, 4, 0.1, 0.05, 3000), (6, 0, 0.0, 0.1, 200), (12, 3, 5.0, 0.01, 500), (2, 1, 0.1, 0.1, 10)]:
+        Z = rng.normal(size=(n, F))
+        e = rng.permutation(n).astype(np.float64) * 3.0 + 50.0
+        if n > 4:
+            e[1] = e[0]                                        # a tie in the ground truth
+        b, g, loss = binding.rank_calibrate(Z, e, lam, lr, iters)
+        wb, wg, wl = sim.fit_rank_calibration(Z, e, lam, lr, iters)
+        assert np.allclose(b, wb, rtol=1e-9, atol=1e-12) and np.allclose(g, wg, rtol=1e-9, atol=1e-12)
+        assert abs(loss - wl) <= 1e-9 * max(1.0, abs(wl))
+    with pytest.raises(binding.GreenGNNError):
+        binding.rank_calibrate(np.zeros((70, 2)), np.zeros(70), 0.1, 0.1, 1)

@@ -136,3 +136,45 @@ def test_window_selection_is_the_argmin_and_sees_the_trade_off(tiny_trace):
     # remote owner, so W batches x 3 owners become 3: 12 -> 6 -> 3 transfers for 4 batches
     full = [sim.simulate(trace, w.part_offsets, 0, -1, W, m, carry_over=0)["rebuild_events"] for W in cands]
     assert full == [12, 6, 3]
+
+
+# ---- NEXT-3: rank calibration, Eq. (5) ---------------------------------------------------------
+def _cal_problem(n=7, F=4, seed=2):
+    rng = np.random.default_rng(seed)
+    Z = rng.normal(size=(n, F))
+    e = rng.permutation(n).astype(np.float64) * 3.0 + 50.0        # a strict ground-truth ranking
+    return Z, e
+
+
+def test_rank_loss_closed_form_at_zero_and_gradient():
+    Z, e = _cal_problem()
+    n, F = Z.shape
+    lam = 0.3
+    # at beta = 0, gamma = 0 every pair contributes log 2
+    assert abs(sim.rank_loss(np.zeros(F), np.zeros(n), Z, e, lam) - (n * (n - 1) / 2) * np.log(2.0)) < 1e-12
+    # one gradient step of fit_rank_calibration equals -lr * (finite-difference gradient of Eq. 5)
+    lr, h = 1e-3, 1e-6
+    b1, g1, _ = sim.fit_rank_calibration(Z, e, lam, lr, 1)
+    for f in range(F):
+        d = np.zeros(F); d[f] = h
+        num = (sim.rank_loss(d, np.zeros(n), Z, e, lam) - sim.rank_loss(-d, np.zeros(n), Z, e, lam)) / (2 * h)
+        assert abs(b1[f] + lr * num) < 1e-9
+    for i in range(n):
+        d = np.zeros(n); d[i] = h
+        num = (sim.rank_loss(np.zeros(F), d, Z, e, lam) - sim.rank_loss(np.zeros(F), -d, Z, e, lam)) / (2 * h)
+        assert abs(g1[i] + lr * num) < 1e-9
+
+
+def test_rank_calibration_recovers_the_measured_order_and_regularises():
+    Z, e = _cal_problem()
+    l0 = sim.rank_loss(np.zeros(Z.shape[1]), np.zeros(len(e)), Z, e, 0.1)
+    beta, gamma, loss = sim.fit_rank_calibration(Z, e, 0.1, 0.05, 3000)
+    assert loss < 0.2 * l0
+    S = Z @ beta + gamma
+    assert np.array_equal(np.argsort(S), np.argsort(e))           # Kendall tau = 1 on the calibration set
+    b_big, _, _ = sim.fit_rank_calibration(Z, e, 50.0, 0.005, 3000)
+    assert np.linalg.norm(b_big) < 0.1 * np.linalg.norm(beta)     # lambda ||beta||^2 shrinks beta
+    # ties in the ground truth contribute no gradient
+    e2 = e.copy(); e2[:] = 1.0
+    b0, g0, _ = sim.fit_rank_calibration(Z, e2, 0.1, 0.05, 10)
+    assert not b0.any() and not g0.any()
