@@ -20,8 +20,6 @@
 //                    per warp); rows it cannot prove exact are appended to a fallback list
 //   k_select_warp    bins with deg >= kThreadDeg, then the fallback list: ONE WARP PER ROW,
 //                    largest rows first, dynamic queue
-#include <cstdlib>
-
 #include "common.cuh"
 #include "kernels.h"
 
@@ -687,13 +685,7 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
   dim3 grid(tiles, W);
   SamplePlan* plan = static_cast<SamplePlan*>(wk.plan);
   const bool thread_path = fanout <= kThreadMaxFanout;
-  static int deg_log2 = -1;
-  if (deg_log2 < 0) {
-    const char* e = getenv("GG_THREAD_DEG_LOG2");
-    deg_log2 = e ? atoi(e) : kThreadDegLog2;
-    if (deg_log2 > 16) deg_log2 = 16;
-  }
-  const int min_warp_bin = thread_path ? 2 * deg_log2 : 0;
+  const int min_warp_bin = thread_path ? 2 * kThreadDegLog2 : 0;
   cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
   count_launches(thread_path ? 5 : 4);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
