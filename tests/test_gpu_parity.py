@@ -117,6 +117,21 @@ def test_single_seed_batches_and_partial_last_window(workload, dev):
     pu.check_epoch(w, W=1, n_hot=0)
 
 
+def test_max_window_255_counts_fill_the_8_bit_lanes(workload, dev):
+    """W = GG_MAX_WINDOW = 255 batches that all contain the same seed: its access count is 255,
+    the largest value the packed 8-bit counters hold; hot-set selection with a budget then has
+    a 255-bin histogram to threshold."""
+    import dataclasses
+    w0 = workload("small", dev)
+    hub = int(w0.batches[0][0])
+    batches = [np.array([hub, int(w0.batches[(i // 1000) % 10][i % 1000 + 1])], np.int32) for i in range(255)]
+    batches = [b if b[0] != b[1] else b[:1] for b in batches]
+    w = dataclasses.replace(w0, batches=batches)
+    s = pu.check_epoch(w, W=255, n_hot=2000)
+    assert s["windows"] == 1 and s["batches"] == 255
+    pu.check_epoch(w, W=128, n_hot=-1)
+
+
 def test_selection_fallbacks_are_rare_by_default(workload, dev):
     from paper_2606_02916_b200 import binding
     w = workload("dense_mini", dev)
