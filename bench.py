@@ -427,6 +427,40 @@ def run_ours(args):
                     "PAPER.md:345 Kendall tau 0.62-1.00 on its cluster",
         }
 
+    # ---- BASELINE.json configs[2]: batch in {1024, 2048, 4096} at the same W -------------------
+    vs_batch = {}
+    if not args.no_sweep and world == 1 and args.config == "products":
+        vs_batch[str(args.batch)] = {"mini_batches_per_s": value, "seeds_per_s": value * args.batch}
+        all_seeds = np.concatenate(batches)
+        for Bx in (2048, 4096):
+            if Bx == args.batch:
+                continue
+            bx = [all_seeds[i:i + Bx] for i in range(0, len(all_seeds), Bx)]
+            g.close()
+            g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=W, staging_mode=args.staging_mode,
+                                       max_live_windows=args.lookahead + 1, max_batch=Bx)
+            fx = torch.empty(int(cap_rows * Bx / args.batch) + 1024, w.dim, dtype=w.dtype, device=dev)
+            def ep_b():
+                ep.run_epoch(g, bx, w.fanouts, W, fx, stream=stream, first_window_id=0, lookahead=LA)
+                torch.cuda.synchronize(dev)
+                g.cache_reset()
+            n_warm = max(2, -(-(LA + 1) // max(1, -(-len(bx) // W))) + 1)      # every window arena used at least once
+            for _ in range(n_warm):
+                ep_b()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(3):
+                ep_b()
+            b.record(stream)
+            torch.cuda.synchronize(dev)
+            v = 3 * len(bx) / (a.elapsed_time(b) * 1e-3)
+            vs_batch[str(Bx)] = {"mini_batches_per_s": v, "seeds_per_s": v * Bx, "mini_batches_per_epoch": len(bx)}
+            del fx
+        g.close()
+        g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
+                                   staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
+                                   host_threads=args.host_threads)
+
     # ---- variant: epochs back to back with the cache carried over (reading S15: the cache
     # persists across epochs; the trace repeats), no reset and no drain between
     # epochs -- what a long training run sees after its first epoch
@@ -535,7 +569,7 @@ def run_ours(args):
         "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
         "roofline": roof, "roofline_gather": roof_gather, "kernels_alone": serial, "stages": stages, "vs_W": vs_w,
-        "J_per_epoch_vs_W": j_w, "simulator": simulator, "variants": variants,
+        "J_per_epoch_vs_W": j_w, "vs_batch_at_W": vs_batch, "simulator": simulator, "variants": variants,
         "gpu_stall_ms_per_step": (main["prof"]["wait"]["ms"] / args.steps) if "wait" in main["prof"] else None,
         "energy": {"J_per_step": (main["joules"] / args.steps) if main["joules"] is not None else None,
                    "avg_W": (main["joules"] / main["wall"]) if main["joules"] is not None else None,

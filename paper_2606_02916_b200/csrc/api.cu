@@ -686,10 +686,17 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
     const int ri = g->resp_idx;
     g->resp_idx ^= 1;
     if (g->resp_used[ri]) CU(cudaEventSynchronize(g->resp_free[ri]));  // its previous copies are done
-    void* pp = g->h_resp[ri];
-    rc = ensure_pinned(&pp, &g->h_resp_cap[ri], w->n_delta * rb);
-    g->h_resp[ri] = (uint8_t*)pp;
-    if (rc != GG_OK) return rc;
+    // both response buffers grow together: pinning hundreds of MB takes longer than a whole
+    // window, and the cold first window of an epoch lands on either buffer
+    for (int k = 0; k < 2; ++k) {
+      const int bi = k == 0 ? ri : (ri ^ 1);
+      if (g->h_resp_cap[bi] >= w->n_delta * rb) continue;
+      if (bi != ri && g->resp_used[bi]) CU(cudaEventSynchronize(g->resp_free[bi]));
+      void* pp = g->h_resp[bi];
+      rc = ensure_pinned(&pp, &g->h_resp_cap[bi], w->n_delta * rb);
+      g->h_resp[bi] = (uint8_t*)pp;
+      if (rc != GG_OK) return rc;
+    }
     int64_t q0 = 0;
     for (int m = 0; m < g->R.P; ++m) {
       const int64_t nm = w->bulk[m];
