@@ -422,6 +422,21 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
   g->planned_cnt_tmp = std::max(g->planned_cnt_tmp, cnt_tmp);
   g->planned_t64 = std::max(g->planned_t64, t64);
   g->planned_miss = std::max(g->planned_miss, mcap);
+  // every window arena now, while the pipeline is drained: an arena that met its first (or a
+  // larger) window inside an epoch used to cudaMalloc hundreds of MB under the running pipeline
+  for (int s = 0; s < g->n_win; ++s) {
+    Window* a = &g->win[s];
+    if (a->live) continue;
+    const int w0 = a->W, l0 = a->L;
+    int f0[GG_MAX_LAYERS];
+    for (int h = 0; h < GG_MAX_LAYERS; ++h) f0[h] = a->fanouts[h];
+    a->W = W; a->L = L;
+    for (int h = 0; h < L; ++h) a->fanouts[h] = fanouts[h];
+    gg_status rc = alloc_window(g, a);
+    a->W = w0; a->L = l0;
+    for (int h = 0; h < GG_MAX_LAYERS; ++h) a->fanouts[h] = f0[h];
+    if (rc != GG_OK) return rc;
+  }
   return GG_OK;
 }
 #undef ENS
