@@ -163,6 +163,53 @@ def test_lookahead_one_is_algorithm_1_literal(workload, dev):
         assert np.array_equal(a[0], c[0]) and torch.equal(a[1], c[1]) and np.array_equal(a[2], c[2])
 
 
+def test_pipeline_stress_X_b_is_the_same_for_every_schedule(workload, dev):
+    """X_b and N_b do not depend on W, n_hot, carry-over, staging mode, lookahead or
+    the number of cache buffers.  200 epochs over random schedules of the four-thread pipeline;
+    every batch's N_b and X_b must hash to the value of the first epoch (a lost wait between the
+    sampler, selector, stager and caller streams shows up here as a mismatch or a hang)."""
+    _stress(workload("small", dev), dev, n_cfg=40, epochs=5, max_window=8, ws=[1, 2, 3, 4, 8], seed=11)
+
+
+def test_pipeline_stress_at_products_size(workload, dev):
+    """The same check with full-size kernels (N = 2.4 M, ~340 k rows per batch), where the
+    streams really overlap: the first 40 mini-batches under 8 schedules."""
+    import dataclasses
+    w = workload("products", dev)
+    _stress(dataclasses.replace(w, batches=w.batches[:40]), dev, n_cfg=8, epochs=2, max_window=16,
+            ws=[1, 4, 7, 16], seed=12, budgets=[-1, 0, 180000])
+
+
+def _stress(w, dev, n_cfg, epochs, max_window, ws, seed, budgets=(-1, 0, 3000, 20000)):
+    from paper_2606_02916_b200 import epoch as ep
+    rng = np.random.default_rng(seed)
+    ref = {}
+    feats = torch.empty(min(w.num_nodes, 600_000), w.dim, dtype=w.dtype, device=dev)
+
+    def on_batch(k, j, bi, r):
+        x = r["features"].contiguous().view(torch.int32)
+        h = (int(x.to(torch.int64).sum().item()), int(r["input_nodes"].to(torch.int64).sum().item()), r["n_input"])
+        if bi in ref:
+            assert ref[bi] == h, "batch %d differs from the first epoch" % bi
+        else:
+            ref[bi] = h
+
+    wid = 0
+    for cfg_i in range(n_cfg):
+        la = int(rng.integers(1, 6))
+        g = ep.graph_from_workload(w, n_hot=int(rng.choice(list(budgets))), carry_over=int(rng.integers(0, 2)),
+                                   max_window=max_window, staging_mode=int(rng.integers(0, 2)), max_live_windows=la + 1,
+                                   cache_buffers=int(rng.integers(2, 5)), host_threads=int(rng.choice([0, 1, 3])))
+        for e in range(epochs):
+            W = int(rng.choice(ws))
+            ep.run_epoch(g, w.batches, w.fanouts, W, feats, on_batch=on_batch, first_window_id=wid, lookahead=la)
+            wid += 100
+            if rng.integers(0, 2):
+                g.cache_reset()
+        g.close()
+    assert len(ref) == len(w.batches)
+
+
 def test_determinism_two_epochs_identical(workload, dev):
     from paper_2606_02916_b200 import epoch as ep
     w = workload("small", dev)
