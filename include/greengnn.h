@@ -333,6 +333,30 @@ gg_status gg_simulate(gg_graph* g, const int32_t* seeds, const int64_t* batch_of
 gg_status gg_rank_calibrate(const double* z, const double* e_gt, int32_t n, int32_t F, double lambda_,
                             double lr, int32_t iters, double* beta, double* gamma, double* loss);
 
+/* ---- NEXT-4: the consumer the staging overlaps with (Alg. 1 l.15) ----------
+ * GraphSAGE with the mean aggregator over the blocks gg_batch_gather returns, fp32:
+ *   agg_i = mean of h_in[src_local[e]] over row i of the block (0 for an empty row)
+ *   h_out_i = act(h_in[i] W_self + agg_i W_neigh + b), ReLU on every layer but the last
+ * layer l consumes block num_layers-1-l (layer 0 reads the feature tensor X_b); the loss is the mean
+ * softmax cross-entropy of the seeds against `labels`; parameters move by plain SGD (no dropout:
+ * DESIGN.md reading S27).  dims: host [num_layers+1], dims[0] = feature dim (features must be
+ * GG_F32), dims[num_layers] = classes; 1 <= dims[l] <= 128 for l < num_layers, dims[l+1] <= 64.
+ * w_self / w_neigh / bias: host arrays of num_layers pointers to row-major [dims[l]][dims[l+1]] /
+ * [dims[l+1]] initial values (copied). */
+typedef struct gg_sage gg_sage;
+gg_status gg_sage_create(int32_t num_layers, const int32_t* dims, const float* const* w_self,
+                         const float* const* w_neigh, const float* const* bias, gg_sage** out);
+gg_status gg_sage_destroy(gg_sage* m);
+/* One training step on `cuda_stream` (asynchronous): forward, loss, backward, SGD update.
+ * batch: what gg_batch_gather filled (its features buffer must hold fp32 rows of dims[0]);
+ * labels: device int32 [blocks[0].n_dst] in [0, classes); loss_out: device float, receives the
+ * loss before the update (may be NULL).  The model's scratch grows on demand (that first call
+ * synchronises).  Errors: INVALID_ARG (nulls, layer count or dims that do not match the batch). */
+gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* labels, float lr,
+                       void* cuda_stream, float* loss_out);
+/* Copies layer l's parameters to host arrays (synchronises the device). */
+gg_status gg_sage_params(gg_sage* m, int32_t layer, float* w_self, float* w_neigh, float* bias);
+
 const char* gg_last_error(void);
 const char* gg_version(void);
 

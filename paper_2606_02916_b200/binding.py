@@ -85,7 +85,8 @@ PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage
 
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
-           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_simulate", "gg_rank_calibrate"]
+           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_simulate", "gg_rank_calibrate",
+           "gg_sage_create", "gg_sage_destroy", "gg_sage_step", "gg_sage_params"]
 
 _lib = None
 
@@ -127,6 +128,10 @@ def load_library(path: Optional[str] = None):
     lib.gg_simulate.argtypes = [vp, vp, vp, i32, u64, vp, i32, vp, i32, P(gg_energy_model), P(gg_sim_result),
                                 P(i32), vp, vp]
     lib.gg_rank_calibrate.argtypes = [vp, vp, i32, i32, C.c_double, C.c_double, i32, vp, vp, vp]
+    lib.gg_sage_create.argtypes = [i32, vp, vp, vp, vp, P(vp)]
+    lib.gg_sage_destroy.argtypes = [vp]
+    lib.gg_sage_step.argtypes = [vp, P(gg_batch_out), vp, C.c_float, vp, vp]
+    lib.gg_sage_params.argtypes = [vp, i32, vp, vp, vp]
     lib.gg_last_error.restype = C.c_char_p
     lib.gg_version.restype = C.c_char_p
     for s in SYMBOLS:
@@ -167,6 +172,55 @@ def rank_calibrate(Z: np.ndarray, e_gt: np.ndarray, lam: float, lr: float, iters
     _check_global(load_library().gg_rank_calibrate(Z.ctypes.data, e.ctypes.data, n, F, lam, lr, iters,
                                                    beta.ctypes.data, gamma.ctypes.data, loss.ctypes.data))
     return beta[:F], gamma, float(loss[0])
+
+
+class Sage:
+    """GraphSAGE-mean consumer (NEXT-4) over the blocks gg_batch_gather returns.
+    params: list per layer of dicts W_self [din, dout], W_neigh [din, dout], b [dout] (float32)."""
+
+    def __init__(self, params: Sequence[Dict[str, np.ndarray]], device):
+        self.lib = load_library()
+        self.device = torch.device(device)
+        self.dims = [int(params[0]["W_self"].shape[0])] + [int(p["W_self"].shape[1]) for p in params]
+        L = len(params)
+        keep = [[np.ascontiguousarray(p[k], dtype=np.float32) for p in params] for k in ("W_self", "W_neigh", "b")]
+        arrs = [(vp * L)(*[a.ctypes.data for a in ks]) for ks in keep]
+        dims = np.ascontiguousarray(self.dims, dtype=np.int32)
+        h = vp()
+        with torch.cuda.device(self.device):
+            _check_global(self.lib.gg_sage_create(L, dims.ctypes.data, arrs[0], arrs[1], arrs[2], C.byref(h)))
+        self.h, self.L = h, L
+        self.loss = torch.zeros(1, dtype=torch.float32, device=self.device)
+
+    def step(self, r: Dict, labels: torch.Tensor, lr: float, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        """One training step on the batch dict Graph.batch_gather returned; labels: int32 device
+        tensor [n_seeds].  Returns the (device) loss tensor of this step (asynchronous)."""
+        assert labels.is_cuda and labels.dtype == torch.int32 and labels.is_contiguous()
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        _check_global(self.lib.gg_sage_step(self.h, C.byref(r["_out"]), labels.data_ptr(), lr, st.cuda_stream,
+                                            self.loss.data_ptr()))
+        return self.loss
+
+    def params(self) -> List[Dict[str, np.ndarray]]:
+        out = []
+        for l in range(self.L):
+            ws = np.zeros((self.dims[l], self.dims[l + 1]), np.float32)
+            wn = np.zeros_like(ws)
+            b = np.zeros(self.dims[l + 1], np.float32)
+            _check_global(self.lib.gg_sage_params(self.h, l, ws.ctypes.data, wn.ctypes.data, b.ctypes.data))
+            out.append(dict(W_self=ws, W_neigh=wn, b=b))
+        return out
+
+    def close(self):
+        if self.h:
+            self.lib.gg_sage_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def gg_key(seed: int, batch: int, layer: int, dst: int, edge_pos: int) -> int:
@@ -314,6 +368,7 @@ class Graph:
         self._check(self.lib.gg_batch_gather(self.h, window_id, b, C.byref(o), st.cuda_stream))
         r = self._unpack(o)
         r["features"] = features[:o.n_input]
+        r["_out"] = o                      # the filled gg_batch_out (what gg_sage_step consumes)
         return r
 
     def misses(self, r: Dict):

@@ -40,6 +40,11 @@ static gg_status fail(gg_status s, const char* fmt, ...) {
   t_err = buf;
   return s;
 }
+// for the other translation units behind the ABI (sage.cu)
+gg_status report_error(gg_status s, const char* msg) {
+  t_err = msg;
+  return s;
+}
 #define CU(call)                                                                          \
   do {                                                                                    \
     cudaError_t e_ = (call);                                                              \

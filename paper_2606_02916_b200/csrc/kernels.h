@@ -114,6 +114,7 @@ void launch_classify(cudaStream_t st, const int32_t* db_nodes, const int64_t* db
 void launch_sim_events(cudaStream_t st, const int32_t* delta, const int32_t* counters, int K, int B, int W,
                        const gg_energy_model& E, int P, int64_t row_bytes, gg_sim_result* out_dev);
 
+gg_status report_error(gg_status s, const char* msg);   // sets gg_last_error() of the calling thread
 cudaError_t rank_calibrate(const double* z_host, const double* e_host, int n, int F, double lam, double lr,
                            int iters, double* beta_host, double* gamma_host, double* loss_host);
 
