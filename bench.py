@@ -494,6 +494,40 @@ def run_ours(args):
                     "193-batch epoch holds ONE batch, C_k = H_k (reading S11) then evicts almost everything, and the next epoch "
                     "starts nearly cold anyway"}
 
+    # ---- NEXT-4: the same epoch with the paper's consumer behind every gather (Alg. 1 l.15): a
+    # GraphSAGE-mean model, one layer per hop, 16 hidden units, 47 synthetic classes
+    if not args.no_sweep and world == 1 and w.dtype == torch.float32 and w.dim <= 128:
+        Lm = len(w.fanouts)
+        dims = [w.dim] + [16] * (Lm - 1) + [47]
+        rng = np.random.default_rng(7)
+        p0 = [dict(W_self=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
+                   W_neigh=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
+                   b=np.zeros(dims[l + 1], np.float32)) for l in range(Lm)]
+        model = binding.Sage(p0, dev)
+        labels = torch.randint(0, 47, (n_b, args.batch), dtype=torch.int32, device=dev)
+        losses = []
+
+        def train(k, j, bi, r):
+            model.step(r, labels[bi, :r["blocks"][0]["n_dst"]].contiguous(), 0.003, stream)
+
+        def epoch_c(wid0):
+            ep.run_epoch(g, batches, w.fanouts, W, feats, on_batch=train, stream=stream, first_window_id=wid0, lookahead=LA)
+            torch.cuda.synchronize(dev)
+            losses.append(float(model.loss.cpu()[0]))
+            g.cache_reset()
+        epoch_c(11 * 10 ** 6)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for e in range(3):
+            epoch_c(11 * 10 ** 6 + 1000 * (e + 1))
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        variants["with_graphsage_consumer"] = {
+            "value": 3 * n_b / (a.elapsed_time(b) * 1e-3), "unit": UNIT, "model": "GraphSAGE-mean, dims %s, SGD lr 0.003" % dims,
+            "last_batch_loss_per_epoch": losses,
+            "note": "forward + loss + backward + update of every mini-batch on the caller's stream right behind its gather"}
+        model.close()
+
     # ---- variant (NEXT-2): GPU-initiated pull staging instead of host pack + cudaMemcpyAsync ----
     if not args.no_sweep and world == 1 and args.staging_mode == 0:
         g.close()

@@ -7,9 +7,10 @@
 //                held TRANSPOSED in shared memory (lane-consecutive columns: no bank conflicts);
 //                writes agg (kept for the backward pass) and the activated output
 //   k_sage_loss  one thread per seed: softmax cross-entropy, its gradient, per-seed loss
-//   k_sage_bwd   per row: activation mask, parameter gradients accumulated in shared memory and
-//                flushed once per CTA, and (layers > 0) the gradient of the layer's input, scattered
-//                through the mean with float atomics
+//   k_sage_wgrad parameter gradients as a skinny reduction over the rows (register accumulators,
+//                coalesced reads of h_in / agg, g tiles in shared memory)
+//   k_sage_bwd   (layers > 0) the gradient of the layer's input: activation mask, the two small
+//                products against the transposed weights, scattered through the mean with float atomics
 //   k_sage_sgd   p -= lr * g, g = 0
 // Nothing here is a large dense contraction (hidden size 16): the step is bound by the gather-like
 // reads of the aggregation, not by tensor-core work.
@@ -30,20 +31,36 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
+// one halving step of the reduce-scatter butterfly: N values stay, N go to the partner lane
+template <int N, int OFF>
+__device__ __forceinline__ void bfly(float (&p)[16], int lane) {
+  const bool hi = (lane & OFF) != 0;
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    const float send = hi ? p[k] : p[k + N];
+    const float keepv = hi ? p[k + N] : p[k];
+    p[k] = keepv + __shfl_xor_sync(0xffffffffu, send, OFF);
+  }
+}
+
 template <bool RELU>
-__global__ void __launch_bounds__(kSageWarps * 32)
+__global__ void __launch_bounds__(kSageWarps * 32, 4)
 k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
            const int32_t* __restrict__ src_local, int n_dst, int din, int dout,
            const float* __restrict__ w_self, const float* __restrict__ w_neigh,
            const float* __restrict__ bias, float* __restrict__ agg_out, float* __restrict__ h_out) {
-  extern __shared__ float s_w[];   // [2][dout][din] transposed weights, then [dout] bias
+  extern __shared__ float s_w[];   // two weight matrices (layout below), then [dout] bias
   float* ws = s_w;
-  float* wn = s_w + dout * din;
-  float* sb = wn + dout * din;
+  float* wn = s_w + 17 * din + dout * din;   // room for either layout
+  float* sb = wn + 17 * din + dout * din;
+  // dout <= 16: rows of 17 floats per input column ([c][17]: odd pitch, lane-consecutive columns hit
+  // distinct banks and output o is an immediate offset); otherwise transposed [o][din]
+  const bool narrow = dout <= 16;
   for (int k = threadIdx.x; k < din * dout; k += blockDim.x) {
     const int c = k / dout, o = k - c * dout;
-    ws[o * din + c] = w_self[k];
-    wn[o * din + c] = w_neigh[k];
+    const int at = narrow ? c * 17 + o : o * din + c;
+    ws[at] = w_self[k];
+    wn[at] = w_neigh[k];
   }
   for (int k = threadIdx.x; k < dout; k += blockDim.x) sb[k] = bias[k];
   __syncthreads();
@@ -57,36 +74,75 @@ k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
       ac[s] = 0.0f;
     }
     const int e0 = indptr[i], e1 = indptr[i + 1];
-    for (int e = e0; e < e1; ++e) {
-      const int64_t src = __ldg(src_local + e);
+    for (int eb = e0; eb < e1; eb += 32) {
+      // 32 neighbor ids at a time, then their rows back to back (independent loads)
+      const int mine = eb + lane < e1 ? __ldg(src_local + eb + lane) : 0;
+      const int cnt = min(32, e1 - eb);
+#pragma unroll 4
+      for (int q = 0; q < cnt; ++q) {
+        const int64_t src = __shfl_sync(0xffffffffu, mine, q);
 #pragma unroll
-      for (int s = 0; s < kSlotsIn; ++s) {
-        const int c = lane + 32 * s;
-        if (c < din) ac[s] += h_in[src * din + c];
+        for (int s = 0; s < kSlotsIn; ++s) {
+          const int c = lane + 32 * s;
+          if (c < din) ac[s] += __ldg(h_in + src * din + c);
+        }
       }
     }
     const float deg = (float)(e1 - e0);
 #pragma unroll
     for (int s = 0; s < kSlotsIn; ++s) {
       const int c = lane + 32 * s;
-      if (e1 > e0) ac[s] = ac[s] / deg;
+      ac[s] = (e1 > e0 && c < din) ? ac[s] / deg : 0.0f;
       if (c < din) agg_out[(int64_t)i * din + c] = ac[s];
     }
-    float keep[kSlotsOut] = {0.0f, 0.0f};
-    for (int o = 0; o < dout; ++o) {
-      float p = 0.0f;
+    if (dout <= 16) {
+      // 16 partial sums per lane, reduced across the warp by a halving butterfly: 8+4+2+1+1
+      // shuffles instead of 16 x 5 (the per-output warp_sum made this kernel shuffle-bound)
+      float p[16];
+      const float* wsp[kSlotsIn];   // column clamped into the row: xs / ac are 0 beyond din, so no predicate is needed
+      const float* wnp[kSlotsIn];
 #pragma unroll
       for (int s = 0; s < kSlotsIn; ++s) {
-        const int c = lane + 32 * s;
-        if (c < din) p += xs[s] * ws[o * din + c] + ac[s] * wn[o * din + c];
+        const int cc = min(lane + 32 * s, din - 1);
+        wsp[s] = ws + cc * 17;
+        wnp[s] = wn + cc * 17;
       }
-      p = warp_sum(p);
-      if (lane == (o & 31)) keep[o >> 5] = p + sb[o];
-    }
 #pragma unroll
-    for (int t = 0; t < kSlotsOut; ++t) {
-      const int o = lane + 32 * t;
-      if (o < dout) h_out[(int64_t)i * dout + o] = RELU ? fmaxf(keep[t], 0.0f) : keep[t];
+      for (int o = 0; o < 16; ++o) {
+        float v = 0.0f;
+        if (o < dout) {      // warp-uniform
+#pragma unroll
+          for (int s = 0; s < kSlotsIn; ++s) v = fmaf(xs[s], wsp[s][o], fmaf(ac[s], wnp[s][o], v));
+        }
+        p[o] = v;
+      }
+      bfly<8, 16>(p, lane);
+      bfly<4, 8>(p, lane);
+      bfly<2, 4>(p, lane);
+      bfly<1, 2>(p, lane);
+      p[0] += __shfl_xor_sync(0xffffffffu, p[0], 1);
+      const int o = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+      if ((lane & 1) == 0 && o < dout) {
+        const float v = p[0] + sb[o];
+        h_out[(int64_t)i * dout + o] = RELU ? fmaxf(v, 0.0f) : v;
+      }
+    } else {
+      float keep[kSlotsOut] = {0.0f, 0.0f};
+      for (int o = 0; o < dout; ++o) {
+        float p = 0.0f;
+#pragma unroll
+        for (int s = 0; s < kSlotsIn; ++s) {
+          const int c = lane + 32 * s;
+          if (c < din) p += xs[s] * ws[o * din + c] + ac[s] * wn[o * din + c];
+        }
+        p = warp_sum(p);
+        if (lane == (o & 31)) keep[o >> 5] = p + sb[o];
+      }
+#pragma unroll
+      for (int t = 0; t < kSlotsOut; ++t) {
+        const int o = lane + 32 * t;
+        if (o < dout) h_out[(int64_t)i * dout + o] = RELU ? fmaxf(keep[t], 0.0f) : keep[t];
+      }
     }
   }
 }
@@ -128,7 +184,7 @@ __global__ void __launch_bounds__(1024) k_sage_loss_mean(const float* __restrict
 
 // d_out [n_dst][dout]: gradient of the loss wrt the layer's activated output.  Accumulates the
 // parameter gradients; when d_in != nullptr also the gradient wrt the layer's input rows.
-template <bool RELU>
+template <bool RELU, bool PARAMS>
 __global__ void __launch_bounds__(kSageWarps * 32)
 k_sage_bwd(const float* __restrict__ h_in, const float* __restrict__ agg, const float* __restrict__ h_out,
            const float* __restrict__ d_out, const int32_t* __restrict__ indptr,
@@ -136,7 +192,7 @@ k_sage_bwd(const float* __restrict__ h_in, const float* __restrict__ agg, const 
            const float* __restrict__ w_self, const float* __restrict__ w_neigh,
            float* __restrict__ g_self, float* __restrict__ g_neigh, float* __restrict__ g_bias,
            float* __restrict__ d_in) {
-  extern __shared__ float s_w[];   // [2][din*dout] gradient accumulators, [dout] bias grads, [2][dout][din] transposed weights
+  extern __shared__ float s_w[];   // [2][dout][din] gradient accumulators (transposed), [dout] bias grads, [2][dout][din] transposed weights
   float* as = s_w;
   float* an = as + din * dout;
   float* ab = an + din * dout;
@@ -161,7 +217,7 @@ k_sage_bwd(const float* __restrict__ h_in, const float* __restrict__ agg, const 
       if (o < dout) {
         v = d_out[(int64_t)i * dout + o];
         if (RELU && !(h_out[(int64_t)i * dout + o] > 0.0f)) v = 0.0f;
-        if (v != 0.0f) atomicAdd(&ab[o], v);
+        if (PARAMS && v != 0.0f) atomicAdd(&ab[o], v);
       }
       g[t] = v;
     }
@@ -181,8 +237,10 @@ k_sage_bwd(const float* __restrict__ h_in, const float* __restrict__ agg, const 
       for (int s = 0; s < kSlotsIn; ++s) {
         const int c = lane + 32 * s;
         if (c < din) {
-          atomicAdd(&as[c * dout + o], xs[s] * go);
-          atomicAdd(&an[c * dout + o], ag[s] * go);
+          if (PARAMS) {
+            atomicAdd(&as[o * din + c], xs[s] * go);   // transposed: lane-consecutive columns, no bank conflicts
+            atomicAdd(&an[o * din + c], ag[s] * go);
+          }
           if (d_in) {
             ds[s] += go * ws[o * din + c];
             da[s] += go * wn[o * din + c];
@@ -208,13 +266,83 @@ k_sage_bwd(const float* __restrict__ h_in, const float* __restrict__ agg, const 
       }
     }
   }
+  if (!PARAMS) return;
   __syncthreads();
   for (int k = threadIdx.x; k < din * dout; k += blockDim.x) {
-    if (as[k] != 0.0f) atomicAdd(&g_self[k], as[k]);
-    if (an[k] != 0.0f) atomicAdd(&g_neigh[k], an[k]);
+    const int c = k / dout, o = k - c * dout;
+    const float vs = as[o * din + c], vn = an[o * din + c];
+    if (vs != 0.0f) atomicAdd(&g_self[k], vs);
+    if (vn != 0.0f) atomicAdd(&g_neigh[k], vn);
   }
   for (int k = threadIdx.x; k < dout; k += blockDim.x)
     if (ab[k] != 0.0f) atomicAdd(&g_bias[k], ab[k]);
+}
+
+// Parameter gradients of a layer as a skinny reduction over the destination rows:
+//   dW_self = h_in[:n_dst]^T g, dW_neigh = agg^T g, db = sum g,   g = d_out masked by the ReLU.
+// Thread t owns input column c = t % 128 and the output half t / 128 (OH outputs) in registers; a CTA
+// walks tiles of 64 rows whose g rows sit in shared memory, reading h_in / agg coalesced once.
+constexpr int kWgRows = 64;
+template <bool RELU, int OH>
+__global__ void __launch_bounds__(256)
+k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, const float* __restrict__ h_out,
+             const float* __restrict__ d_out, int n_dst, int din, int dout, float* __restrict__ g_self,
+             float* __restrict__ g_neigh, float* __restrict__ g_bias) {
+  __shared__ float sg[kWgRows][2 * OH];
+  const int c = threadIdx.x & 127, half = threadIdx.x >> 7;
+  float a_s[OH], a_n[OH];
+#pragma unroll
+  for (int k = 0; k < OH; ++k) a_s[k] = a_n[k] = 0.0f;
+  float a_b = 0.0f;
+  const int tiles = (n_dst + kWgRows - 1) / kWgRows;
+  for (int t = blockIdx.x; t < tiles; t += gridDim.x) {
+    const int r0 = t * kWgRows, rows = min(kWgRows, n_dst - r0);
+    __syncthreads();
+    for (int k = threadIdx.x; k < kWgRows * 2 * OH; k += 256) {
+      const int r = k / (2 * OH), o = k - r * (2 * OH);
+      float v = 0.0f;
+      if (r < rows && o < dout) {
+        v = d_out[(int64_t)(r0 + r) * dout + o];
+        if (RELU && !(h_out[(int64_t)(r0 + r) * dout + o] > 0.0f)) v = 0.0f;
+      }
+      sg[r][o] = v;
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < 2 * OH)
+      for (int r = 0; r < rows; ++r) a_b += sg[r][threadIdx.x];
+    if (c < din) {
+      for (int r = 0; r < rows; ++r) {
+        const float xv = __ldg(h_in + (int64_t)(r0 + r) * din + c), av = __ldg(agg + (int64_t)(r0 + r) * din + c);
+#pragma unroll
+        for (int k = 0; k < OH; ++k) {
+          const float gv = sg[r][half * OH + k];
+          a_s[k] += xv * gv;
+          a_n[k] += av * gv;
+        }
+      }
+    }
+  }
+  if (c < din) {
+#pragma unroll
+    for (int k = 0; k < OH; ++k) {
+      const int o = half * OH + k;
+      if (o < dout) {
+        if (a_s[k] != 0.0f) atomicAdd(&g_self[c * dout + o], a_s[k]);
+        if (a_n[k] != 0.0f) atomicAdd(&g_neigh[c * dout + o], a_n[k]);
+      }
+    }
+  }
+  if ((int)threadIdx.x < 2 * OH && (int)threadIdx.x < dout && a_b != 0.0f) atomicAdd(&g_bias[threadIdx.x], a_b);
+}
+
+template <bool RELU>
+static void launch_wgrad(cudaStream_t st, const float* h_in, const float* agg, const float* h_out, const float* d_out,
+                         int n_dst, int din, int dout, float* gs, float* gn, float* gb) {
+  int grid = (n_dst + kWgRows - 1) / kWgRows;
+  grid = grid < 1 ? 1 : (grid > 148 * 4 ? 148 * 4 : grid);
+  if (dout <= 16) k_sage_wgrad<RELU, 8><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, gs, gn, gb);
+  else if (dout <= 48) k_sage_wgrad<RELU, 24><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, gs, gn, gb);
+  else k_sage_wgrad<RELU, 32><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, gs, gn, gb);
 }
 
 __global__ void __launch_bounds__(256) k_sage_sgd(float* __restrict__ p, float* __restrict__ g, int n, float lr) {
@@ -352,8 +480,8 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     const int big = 160 * 1024;
     cudaFuncSetAttribute(k_sage_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sage_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sage_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sage_bwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    cudaFuncSetAttribute(k_sage_bwd<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    cudaFuncSetAttribute(k_sage_bwd<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     attr_set = true;
   }
   auto grid_for = [](int n) { int g = (n + kSageWarps - 1) / kSageWarps; return g < 1 ? 1 : (g > 148 * 8 ? 148 * 8 : g); };
@@ -362,7 +490,7 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
   for (int l = 0; l < L; ++l) {
     const gg_block& b = batch->blocks[L - 1 - l];
     const int din = m->dims[l], dout = m->dims[l + 1];
-    const size_t smem = (size_t)(2 * din * dout + dout) * sizeof(float);
+    const size_t smem = (size_t)(2 * (17 * din + din * dout) + dout) * sizeof(float);
     if (l < L - 1)
       k_sage_fwd<true><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h, b.indptr, b.src_local, b.n_dst, din, dout,
           p_self(m, l, m->params), p_neigh(m, l, m->params), p_bias(m, l, m->params), m->agg[l].p, m->out[l].p);
@@ -384,17 +512,25 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     if (d_in) cudaMemsetAsync(d_in, 0, (size_t)b.n_src * din * sizeof(float), st);
     const size_t smem = (size_t)(4 * din * dout + dout) * sizeof(float);
     if (l < L - 1)
-      k_sage_bwd<true><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h_in, m->agg[l].p, m->out[l].p, d_out, b.indptr,
-          b.src_local, b.n_dst, din, dout, p_self(m, l, m->params), p_neigh(m, l, m->params),
-          p_self(m, l, m->grads), p_neigh(m, l, m->grads), p_bias(m, l, m->grads), d_in);
+      launch_wgrad<true>(st, h_in, m->agg[l].p, m->out[l].p, d_out, b.n_dst, din, dout, p_self(m, l, m->grads),
+                         p_neigh(m, l, m->grads), p_bias(m, l, m->grads));
     else
-      k_sage_bwd<false><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h_in, m->agg[l].p, m->out[l].p, d_out, b.indptr,
-          b.src_local, b.n_dst, din, dout, p_self(m, l, m->params), p_neigh(m, l, m->params),
-          p_self(m, l, m->grads), p_neigh(m, l, m->grads), p_bias(m, l, m->grads), d_in);
+      launch_wgrad<false>(st, h_in, m->agg[l].p, m->out[l].p, d_out, b.n_dst, din, dout, p_self(m, l, m->grads),
+                          p_neigh(m, l, m->grads), p_bias(m, l, m->grads));
+    if (d_in) {
+      if (l < L - 1)
+        k_sage_bwd<true, false><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h_in, m->agg[l].p, m->out[l].p, d_out, b.indptr,
+            b.src_local, b.n_dst, din, dout, p_self(m, l, m->params), p_neigh(m, l, m->params),
+            p_self(m, l, m->grads), p_neigh(m, l, m->grads), p_bias(m, l, m->grads), d_in);
+      else
+        k_sage_bwd<false, false><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h_in, m->agg[l].p, m->out[l].p, d_out, b.indptr,
+            b.src_local, b.n_dst, din, dout, p_self(m, l, m->params), p_neigh(m, l, m->params),
+            p_self(m, l, m->grads), p_neigh(m, l, m->grads), p_bias(m, l, m->grads), d_in);
+    }
     d_out = d_in;
   }
   k_sage_sgd<<<(int)((m->n_params + 255) / 256), 256, 0, st>>>(m->params, m->grads, (int)m->n_params, lr);
-  count_launches(2 * L + 3);
+  count_launches(3 * L + 2);
   if (cudaGetLastError() != cudaSuccess) return report_error(GG_ERR_CUDA, "a consumer kernel failed to launch");
   return GG_OK;
 }
