@@ -132,6 +132,53 @@ def test_max_window_255_counts_fill_the_8_bit_lanes(workload, dev):
     pu.check_epoch(w, W=128, n_hot=-1)
 
 
+def _hub_workload(dev, seed=5):
+    """A graph with four hubs of 33 k .. 150 k in-edges among 200 k nodes of degree 3 whose rows
+    all contain a hub, so the hubs are destinations of hop 0 and of hop 1."""
+    from paper_2606_02916_b200 import inputs
+    rng = np.random.default_rng(seed)
+    n = 200_000
+    hub_deg = [33_000, 40_000, 70_000, 150_000]
+    rows = []
+    for h, d in enumerate(hub_deg):
+        rows.append(np.sort(rng.choice(np.arange(4, n), size=d, replace=False)).astype(np.int32))
+    small = np.stack([rng.integers(0, 4, n - 4), rng.integers(4, n, n - 4), rng.integers(4, n, n - 4)], axis=1)
+    small = np.sort(small, axis=1).astype(np.int32)
+    deg = np.concatenate([hub_deg, np.full(n - 4, 3)]).astype(np.int64)
+    indptr = np.concatenate([[0], np.cumsum(deg)]).astype(np.int64)
+    indices = np.concatenate(rows + [small.reshape(-1)]).astype(np.int32)
+    po = np.array([0, n // 4, n // 2, 3 * n // 4, n], np.int64)
+    dim = 8
+    feat = rng.normal(size=(n, dim)).astype(np.float32)
+    parts = []
+    for m in range(4):
+        t = torch.from_numpy(feat[po[m]:po[m + 1]].copy())
+        parts.append(t.to(dev) if m == 0 else t.pin_memory())
+    seeds = rng.permutation(np.arange(0, n))[:600].astype(np.int32)
+    seeds[:4] = [0, 1, 2, 3]                                   # the hubs are seeds of batch 0 too
+    batches = [seeds[i:i + 200].copy() for i in range(0, 600, 200)]
+    return inputs.Workload(name="hubs", cfg={}, num_nodes=n, indptr=torch.from_numpy(indptr).to(dev),
+                           indices=torch.from_numpy(indices).to(dev), part_offsets=po, local_part=0,
+                           feat_parts=parts, dim=dim, dtype=torch.float32, batches=batches,
+                           fanouts=[5, 4], seed=1234)
+
+
+def test_hub_rows_of_1e5_edges(dev):
+    from paper_2606_02916_b200 import binding
+    w = _hub_workload(dev)
+    pu.check_epoch(w, W=3, n_hot=-1)
+    pu.check_epoch(w, W=1, n_hot=1000)
+    # and the hand-over to the exact path when the proof fails on rows this long
+    before = binding.sampler_stats()
+    for rs, wa in [(28, 0.0), (0, 500.0), (0, -8.0)]:
+        binding.debug_sampler(rs, wa)
+        try:
+            pu.check_epoch(w, W=3, n_hot=-1, check_features=False)
+        finally:
+            binding.debug_sampler(0, 0.0)
+    assert binding.sampler_stats()["fallbacks"] > before["fallbacks"]
+
+
 def test_selection_fallbacks_are_rare_by_default(workload, dev):
     from paper_2606_02916_b200 import binding
     w = workload("dense_mini", dev)
