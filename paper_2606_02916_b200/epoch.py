@@ -63,3 +63,28 @@ def run_epoch(g: Graph, batches: Sequence[np.ndarray], fanouts: Sequence[int], W
             on_window(wid + k, win)
         g.window_release(wid + k)
     return n
+
+
+def choose_window(g: Graph, batches: Sequence[np.ndarray], fanouts: Sequence[int], candidates: Sequence[int],
+                  model: Dict) -> int:
+    """The paper's offline phase for one epoch: replay the trace for every
+    candidate W on the device (gg_simulate) and return W* = argmin E_phy(W)."""
+    return int(g.simulate(batches, fanouts, [int(c) for c in candidates], model)["best"])
+
+
+def run_adaptive(g: Graph, batches: Sequence[np.ndarray], fanouts: Sequence[int], candidates: Sequence[int],
+                 measure_model: Callable[[], Dict], epochs: int, features: torch.Tensor,
+                 stream: Optional[torch.cuda.Stream] = None, lookahead: int = 2) -> List[int]:
+    """NEXT-2, "adaptive W across epochs": before every epoch the coefficients are
+    re-measured (`measure_model()`, e.g. profiler.measure_energy_model) and W* is re-selected, so
+    a change of the link or of the power state moves the window size.  The trace itself repeats
+    (PAPER.md:126), so with constant coefficients W* is constant.  Returns the W used per epoch.
+    Pure call sequencing: everything is computed by gg_simulate and the runtime path."""
+    used = []
+    for e in range(epochs):
+        model = {k: v for k, v in measure_model().items() if k not in ("probes", "p_active")}
+        W = choose_window(g, batches, fanouts, candidates, model)
+        run_epoch(g, batches, fanouts, W, features, stream=stream, first_window_id=10 ** 7 + 10 ** 5 * e,
+                  lookahead=lookahead)
+        used.append(W)
+    return used

@@ -138,3 +138,30 @@ def test_rank_calibration_eq5(dev):
         assert abs(loss - wl) <= 1e-9 * max(1.0, abs(wl))
     with pytest.raises(binding.GreenGNNError):
         binding.rank_calibrate(np.zeros((70, 2)), np.zeros(70), 0.1, 0.1, 1)
+
+
+def test_adaptive_window_follows_the_coefficients(workload, dev):
+    """NEXT-2 (adaptive W): the per-epoch selector returns what the oracle's offline phase returns
+    for the coefficients measured before that epoch; a costly initiation selects the largest window."""
+    from paper_2606_02916_b200 import epoch as ep
+    w = workload("small", dev)
+    g = ep.graph_from_workload(w, n_hot=3000, max_window=8)
+    feats = torch.empty(w.num_nodes, w.dim, dtype=w.dtype, device=dev)
+    costly, _ = make_model(4, w.row_bytes)
+    costly["eps_init"] = [10.0] * 4
+    costly["lam_init"] = [1.0] * 4
+    cheap, _ = make_model(4, w.row_bytes)
+    cheap["eps_init"] = [0.0] * 4
+    cheap["lam_init"] = [0.0] * 4
+    cheap["eps_pay_a"] = [0.0] * 4
+    cheap["lam_pay_a"] = [0.0] * 4
+    seq = iter([costly, cheap])
+    used = ep.run_adaptive(g, w.batches, w.fanouts, [1, 2, 4, 8], lambda: next(seq), 2, feats)
+    og = ggo.Graph(*w.host_graph())
+    trace = [ggo.Batch(og, b, w.fanouts, w.seed, i).nodes for i, b in enumerate(w.batches)]
+    want = []
+    for d in (costly, cheap):
+        om = sim.EnergyModel(row_bytes=w.row_bytes, **d)
+        want.append(sim.select_window(trace, w.part_offsets, 0, 3000, [1, 2, 4, 8], om)[0])
+    assert used == want and used[0] == 8
+    g.close()
