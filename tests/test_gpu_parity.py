@@ -325,7 +325,7 @@ def test_products_full_size_first_window_W16(workload, dev):
     """configs[2] at full size (N=2,449,029, nnz=123.8M, dim 100), B=1024, W=16, n_hot unlimited:
     the first window (16 mini-batches, ~5.5M sampled nodes) against the oracle, every array."""
     w = workload("products", dev)
-    s = pu.check_epoch(w, W=16, n_hot=-1, max_batches=16, cache_samples=256)
+    s = pu.check_epoch(w, W=16, n_hot=-1, max_batches=16, cache_samples=256, lookahead=6)   # bench.py's arenas
     assert s["batches"] == 16 and s["misses"] == 0 and s["rows"] > 16 * 300_000
 
 
@@ -334,8 +334,8 @@ def test_products_full_size_budgeted_two_windows(workload, dev):
     exercises threshold selection, carry-over and the miss path at full size."""
     w = workload("products", dev)
     n_remote = w.num_nodes - int(w.part_offsets[1] - w.part_offsets[0])
-    s = pu.check_epoch(w, W=2, n_hot=n_remote // 10, max_batches=4, cache_samples=256)
-    assert s["windows"] == 2 and s["misses"] > 0
+    s = pu.check_epoch(w, W=2, n_hot=n_remote // 10, max_batches=6, cache_samples=256, lookahead=6)
+    assert s["windows"] == 3 and s["misses"] > 0
 
 
 def test_dense_full_size_first_window(workload, dev):
