@@ -14,6 +14,7 @@
 //   k_sage_sgd   p -= lr * g, g = 0
 // Nothing here is a large dense contraction (hidden size 16): the step is bound by the gather-like
 // reads of the aggregation, not by tensor-core work.
+#include <algorithm>
 #include <vector>
 
 #include "common.cuh"
@@ -286,19 +287,19 @@ constexpr int kWgRows = 64;
 template <bool RELU, int OH>
 __global__ void __launch_bounds__(256)
 k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, const float* __restrict__ h_out,
-             const float* __restrict__ d_out, int n_dst, int din, int dout, float* __restrict__ g_self,
-             float* __restrict__ g_neigh, float* __restrict__ g_bias) {
+             const float* __restrict__ d_out, int n_dst, int din, int dout, int tile_rows,
+             float* __restrict__ part /* [gridDim.x][2*din*dout + dout] per-CTA partial sums */) {
   __shared__ float sg[kWgRows][2 * OH];
   const int c = threadIdx.x & 127, half = threadIdx.x >> 7;
   float a_s[OH], a_n[OH];
 #pragma unroll
   for (int k = 0; k < OH; ++k) a_s[k] = a_n[k] = 0.0f;
   float a_b = 0.0f;
-  const int tiles = (n_dst + kWgRows - 1) / kWgRows;
+  const int tiles = (n_dst + tile_rows - 1) / tile_rows;
   for (int t = blockIdx.x; t < tiles; t += gridDim.x) {
-    const int r0 = t * kWgRows, rows = min(kWgRows, n_dst - r0);
+    const int r0 = t * tile_rows, rows = min(tile_rows, n_dst - r0);
     __syncthreads();
-    for (int k = threadIdx.x; k < kWgRows * 2 * OH; k += 256) {
+    for (int k = threadIdx.x; k < tile_rows * 2 * OH; k += 256) {
       const int r = k / (2 * OH), o = k - r * (2 * OH);
       float v = 0.0f;
       if (r < rows && o < dout) {
@@ -311,6 +312,7 @@ k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, cons
     if ((int)threadIdx.x < 2 * OH)
       for (int r = 0; r < rows; ++r) a_b += sg[r][threadIdx.x];
     if (c < din) {
+#pragma unroll 4
       for (int r = 0; r < rows; ++r) {
         const float xv = __ldg(h_in + (int64_t)(r0 + r) * din + c), av = __ldg(agg + (int64_t)(r0 + r) * din + c);
 #pragma unroll
@@ -322,27 +324,54 @@ k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, cons
       }
     }
   }
+  float* mine = part + (int64_t)blockIdx.x * (2 * din * dout + dout);
   if (c < din) {
 #pragma unroll
     for (int k = 0; k < OH; ++k) {
       const int o = half * OH + k;
       if (o < dout) {
-        if (a_s[k] != 0.0f) atomicAdd(&g_self[c * dout + o], a_s[k]);
-        if (a_n[k] != 0.0f) atomicAdd(&g_neigh[c * dout + o], a_n[k]);
+        mine[c * dout + o] = a_s[k];
+        mine[din * dout + c * dout + o] = a_n[k];
       }
     }
   }
-  if ((int)threadIdx.x < 2 * OH && (int)threadIdx.x < dout && a_b != 0.0f) atomicAdd(&g_bias[threadIdx.x], a_b);
+  if ((int)threadIdx.x < 2 * OH && (int)threadIdx.x < dout) mine[2 * din * dout + threadIdx.x] = a_b;
 }
 
+// grads[k] += sum over the CTAs' partials in a fixed order (8 interleaved slices, then the slices
+// in order): no atomics, the same bits every run
+__global__ void __launch_bounds__(256) k_sage_wreduce(const float* __restrict__ part, int n_part, int P,
+                                                      float* __restrict__ grads) {
+  __shared__ float sm[8][32];
+  const int kx = threadIdx.x & 31, sl = threadIdx.x >> 5;
+  const int k = blockIdx.x * 32 + kx;
+  float acc = 0.0f;
+  if (k < P)
+    for (int b = sl; b < n_part; b += 8) acc += part[(int64_t)b * P + k];
+  sm[sl][kx] = acc;
+  __syncthreads();
+  if (sl == 0 && k < P) {
+    float t = 0.0f;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) t += sm[q][kx];
+    grads[k] += t;
+  }
+}
+
+constexpr int kWgMaxGrid = 148 * 4;
 template <bool RELU>
 static void launch_wgrad(cudaStream_t st, const float* h_in, const float* agg, const float* h_out, const float* d_out,
-                         int n_dst, int din, int dout, float* gs, float* gn, float* gb) {
-  int grid = (n_dst + kWgRows - 1) / kWgRows;
-  grid = grid < 1 ? 1 : (grid > 148 * 4 ? 148 * 4 : grid);
-  if (dout <= 16) k_sage_wgrad<RELU, 8><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, gs, gn, gb);
-  else if (dout <= 48) k_sage_wgrad<RELU, 24><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, gs, gn, gb);
-  else k_sage_wgrad<RELU, 32><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, gs, gn, gb);
+                         int n_dst, int din, int dout, float* part, float* grads_layer) {
+  // few rows: smaller tiles so that every SM gets one (the tile loop is sequential per CTA)
+  int tile_rows = kWgRows;
+  while (tile_rows > 8 && (n_dst + tile_rows - 1) / tile_rows < 148 * 2) tile_rows >>= 1;
+  int grid = (n_dst + tile_rows - 1) / tile_rows;
+  grid = grid < 1 ? 1 : (grid > kWgMaxGrid ? kWgMaxGrid : grid);
+  if (dout <= 16) k_sage_wgrad<RELU, 8><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
+  else if (dout <= 48) k_sage_wgrad<RELU, 24><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
+  else k_sage_wgrad<RELU, 32><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
+  const int P = 2 * din * dout + dout;
+  k_sage_wreduce<<<(P + 31) / 32, 256, 0, st>>>(part, grid, P, grads_layer);
 }
 
 __global__ void __launch_bounds__(256) k_sage_sgd(float* __restrict__ p, float* __restrict__ g, int n, float lr) {
@@ -378,7 +407,7 @@ struct gg_sage {
   float* grads = nullptr;    // same layout
   int64_t off[GG_MAX_LAYERS + 1] = {0};
   int64_t n_params = 0;
-  gg::FBuf agg[GG_MAX_LAYERS], out[GG_MAX_LAYERS], dh[GG_MAX_LAYERS], loss_i;
+  gg::FBuf agg[GG_MAX_LAYERS], out[GG_MAX_LAYERS], dh[GG_MAX_LAYERS], loss_i, part;
   float* loss_dev = nullptr;
 };
 
@@ -404,6 +433,7 @@ gg_status gg_sage_destroy(gg_sage* m) {
     if (m->dh[l].p) cudaFree(m->dh[l].p);
   }
   if (m->loss_i.p) cudaFree(m->loss_i.p);
+  if (m->part.p) cudaFree(m->part.p);
   delete m;
   return GG_OK;
 }
@@ -471,7 +501,9 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     }
   }
   const int n_seed = batch->blocks[0].n_dst, C = m->dims[L];
-  if (m->loss_i.ensure(n_seed, &grew) != cudaSuccess) {
+  int64_t max_p = 0;
+  for (int l = 0; l < L; ++l) max_p = std::max<int64_t>(max_p, 2ll * m->dims[l] * m->dims[l + 1] + m->dims[l + 1]);
+  if (m->loss_i.ensure(n_seed, &grew) != cudaSuccess || m->part.ensure(max_p * kWgMaxGrid, &grew) != cudaSuccess) {
     cudaGetLastError();
     return report_error(GG_ERR_OOM, "device allocation failed");
   }
@@ -512,11 +544,9 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     if (d_in) cudaMemsetAsync(d_in, 0, (size_t)b.n_src * din * sizeof(float), st);
     const size_t smem = (size_t)(4 * din * dout + dout) * sizeof(float);
     if (l < L - 1)
-      launch_wgrad<true>(st, h_in, m->agg[l].p, m->out[l].p, d_out, b.n_dst, din, dout, p_self(m, l, m->grads),
-                         p_neigh(m, l, m->grads), p_bias(m, l, m->grads));
+      launch_wgrad<true>(st, h_in, m->agg[l].p, m->out[l].p, d_out, b.n_dst, din, dout, m->part.p, p_self(m, l, m->grads));
     else
-      launch_wgrad<false>(st, h_in, m->agg[l].p, m->out[l].p, d_out, b.n_dst, din, dout, p_self(m, l, m->grads),
-                          p_neigh(m, l, m->grads), p_bias(m, l, m->grads));
+      launch_wgrad<false>(st, h_in, m->agg[l].p, m->out[l].p, d_out, b.n_dst, din, dout, m->part.p, p_self(m, l, m->grads));
     if (d_in) {
       if (l < L - 1)
         k_sage_bwd<true, false><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h_in, m->agg[l].p, m->out[l].p, d_out, b.indptr,
@@ -530,7 +560,7 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     d_out = d_in;
   }
   k_sage_sgd<<<(int)((m->n_params + 255) / 256), 256, 0, st>>>(m->params, m->grads, (int)m->n_params, lr);
-  count_launches(3 * L + 2);
+  count_launches(4 * L + 2);
   if (cudaGetLastError() != cudaSuccess) return report_error(GG_ERR_CUDA, "a consumer kernel failed to launch");
   return GG_OK;
 }
