@@ -49,7 +49,7 @@ def test_key_function_matches_golden(lib):
 def test_struct_layouts_match_the_header(tmp_path, lib):
     from paper_2606_02916_b200 import binding
     names = ["gg_csr", "gg_owner_map", "gg_feature_store", "gg_config", "gg_block", "gg_batch_out",
-             "gg_window_trace", "gg_profile"]
+             "gg_window_trace", "gg_profile", "gg_energy_model", "gg_sim_result"]
     prog = '#include <stdio.h>\n#include "greengnn.h"\nint main(){' + "".join(
         'printf("%s %%zu\\n", sizeof(%s));' % (n, n) for n in names) + "return 0;}"
     src = tmp_path / "sz.c"
