@@ -329,6 +329,19 @@ def run_ours(args):
         return dict(sec=sec, wall=wall, launches=binding.launch_count() - l0, prof=prof, clocks=ck,
                     sampler=samp, joules=joules)
 
+    errors = {}
+
+    def recover_graph(old):
+        """After a failed optional leg: drop whatever state the graph is in and start a fresh one."""
+        try:
+            old.close()
+        except Exception:
+            pass
+        torch.cuda.synchronize(dev)
+        return ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
+                                      staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
+                                      host_threads=args.host_threads)
+
     # ---- headline: device-resident inputs --------------------------------------------------
     if args.no_profile:
         r0 = timed(W, args.steps, args.warmup, profile=False, clocks=None)
@@ -399,143 +412,163 @@ def run_ours(args):
     # ---- NEXT-1: the paper's offline phase on this box: coefficients probed here, then the trace
     # simulator + Eqs. (1)-(3) for every candidate W (gg_simulate), against the measured ranking
     simulator = None
-    if sweep_ws and rank == 0:
-        from paper_2606_02916_b200 import profiler
-        cands = sorted([W] + sweep_ws)
-        model = profiler.measure_energy_model(dev, w.row_bytes, P, local_part=rank % P)
-        probes = model.pop("probes")
-        p_active = model.pop("p_active")
-        t0 = time.perf_counter()
-        sim = g.simulate(batches, w.fanouts, cands, model)
-        t_sim = time.perf_counter() - t0
-        pred = [r["e_phy"] for r in sim["results"]]
-        meas_j = [j_w.get(str(c)) for c in cands]
-        meas_t = [n_b / vs_w[str(c)] for c in cands]
-        simulator = {
-            "candidates": cands, "W_star": sim["best"], "offline_phase_s": t_sim,
-            "e_phy_J": pred, "measured_J_per_epoch": meas_j, "measured_s_per_epoch": meas_t,
-            "kendall_tau_vs_measured_J": kendall_tau(pred, meas_j) if all(x is not None for x in meas_j) else None,
-            "kendall_tau_vs_measured_s": kendall_tau(pred, meas_t),
-            "z": [{k: r[k] for k in ("rebuild_events", "miss_events", "t_stall", "hit_ratio", "rebuild_rows", "miss_rows")}
-                  for r in sim["results"]],
-            "coefficients": {"lam_init_s": max(model["lam_init"]), "lam_payload_s_per_row": max(model["lam_pay_b"]),
-                             "eps_init_J": max(model["eps_init"]), "eps_payload_J_per_row": max(model["eps_pay_b"]),
-                             "bw_GB/s": model["bw"] / 1e9, "p_idle_W": model["p_idle"], "p_active_W": p_active,
-                             "probes_bytes_s": probes},
-            "calibration": calibrate(sim["results"], meas_j),
-            "note": "coefficients probed on this box (pinned H2D copies + NVML power); PAPER.md:186 reports < 5 s for the offline phase, "
-                    "PAPER.md:345 Kendall tau 0.62-1.00 on its cluster",
-        }
+    try:
+        if sweep_ws and rank == 0:
+            from paper_2606_02916_b200 import profiler
+            cands = sorted([W] + sweep_ws)
+            model = profiler.measure_energy_model(dev, w.row_bytes, P, local_part=rank % P)
+            probes = model.pop("probes")
+            p_active = model.pop("p_active")
+            t0 = time.perf_counter()
+            sim = g.simulate(batches, w.fanouts, cands, model)
+            t_sim = time.perf_counter() - t0
+            pred = [r["e_phy"] for r in sim["results"]]
+            meas_j = [j_w.get(str(c)) for c in cands]
+            meas_t = [n_b / vs_w[str(c)] for c in cands]
+            simulator = {
+                "candidates": cands, "W_star": sim["best"], "offline_phase_s": t_sim,
+                "e_phy_J": pred, "measured_J_per_epoch": meas_j, "measured_s_per_epoch": meas_t,
+                "kendall_tau_vs_measured_J": kendall_tau(pred, meas_j) if all(x is not None for x in meas_j) else None,
+                "kendall_tau_vs_measured_s": kendall_tau(pred, meas_t),
+                "z": [{k: r[k] for k in ("rebuild_events", "miss_events", "t_stall", "hit_ratio", "rebuild_rows", "miss_rows")}
+                      for r in sim["results"]],
+                "coefficients": {"lam_init_s": max(model["lam_init"]), "lam_payload_s_per_row": max(model["lam_pay_b"]),
+                                 "eps_init_J": max(model["eps_init"]), "eps_payload_J_per_row": max(model["eps_pay_b"]),
+                                 "bw_GB/s": model["bw"] / 1e9, "p_idle_W": model["p_idle"], "p_active_W": p_active,
+                                 "probes_bytes_s": probes},
+                "calibration": calibrate(sim["results"], meas_j),
+                "note": "coefficients probed on this box (pinned H2D copies + NVML power); PAPER.md:186 reports < 5 s for the offline phase, "
+                        "PAPER.md:345 Kendall tau 0.62-1.00 on its cluster",
+            }
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['simulator'] = repr(exc)
+        g = recover_graph(g)
 
     # ---- BASELINE.json configs[2]: batch in {1024, 2048, 4096} at the same W -------------------
     vs_batch = {}
-    if not args.no_sweep and world == 1 and args.config == "products":
-        vs_batch[str(args.batch)] = {"mini_batches_per_s": value, "seeds_per_s": value * args.batch}
-        all_seeds = np.concatenate(batches)
-        for Bx in (2048, 4096):
-            if Bx == args.batch:
-                continue
-            bx = [all_seeds[i:i + Bx] for i in range(0, len(all_seeds), Bx)]
-            g.close()
-            g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=W, staging_mode=args.staging_mode,
-                                       max_live_windows=args.lookahead + 1, max_batch=Bx)
-            fx = torch.empty(int(cap_rows * Bx / args.batch) + 1024, w.dim, dtype=w.dtype, device=dev)
-            def ep_b():
-                ep.run_epoch(g, bx, w.fanouts, W, fx, stream=stream, first_window_id=0, lookahead=LA)
+    try:
+        if not args.no_sweep and world == 1 and args.config == "products":
+            vs_batch[str(args.batch)] = {"mini_batches_per_s": value, "seeds_per_s": value * args.batch}
+            all_seeds = np.concatenate(batches)
+            for Bx in (2048, 4096):
+                if Bx == args.batch:
+                    continue
+                bx = [all_seeds[i:i + Bx] for i in range(0, len(all_seeds), Bx)]
+                g.close()
+                g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=W, staging_mode=args.staging_mode,
+                                           max_live_windows=args.lookahead + 1, max_batch=Bx)
+                fx = torch.empty(int(cap_rows * Bx / args.batch) + 1024, w.dim, dtype=w.dtype, device=dev)
+                def ep_b():
+                    ep.run_epoch(g, bx, w.fanouts, W, fx, stream=stream, first_window_id=0, lookahead=LA)
+                    torch.cuda.synchronize(dev)
+                    g.cache_reset()
+                n_warm = max(2, -(-(LA + 1) // max(1, -(-len(bx) // W))) + 1)      # every window arena used at least once
+                for _ in range(n_warm):
+                    ep_b()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(3):
+                    ep_b()
+                b.record(stream)
                 torch.cuda.synchronize(dev)
-                g.cache_reset()
-            n_warm = max(2, -(-(LA + 1) // max(1, -(-len(bx) // W))) + 1)      # every window arena used at least once
-            for _ in range(n_warm):
-                ep_b()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            for _ in range(3):
-                ep_b()
-            b.record(stream)
-            torch.cuda.synchronize(dev)
-            v = 3 * len(bx) / (a.elapsed_time(b) * 1e-3)
-            vs_batch[str(Bx)] = {"mini_batches_per_s": v, "seeds_per_s": v * Bx, "mini_batches_per_epoch": len(bx)}
-            del fx
-        g.close()
-        g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
-                                   staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
-                                   host_threads=args.host_threads)
+                v = 3 * len(bx) / (a.elapsed_time(b) * 1e-3)
+                vs_batch[str(Bx)] = {"mini_batches_per_s": v, "seeds_per_s": v * Bx, "mini_batches_per_epoch": len(bx)}
+                del fx
+            g.close()
+            g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
+                                       staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
+                                       host_threads=args.host_threads)
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['vs_batch'] = repr(exc)
+        g = recover_graph(g)
 
     # ---- variant: epochs back to back with the cache carried over (reading S15: the cache
     # persists across epochs; the trace repeats), no reset and no drain between
     # epochs -- what a long training run sees after its first epoch
     variants = {}
-    if not args.no_sweep and world == 1:
-        KE = 4
-        wins = ep.windows_of(n_b, W)
-        seq = [(e, k) for e in range(KE + 1) for k in range(len(wins))]      # epoch 0 warms the cache
-        wid = lambda i: 9 * 10 ** 6 + i
-        def stage_i(i):
-            win = wins[seq[i][1]]
-            g.window_stage(wid(i), win.start, [batches[j] for j in win], w.fanouts)
-        for i in range(min(LA, len(seq))):
-            stage_i(i)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for i in range(len(seq)):
-            if i == len(wins):
-                ev0.record(stream)                                           # first gather of epoch 1
-            if i + LA < len(seq):
-                stage_i(i + LA)
-            for j in range(len(wins[seq[i][1]])):
-                g.batch_gather(wid(i), j, feats, stream)
-            g.window_release(wid(i))
-        ev1.record(stream)
-        torch.cuda.synchronize(dev)
-        g.cache_reset()
-        variants["warm_cache_back_to_back_epochs"] = {
-            "value": KE * n_b / (ev0.elapsed_time(ev1) * 1e-3), "unit": UNIT, "epochs": KE,
-            "note": "no cache reset and no drain between epochs (the cache persists across epochs, the trace repeats): "
-                    "measured because the headline protocol resets the cache every epoch; it helps little here: the last window of a "
-                    "193-batch epoch holds ONE batch, C_k = H_k (reading S11) then evicts almost everything, and the next epoch "
-                    "starts nearly cold anyway"}
+    try:
+        if not args.no_sweep and world == 1:
+            KE = 4
+            wins = ep.windows_of(n_b, W)
+            seq = [(e, k) for e in range(KE + 1) for k in range(len(wins))]      # epoch 0 warms the cache
+            wid = lambda i: 9 * 10 ** 6 + i
+            def stage_i(i):
+                win = wins[seq[i][1]]
+                g.window_stage(wid(i), win.start, [batches[j] for j in win], w.fanouts)
+            for i in range(min(LA, len(seq))):
+                stage_i(i)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for i in range(len(seq)):
+                if i == len(wins):
+                    ev0.record(stream)                                           # first gather of epoch 1
+                if i + LA < len(seq):
+                    stage_i(i + LA)
+                for j in range(len(wins[seq[i][1]])):
+                    g.batch_gather(wid(i), j, feats, stream)
+                g.window_release(wid(i))
+            ev1.record(stream)
+            torch.cuda.synchronize(dev)
+            g.cache_reset()
+            variants["warm_cache_back_to_back_epochs"] = {
+                "value": KE * n_b / (ev0.elapsed_time(ev1) * 1e-3), "unit": UNIT, "epochs": KE,
+                "note": "no cache reset and no drain between epochs (the cache persists across epochs, the trace repeats): "
+                        "measured because the headline protocol resets the cache every epoch; it helps little here: the last window of a "
+                        "193-batch epoch holds ONE batch, C_k = H_k (reading S11) then evicts almost everything, and the next epoch "
+                        "starts nearly cold anyway"}
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['warm_cache'] = repr(exc)
+        g = recover_graph(g)
 
     # ---- NEXT-4: the same epoch with the paper's consumer behind every gather (Alg. 1 l.15): a
     # GraphSAGE-mean model, one layer per hop, 16 hidden units, 47 synthetic classes
-    if not args.no_sweep and world == 1 and w.dtype == torch.float32 and w.dim <= 128:
-        Lm = len(w.fanouts)
-        dims = [w.dim] + [16] * (Lm - 1) + [47]
-        rng = np.random.default_rng(7)
-        p0 = [dict(W_self=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
-                   W_neigh=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
-                   b=np.zeros(dims[l + 1], np.float32)) for l in range(Lm)]
-        model = binding.Sage(p0, dev)
-        labels = torch.randint(0, 47, (n_b, args.batch), dtype=torch.int32, device=dev)
-        losses = []
+    try:
+        if not args.no_sweep and world == 1 and w.dtype == torch.float32 and w.dim <= 128:
+            Lm = len(w.fanouts)
+            dims = [w.dim] + [16] * (Lm - 1) + [47]
+            rng = np.random.default_rng(7)
+            p0 = [dict(W_self=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
+                       W_neigh=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
+                       b=np.zeros(dims[l + 1], np.float32)) for l in range(Lm)]
+            model = binding.Sage(p0, dev)
+            labels = torch.randint(0, 47, (n_b, args.batch), dtype=torch.int32, device=dev)
+            losses = []
 
-        def train(k, j, bi, r):
-            model.step(r, labels[bi, :r["blocks"][0]["n_dst"]].contiguous(), 0.003, stream)
+            def train(k, j, bi, r):
+                model.step(r, labels[bi, :r["blocks"][0]["n_dst"]].contiguous(), 0.003, stream)
 
-        def epoch_c(wid0):
-            ep.run_epoch(g, batches, w.fanouts, W, feats, on_batch=train, stream=stream, first_window_id=wid0, lookahead=LA)
+            def epoch_c(wid0):
+                ep.run_epoch(g, batches, w.fanouts, W, feats, on_batch=train, stream=stream, first_window_id=wid0, lookahead=LA)
+                torch.cuda.synchronize(dev)
+                losses.append(float(model.loss.cpu()[0]))
+                g.cache_reset()
+            epoch_c(11 * 10 ** 6)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for e in range(3):
+                epoch_c(11 * 10 ** 6 + 1000 * (e + 1))
+            b.record(stream)
             torch.cuda.synchronize(dev)
-            losses.append(float(model.loss.cpu()[0]))
-            g.cache_reset()
-        epoch_c(11 * 10 ** 6)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        for e in range(3):
-            epoch_c(11 * 10 ** 6 + 1000 * (e + 1))
-        b.record(stream)
-        torch.cuda.synchronize(dev)
-        variants["with_graphsage_consumer"] = {
-            "value": 3 * n_b / (a.elapsed_time(b) * 1e-3), "unit": UNIT, "model": "GraphSAGE-mean, dims %s, SGD lr 0.003" % dims,
-            "last_batch_loss_per_epoch": losses,
-            "note": "forward + loss + backward + update of every mini-batch on the caller's stream right behind its gather"}
-        model.close()
+            variants["with_graphsage_consumer"] = {
+                "value": 3 * n_b / (a.elapsed_time(b) * 1e-3), "unit": UNIT, "model": "GraphSAGE-mean, dims %s, SGD lr 0.003" % dims,
+                "last_batch_loss_per_epoch": losses,
+                "note": "forward + loss + backward + update of every mini-batch on the caller's stream right behind its gather"}
+            model.close()
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['consumer'] = repr(exc)
+        g = recover_graph(g)
 
     # ---- variant (NEXT-2): GPU-initiated pull staging instead of host pack + cudaMemcpyAsync ----
-    if not args.no_sweep and world == 1 and args.staging_mode == 0:
-        g.close()
-        g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws), staging_mode=1,
-                                   max_live_windows=args.lookahead + 1)
-        r = timed(W, 3, 2)
-        variants["staging_mode_1_gpu_pull"] = {"value": 3 * n_b / r["sec"], "unit": UNIT,
-                                               "note": "k_rows<.,1> reads the owners' pinned rows over PCIe (12 CTAs), no host pack, no ID read-back"}
+    try:
+        if not args.no_sweep and world == 1 and args.staging_mode == 0:
+            g.close()
+            g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws), staging_mode=1,
+                                       max_live_windows=args.lookahead + 1)
+            r = timed(W, 3, 2)
+            variants["staging_mode_1_gpu_pull"] = {"value": 3 * n_b / r["sec"], "unit": UNIT,
+                                                   "note": "k_rows<.,1> reads the owners' pinned rows over PCIe (12 CTAs), no host pack, no ID read-back"}
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['gpu_pull'] = repr(exc)
+        g = recover_graph(g)
 
     if rank != 0:
         return
@@ -604,6 +637,7 @@ def run_ours(args):
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
         "roofline": roof, "roofline_gather": roof_gather, "kernels_alone": serial, "stages": stages, "vs_W": vs_w,
         "J_per_epoch_vs_W": j_w, "vs_batch_at_W": vs_batch, "simulator": simulator, "variants": variants,
+        "errors": errors,
         "gpu_stall_ms_per_step": (main["prof"]["wait"]["ms"] / args.steps) if "wait" in main["prof"] else None,
         "energy": {"J_per_step": (main["joules"] / args.steps) if main["joules"] is not None else None,
                    "avg_W": (main["joules"] / main["wall"]) if main["joules"] is not None else None,
