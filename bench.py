@@ -311,8 +311,11 @@ def run_ours(args):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
         e0.record(stream)
+        per_epoch = []
         for e in range(K):
-            one_epoch(Wx, sink, wid0=1000 * (warm + e))
+            t_e = time.perf_counter()
+            one_epoch(Wx, sink, wid0=1000 * (warm + e))      # ends with a device synchronise
+            per_epoch.append(1e3 * (time.perf_counter() - t_e))
         e1.record(stream)
         torch.cuda.synchronize(dev)
         wall = time.perf_counter() - t0
@@ -327,7 +330,7 @@ def run_ours(args):
         samp = {k: s1[k] - s0[k] for k in s0} if profile else None
         joules = (mj1 - mj0) / 1e3 if (mj0 is not None and mj1 is not None) else None
         return dict(sec=sec, wall=wall, launches=binding.launch_count() - l0, prof=prof, clocks=ck,
-                    sampler=samp, joules=joules)
+                    sampler=samp, joules=joules, per_epoch_ms=per_epoch)
 
     errors = {}
 
@@ -635,6 +638,8 @@ def run_ours(args):
                          % (w.num_nodes * w.row_bytes / 1e6, tr_acc["n_access"] / n_b * w.row_bytes / 1e6)},
         "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
+        "epoch_ms": {"median": statistics.median(main["per_epoch_ms"]), "min": min(main["per_epoch_ms"]),
+                     "max": max(main["per_epoch_ms"]), "note": "host clock around each epoch incl. its final synchronise and cache reset"},
         "roofline": roof, "roofline_gather": roof_gather, "kernels_alone": serial, "stages": stages, "vs_W": vs_w,
         "J_per_epoch_vs_W": j_w, "vs_batch_at_W": vs_batch, "simulator": simulator, "variants": variants,
         "errors": errors,
