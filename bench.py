@@ -545,14 +545,18 @@ def run_ours(args):
                 losses.append(float(model.loss.cpu()[0]))
                 g.cache_reset()
             epoch_c(11 * 10 ** 6)
+            g.profile_enable(True)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
             for e in range(3):
                 epoch_c(11 * 10 ** 6 + 1000 * (e + 1))
             b.record(stream)
             torch.cuda.synchronize(dev)
+            stall_c = g.profile_get()["wait"]["ms"] / 3
+            g.profile_enable(False)
             variants["with_graphsage_consumer"] = {
                 "value": 3 * n_b / (a.elapsed_time(b) * 1e-3), "unit": UNIT, "model": "GraphSAGE-mean, dims %s, SGD lr 0.003" % dims,
+                "gpu_stall_ms_per_epoch": stall_c,
                 "last_batch_loss_per_epoch": losses,
                 "note": "forward + loss + backward + update of every mini-batch on the caller's stream right behind its gather"}
             model.close()
