@@ -1169,22 +1169,25 @@ gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_i
     rc = ensure_shared(g, W, num_layers, fanouts, nullptr);
     if (rc != GG_OK) return rc;
   }
-  w->id = window_id; w->live = true; w->W = W; w->L = num_layers; w->first_batch = first_batch_index;
-  w->seq = g->stage_counter;
-  w->cs = &g->cslot[g->stage_counter % (uint64_t)g->n_cs];
-  for (int h = 0; h < num_layers; ++h) w->fanouts[h] = fanouts[h];
-  w->seeds.assign(seeds, seeds + S);
-  w->boff.assign(batch_offsets, batch_offsets + W + 1);
-  w->ms_wait = 0;
   tl("stage_call", window_id);
   {
+    // identity and sequence number change under the lock: the selector thread reads them in its
+    // wait predicate (is the cache slot's tenant still the live window n_cs stages back?)
     std::lock_guard<std::mutex> l(g->mu);
+    w->id = window_id; w->live = true; w->W = W; w->L = num_layers; w->first_batch = first_batch_index;
+    w->seq = g->stage_counter;
+    w->cs = &g->cslot[g->stage_counter % (uint64_t)g->n_cs];
+    for (int h = 0; h < num_layers; ++h) w->fanouts[h] = fanouts[h];
+    w->seeds.assign(seeds, seeds + S);
+    w->boff.assign(batch_offsets, batch_offsets + W + 1);
+    w->ms_wait = 0;
     w->enqueued = false; w->status = GG_OK; w->error.clear();
     g->jobs_a.push_back(w);
     g->busy += 1;
   }
   g->stage_counter += 1;
   g->cv_a.notify_one();
+  g->cv_done.notify_all();
   return GG_OK;
 }
 
