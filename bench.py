@@ -242,6 +242,13 @@ class E2ESink:
             self.done[k] = d
         self.i += 1
 
+    def fence(self, stream):
+        """Orders `stream` behind every copy issued so far: they read the window's block arrays and
+        N_b, which gg_window_release(stream) hands back to the sampler."""
+        last = self.done[(self.i - 1) & 1] if self.i else None
+        if last is not None:
+            stream.wait_event(last)
+
     def finish(self):
         self.copy_stream.synchronize()
 
@@ -291,7 +298,8 @@ def run_ours(args):
                     g.window_stage(wid0 + k + LA, nxt.start, [batches[i] for i in nxt], w.fanouts)
                 for j, _bi in enumerate(win):
                     sink.consume(g.batch_gather(wid0 + k, j, sink.buffer(), stream))
-                g.window_release(wid0 + k)
+                sink.fence(stream)
+                g.window_release(wid0 + k, stream)
             sink.finish()
         torch.cuda.synchronize(dev)
         g.cache_reset()

@@ -110,7 +110,9 @@ typedef struct {
                              to the miss path, it is never an error (reading S9) */
   int64_t max_input_nodes; /* cap on |N_b|; <= 0 = derived from the fanouts, capped at N */
   int32_t staging_mode;   /* 0 = owner-service pack on host threads + one cudaMemcpyAsync per
-                             owner (BASELINE.json:north_star (d));
+                             owner (BASELINE.json:north_star (d)); an owner whose store is DEVICE
+                             memory (e.g. a peer GPU's HBM) is served by the pull kernel instead,
+                             since host threads cannot read it;
                              1 = one GPU-initiated pull kernel per owner reading the pinned store */
   int32_t host_threads;   /* owner-service pack threads; <= 0 = min(16, hardware threads) */
   int32_t cache_buffers;  /* HBM cache buffers (+ slot maps) in rotation, window k uses k mod n.  2 = the
@@ -141,8 +143,12 @@ gg_status gg_graph_destroy(gg_graph* g);
  *                  keyed with first_batch_index+i (reading S7: epoch is not hashed)
  *   fanouts        host int32 [num_layers], hop order outward from the seeds, 1..GG_MAX_FANOUT
  * Errors: INVALID_ARG (nulls, W<1 or >max_window, L<1 or >max_layers, a batch larger than
- * max_batch or empty window, seed outside [0,N)), STATE (max_live_windows already live, or
- * window_id already live), CAPACITY (caps derived from fanouts exceed int32 indexing). */
+ * max_batch or empty window, seed outside [0,N)), STATE (max_live_windows already live,
+ * window_id already live, or the window needs larger shared scratch -- a bigger W or bigger
+ * fanouts than any window staged so far -- while other windows are live: release them first),
+ * CAPACITY (caps derived from fanouts exceed int32 indexing).  A frontier that outgrows
+ * max_input_nodes is reported as CAPACITY by the window's first gg_batch_info / gg_batch_gather;
+ * the window then holds no valid output and the graph stays usable after its release. */
 gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_index,
                           const int32_t* seeds, const int64_t* batch_offsets, int32_t W,
                           const int32_t* fanouts, int32_t num_layers);
@@ -161,7 +167,10 @@ typedef struct {
   const int32_t* input_nodes; /* device [n_input] = N_b; feature row i belongs to input_nodes[i] */
   void* features;             /* IN: caller-owned device buffer, row-major, row pitch = dim*elt */
   int64_t features_capacity_rows; /* IN */
-  /* miss list M_b in ascending position (valid after the gather's stream work completes) */
+  /* miss list M_b in ascending position.  ONE set of buffers per gg_graph: valid from the point of
+   * the gather's stream where this gather's work completes until the NEXT gg_batch_gather on this
+   * graph is enqueued, whose kernels overwrite them in stream order (work enqueued on the same
+   * stream between the two gathers reads them safely; another stream must be ordered by the caller) */
   const int32_t* miss_pos;  /* device [n_input] capacity */
   const int32_t* miss_id;   /* device */
   const int32_t* n_miss;    /* device scalar */
@@ -181,9 +190,17 @@ gg_status gg_batch_info(gg_graph* g, int64_t window_id, int32_t batch_in_window,
 gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t batch_in_window,
                           gg_batch_out* out, void* cuda_stream);
 
-/* Frees the window's blocks; its cache buffer becomes reusable once the gathers already
- * enqueued have run (the library orders this with events, the call does not block on the GPU). */
-gg_status gg_window_release(gg_graph* g, int64_t window_id);
+/* Ends the window's life: its blocks, N_b lists and miss lists may be overwritten by a later
+ * window, its cache buffer becomes reusable.  The call does not block on the GPU; the library
+ * orders the reuse behind
+ *   (1) every gg_batch_gather already enqueued for the window (on whatever stream it ran), and
+ *   (2) everything enqueued so far on `cuda_stream` (a cudaStream_t; NULL = default stream): the
+ *       stream on which the CALLER's last use of the window's device pointers was issued -- a
+ *       consumer step behind the last gather (gg_sage_step), a device-to-host copy of the blocks.
+ * A consumer that reads the window's pointers on some other stream must make `cuda_stream` wait
+ * for that stream (cudaStreamWaitEvent) before the release, or synchronise it.  The caller's own
+ * features buffer is not covered: it belongs to the caller. */
+gg_status gg_window_release(gg_graph* g, int64_t window_id, void* cuda_stream);
 
 typedef struct {
   int32_t W, num_parts;

@@ -113,7 +113,7 @@ def load_library(path: Optional[str] = None):
     lib.gg_window_stage.argtypes = [vp, i64, u64, vp, vp, i32, vp, i32]
     lib.gg_batch_info.argtypes = [vp, i64, i32, P(gg_batch_out)]
     lib.gg_batch_gather.argtypes = [vp, i64, i32, P(gg_batch_out), vp]
-    lib.gg_window_release.argtypes = [vp, i64]
+    lib.gg_window_release.argtypes = [vp, i64, vp]
     lib.gg_trace.argtypes = [vp, i64, P(gg_window_trace)]
     lib.gg_window_export.argtypes = [vp, i64, i32, vp, i64, P(i64)]
     lib.gg_cache_read.argtypes = [vp, i64, vp, i64, vp]
@@ -378,8 +378,11 @@ class Graph:
         n = int(_view_i32(nm, 1, self.device).cpu()[0])
         return (_view_i32(mp, n, self.device).cpu().numpy(), _view_i32(mi, n, self.device).cpu().numpy())
 
-    def window_release(self, window_id: int):
-        self._check(self.lib.gg_window_release(self.h, window_id))
+    def window_release(self, window_id: int, stream: Optional[torch.cuda.Stream] = None):
+        """stream: where the caller's last use of the window's device pointers was enqueued
+        (default: torch's current stream); the arena is recycled only behind that point."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._check(self.lib.gg_window_release(self.h, window_id, st.cuda_stream))
 
     # -- gg_trace / exports --------------------------------------------------------------------
     def trace(self, window_id: int, W: int) -> Dict:

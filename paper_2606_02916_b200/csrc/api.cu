@@ -203,6 +203,8 @@ struct Window {
   cudaEvent_t sampled = nullptr;  // phase A complete (stream A)
   cudaEvent_t ready = nullptr;    // cache ready (stream B)
   cudaEvent_t gather_done = nullptr;
+  cudaEvent_t consumer_done = nullptr;   // recorded by gg_window_release on the caller's stream
+  bool consumer_recorded = false;
   cudaEvent_t ev_copy[2 * GG_MAX_PARTS + 2] = {nullptr};  // start/stop per bulk copy, last pair = carry
   bool timing_pending = false;    // ms_h2d / ms_carry not yet read from the events
   int32_t* h_req = nullptr;       // pinned: this window's request IDs (device -> host), mode 0
@@ -280,6 +282,7 @@ struct gg_graph {
   const int32_t* indices = nullptr;
   OwnerRanges R;
   StorePtrs store;
+  bool store_on_device[GG_MAX_PARTS] = {false};  // a non-local owner whose rows the GPU addresses as device memory
   int dim = 0, rb = 0;
   gg_dtype dtype = GG_F32;
   gg_config cfg;
@@ -460,6 +463,17 @@ static gg_status ensure_pinned(void** p, int64_t* cap, int64_t want) {
   return GG_OK;
 }
 
+// A window that fails after its seeds were marked leaves bits in the per-batch bitmaps and counts
+// in the packed access counters that the sparse clear (which walks the node lists) cannot reach:
+// IDs beyond the frontier cap were never written to a list.  Dense reset, so the next window on
+// this graph starts from the clean state every window assumes.
+static void reset_sampler_state(gg_graph* g) {
+  cudaMemsetAsync(g->seen.p, 0, (size_t)g->F.gen_pitch * sizeof(uint32_t), g->side);
+  cudaMemsetAsync(g->newbits.p, 0, (size_t)g->F.gen_pitch * g->n_gen * sizeof(uint32_t), g->side);
+  cudaMemsetAsync(g->cnt8.p, 0, (size_t)g->cnt_words * sizeof(uint32_t), g->side);
+  cudaStreamSynchronize(g->side);
+}
+
 // ---- phase A (sampler thread, stream `side`): a-1, a-2, a-3 ---------------------------------
 static gg_status stage_a(gg_graph* g, Window* w) {
   const int W = w->W, L = w->L, Wmax = g->cfg.max_window;
@@ -474,6 +488,10 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   CU(cudaStreamWaitEvent(st, w->ready, 0));
   if (w->gather_recorded) CU(cudaStreamWaitEvent(st, w->gather_done, 0));
   w->gather_recorded = false;
+  // ... and by the consumer's own kernels / copies behind those gathers (the blocks, N_b): the
+  // release recorded the point of the caller's stream after which the arena may be overwritten
+  if (w->consumer_recorded) CU(cudaStreamWaitEvent(st, w->consumer_done, 0));
+  w->consumer_recorded = false;
 
   // seeds and per-(batch, layer) key prefixes -> device
   BatchOffsets seed_off;
@@ -528,9 +546,11 @@ static gg_status stage_a(gg_graph* g, Window* w) {
     launch_copy_words(st, g->h_small + Wmax, H.edge_off_dev.p, W + 1);
     launch_copy_words(st, g->h_small + 2 * Wmax + 2, g->err_flag.p, 1);
     CU(cudaStreamSynchronize(st));
-    if (g->h_small[2 * Wmax + 2])
+    if (g->h_small[2 * Wmax + 2]) {
+      reset_sampler_state(g);
       return fail(GG_ERR_CAPACITY, "hop %d: a batch's frontier exceeds max_input_nodes = %lld", h,
                   (long long)w->node_pitch);
+    }
     w->n_front[h + 1].assign(g->h_small, g->h_small + W);
     H.edge_off.assign(g->h_small + Wmax, g->h_small + Wmax + W + 1);
     if (g->prof.on) {
@@ -721,6 +741,18 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
     for (int m = 0; m < g->R.P; ++m) {
       const int64_t nm = w->bulk[m];
       if (nm == 0) continue;
+      if (g->store_on_device[m]) {
+        // this owner's store is device memory (e.g. a peer's HBM): host threads cannot read it, so
+        // its bulk transfer is the pull kernel of staging_mode 1, still one transfer per owner
+        cudaEvent_t pd = g->prof.begin(sc);
+        CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies], sc));
+        launch_rows_from_store(sc, w->req_ids.p + q0, (int)nm, g->store, g->R, cs->cache, q0, rb, (int)rb, false);
+        CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies + 1], sc));
+        g->prof.end(sc, pd, GG_PROF_STAGE_COPY, nm * rb);
+        w->bulk_copies += 1;
+        q0 += nm;
+        continue;
+      }
       // owner service: gather owner m's requested rows into a contiguous response
       const double p0 = now_ms();
       const uint8_t* base = g->store.base[m];
@@ -919,6 +951,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
     if (w.sampled) cudaEventDestroy(w.sampled);
     if (w.ready) cudaEventDestroy(w.ready);
     if (w.gather_done) cudaEventDestroy(w.gather_done);
+    if (w.consumer_done) cudaEventDestroy(w.consumer_done);
     if (w.h_req) cudaFreeHost(w.h_req);
     for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) if (w.ev_copy[c]) cudaEventDestroy(w.ev_copy[c]);
   }
@@ -999,6 +1032,9 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   for (int m = 0; m <= P; ++m) g->R.lo[m] = owners->part_offsets[m];
   for (int m = P + 1; m <= GG_MAX_PARTS; ++m) g->R.lo[m] = g->N;
   for (int m = 0; m < GG_MAX_PARTS; ++m) g->store.base[m] = m < P ? (const uint8_t*)store->part_base[m] : nullptr;
+  for (int m = 0; m < P; ++m)
+    g->store_on_device[m] = m != owners->local_part && store->part_base[m] &&
+                            owners->part_offsets[m] < owners->part_offsets[m + 1] && is_device_ptr(store->part_base[m]);
   g->store.stride = store->row_stride_bytes;
   g->dim = store->dim; g->rb = (int)rb; g->dtype = store->dtype; g->cfg = *cfg;
   g->n_cs = cfg->cache_buffers <= 0 ? 2 : std::min(std::max(cfg->cache_buffers, 2), GG_MAX_CACHE_BUFFERS);
@@ -1069,6 +1105,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
     CUC(cudaEventCreateWithFlags(&w.sampled, cudaEventDisableTiming));
     CUC(cudaEventCreateWithFlags(&w.ready, cudaEventDefault));
     CUC(cudaEventCreateWithFlags(&w.gather_done, cudaEventDisableTiming));
+    CUC(cudaEventCreateWithFlags(&w.consumer_done, cudaEventDisableTiming));
     for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) CUC(cudaEventCreate(&w.ev_copy[c]));
   }
   CUC(cudaDeviceSynchronize());
@@ -1161,6 +1198,14 @@ gg_status gg_window_stage(gg_graph* g, int64_t window_id, uint64_t first_batch_i
   gg_status rc = ensure_shared(g, W, num_layers, fanouts, &need_drain);
   if (rc != GG_OK) return rc;
   if (need_drain) {
+    // growing frees and reallocates scratch the pipeline threads are using (and the miss buffers
+    // already handed out in gg_batch_out): only with no window live.  Waiting here instead could
+    // deadlock -- a queued window's phase B may itself be waiting for the caller to release the
+    // window that holds its cache buffer.
+    for (int s = 0; s < g->n_win; ++s)
+      if (g->win[s].live)
+        return fail(GG_ERR_STATE, "window %lld needs larger shared scratch (bigger W or fanouts) than any window staged "
+                    "so far: release every live window first (window %lld is live)", (long long)window_id, (long long)g->win[s].id);
     {
       std::unique_lock<std::mutex> l(g->mu);
       g->cv_done.wait(l, [&] { return g->busy == 0; });
@@ -1251,7 +1296,7 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   return GG_OK;
 }
 
-gg_status gg_window_release(gg_graph* g, int64_t window_id) {
+gg_status gg_window_release(gg_graph* g, int64_t window_id, void* cuda_stream) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
   Window* w = find_window(g, window_id);
   if (!w) return fail(GG_ERR_STATE, "window %lld is not live", (long long)window_id);
@@ -1264,6 +1309,14 @@ gg_status gg_window_release(gg_graph* g, int64_t window_id) {
         if (&g->win[s] != w && g->win[s].live && g->win[s].seq + (uint64_t)g->n_cs == w->seq) blocked = true;
     if (blocked) return fail(GG_ERR_STATE, "release the older live window first");
     g->cv_done.wait(l, [&] { return w->enqueued; });
+  }
+  // Everything the caller enqueued on `cuda_stream` so far may still read the window's blocks and
+  // N_b (a consumer step behind the last gather, a device-to-host copy): the arena's next tenant
+  // is sampled only behind this point of that stream.
+  CU(cudaEventRecord(w->consumer_done, (cudaStream_t)cuda_stream));
+  {
+    std::lock_guard<std::mutex> l(g->mu);
+    w->consumer_recorded = true;
     w->live = false;
   }
   g->cv_done.notify_all();

@@ -193,7 +193,7 @@ void launch_seed_init(cudaStream_t st, const FrontierBufs& F, const int32_t* see
                       const BatchOffsets& seed_off, int W, int32_t* nodes, int64_t node_pitch,
                       uint32_t* cnt8, int32_t* n_front0, int32_t* wtile_sums, int32_t* totals) {
   const int S = seed_off.v[W];
-  const int g = grid_for(S, 256, 148 * 8);
+  const int g = grid_for(S, 256, sm_count() * 8);
   count_launches(4);
   k_seed_init<<<g, 256, 0, st>>>(seeds_dev, seed_off, W, nodes, node_pitch, F.seen, F.newbits,
                                  F.word_pitch, cnt8, n_front0);
@@ -218,7 +218,7 @@ void launch_frontier_hop(cudaStream_t st, const FrontierBufs& F, int hop, int W,
   const int g = hop + 1;
   uint32_t* nb = F.newbits + g * F.gen_pitch;
   int32_t* wp = F.wprefix + g * F.gen_pitch;
-  const int ge = grid_for(max_edges, 256, 148 * 16);
+  const int ge = grid_for(max_edges, 256, sm_count() * 16);
   count_launches(4);
   k_mark<<<ge, 256, 0, st>>>(src_global, edge_off, W, F.seen, nb, F.word_pitch);
   dim3 wg(F.n_wtiles, W);
@@ -236,7 +236,7 @@ void launch_frontier_hop(cudaStream_t st, const FrontierBufs& F, int hop, int W,
 
 void launch_bitmap_clear(cudaStream_t st, const FrontierBufs& F, const int32_t* nodes,
                          int64_t node_pitch, const int32_t* n_final, int max_n, int W, int n_gen) {
-  dim3 g(grid_for(max_n, 256, 148 * 4), W);
+  dim3 g(grid_for(max_n, 256, sm_count() * 4), W);
   count_launches(1);
   k_bitmap_clear<<<g, 256, 0, st>>>(nodes, node_pitch, n_final, W, n_gen, F.seen, F.newbits,
                                     F.gen_pitch, F.word_pitch);

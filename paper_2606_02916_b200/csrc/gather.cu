@@ -361,7 +361,7 @@ void launch_miss_path(cudaStream_t st, const GatherLaunch& G) {
     }
     v2 = ok16 ? 16 : (ok8 ? 8 : 4);
   }
-  const int grid = 148 * 4;
+  const int grid = sm_count() * 4;
   if (v2 == 16) k_rows<16, 1><<<grid, kThreads, 0, st>>>(Rw);
   else if (v2 == 8) k_rows<8, 1><<<grid, kThreads, 0, st>>>(Rw);
   else k_rows<4, 1><<<grid, kThreads, 0, st>>>(Rw);
@@ -376,7 +376,7 @@ void launch_rows_from_list(cudaStream_t st, const int32_t* src_idx, int n, const
   A.dst_base = dst_base; A.dst_row0 = dst_row0; A.dst_stride = dst_stride; A.rb = rb;
   const int vec = pick_vec(rb, src_base, dst_base, src_stride, dst_stride);
   int grid = (n + kRows - 1) / kRows;
-  if (grid > 148 * 8) grid = 148 * 8;
+  if (grid > sm_count() * 8) grid = sm_count() * 8;
   if (vec == 16) k_rows<16, 0><<<grid, kThreads, 0, st>>>(A);
   else if (vec == 8) k_rows<8, 0><<<grid, kThreads, 0, st>>>(A);
   else k_rows<4, 0><<<grid, kThreads, 0, st>>>(A);
@@ -385,7 +385,7 @@ void launch_rows_from_list(cudaStream_t st, const int32_t* src_idx, int n, const
 
 void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const StorePtrs& store,
                             const OwnerRanges& R, uint8_t* dst_base, int64_t dst_row0,
-                            int64_t dst_stride, int rb) {
+                            int64_t dst_stride, int rb, bool over_link) {
   if (n <= 0) return;
   RowsArgs A = {};
   A.n = n; A.src_idx = ids; A.store = store; A.R = R;
@@ -402,7 +402,8 @@ void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const St
   // the sampler (measured, products W=16: 12 / 16 / 24 / 32 / 1184 CTAs -> 3903 / 3657 / 3340 /
   // 3184 / 2607 mini-batches/s).
   constexpr int kPullCtas = 12;
-  if (grid > kPullCtas) grid = kPullCtas;
+  if (over_link) grid = grid > kPullCtas ? kPullCtas : grid;
+  else if (grid > sm_count() * 8) grid = sm_count() * 8;
   if (ok16) k_rows<16, 1><<<grid, kThreads, 0, st>>>(A);
   else if (ok8) k_rows<8, 1><<<grid, kThreads, 0, st>>>(A);
   else k_rows<4, 1><<<grid, kThreads, 0, st>>>(A);

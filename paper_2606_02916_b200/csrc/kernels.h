@@ -9,6 +9,9 @@ namespace gg {
 extern std::atomic<unsigned long long> g_launches;  // kernels launched by this library
 inline void count_launches(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 
+// SMs of the current device (cached per device; launch grids are sized in multiples of it)
+int sm_count();
+
 constexpr int kWordThreads = 256;
 constexpr int kWordTile = 2048;  // 32-bit words per CTA tile in the bitmap / counter passes
 
@@ -103,9 +106,11 @@ void launch_miss_path(cudaStream_t st, const GatherLaunch& G);   // a-8: compact
 void launch_rows_from_list(cudaStream_t st, const int32_t* src_idx, int n, const uint8_t* src_base,
                            int64_t src_stride, uint8_t* dst_base, int64_t dst_row0, int64_t dst_stride,
                            int rb);
+// over_link: the rows come from pinned host memory over PCIe (a dozen CTAs saturate it); false:
+// the owner's store is device memory and the copy takes the full grid
 void launch_rows_from_store(cudaStream_t st, const int32_t* ids, int n, const StorePtrs& store,
                             const OwnerRanges& R, uint8_t* dst_base, int64_t dst_row0,
-                            int64_t dst_stride, int rb);
+                            int64_t dst_stride, int rb, bool over_link = true);
 
 // NEXT-1 trace simulator (simulate.cu)
 void launch_count_db(cudaStream_t st, const int32_t* db_nodes, int64_t begin, int64_t end, uint32_t* cnt8);

@@ -358,15 +358,16 @@ __global__ void __launch_bounds__(256) k_sage_wreduce(const float* __restrict__ 
   }
 }
 
-constexpr int kWgMaxGrid = 148 * 4;
+constexpr int kWgMaxGrid = 1024;   // cap on the wgrad grid (sizes the per-CTA partial-sum buffer); the launch takes 4 CTAs per SM
 template <bool RELU>
 static void launch_wgrad(cudaStream_t st, const float* h_in, const float* agg, const float* h_out, const float* d_out,
                          int n_dst, int din, int dout, float* part, float* grads_layer) {
   // few rows: smaller tiles so that every SM gets one (the tile loop is sequential per CTA)
   int tile_rows = kWgRows;
-  while (tile_rows > 8 && (n_dst + tile_rows - 1) / tile_rows < 148 * 2) tile_rows >>= 1;
+  while (tile_rows > 8 && (n_dst + tile_rows - 1) / tile_rows < sm_count() * 2) tile_rows >>= 1;
   int grid = (n_dst + tile_rows - 1) / tile_rows;
-  grid = grid < 1 ? 1 : (grid > kWgMaxGrid ? kWgMaxGrid : grid);
+  const int gmax = std::min(kWgMaxGrid, sm_count() * 4);
+  grid = grid < 1 ? 1 : (grid > gmax ? gmax : grid);
   if (dout <= 16) k_sage_wgrad<RELU, 8><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
   else if (dout <= 48) k_sage_wgrad<RELU, 24><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
   else k_sage_wgrad<RELU, 32><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
@@ -516,7 +517,8 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     cudaFuncSetAttribute(k_sage_bwd<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     attr_set = true;
   }
-  auto grid_for = [](int n) { int g = (n + kSageWarps - 1) / kSageWarps; return g < 1 ? 1 : (g > 148 * 8 ? 148 * 8 : g); };
+  const int gcap = sm_count() * 8;
+  auto grid_for = [gcap](int n) { int g = (n + kSageWarps - 1) / kSageWarps; return g < 1 ? 1 : (g > gcap ? gcap : g); };
   // forward
   const float* h = (const float*)batch->features;
   for (int l = 0; l < L; ++l) {

@@ -707,9 +707,9 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
     }
     int per_sm = (int)((220 * 1024) / (smem + 1024));
     per_sm = per_sm < 1 ? 1 : (per_sm > 12 ? 12 : per_sm);
-    k_select_thread<<<148 * per_sm, kTThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
+    k_select_thread<<<sm_count() * per_sm, kTThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
   }
-  k_select_warp<<<148 * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
+  k_select_warp<<<sm_count() * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
 }
 
 }  // namespace gg

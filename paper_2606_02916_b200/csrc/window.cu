@@ -18,6 +18,19 @@ namespace gg {
 
 std::atomic<unsigned long long> g_launches{0};
 
+int sm_count() {
+  static int cached[64] = {0};
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64) dev = 0;
+  if (!cached[dev]) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    cached[dev] = n;
+  }
+  return cached[dev];
+}
+
 template <typename T>
 __global__ void __launch_bounds__(1024) k_row_scan(T* __restrict__ tiles, int n, T* __restrict__ total) {
   __shared__ T sm[33];
@@ -274,7 +287,7 @@ void launch_delta_split(cudaStream_t st, const int32_t* hot, int n_hot, const Ow
 void launch_slots_clear(cudaStream_t st, const int32_t* ids, int n, int32_t* slot_map) {
   if (n <= 0) return;
   int g = (n + 255) / 256;
-  if (g > 148 * 8) g = 148 * 8;
+  if (g > sm_count() * 8) g = sm_count() * 8;
   k_slots_clear<<<g, 256, 0, st>>>(ids, n, slot_map);
   count_launches(1);
 }
@@ -298,7 +311,7 @@ void launch_copy_words(cudaStream_t st, void* dst, const void* src, int64_t n_wo
 void launch_fill_i32(cudaStream_t st, int32_t* p, int64_t n, int32_t v) {
   if (n <= 0) return;
   int64_t g = (n + 255) / 256;
-  if (g > 148 * 16) g = 148 * 16;
+  if (g > sm_count() * 16) g = sm_count() * 16;
   k_fill_i32<<<(int)g, 256, 0, st>>>(p, n, v);
   count_launches(1);
 }

@@ -21,12 +21,13 @@ from .binding import Graph
 
 def graph_from_workload(w, n_hot: int = -1, carry_over: int = 1, max_window: int = 32,
                         staging_mode: int = 0, max_cache_rows: int = 0, host_threads: int = 0,
-                        max_batch: Optional[int] = None, max_live_windows: int = 0, cache_buffers: int = 0) -> Graph:
+                        max_batch: Optional[int] = None, max_live_windows: int = 0, cache_buffers: int = 0,
+                        max_input_nodes: int = 0) -> Graph:
     """Builds a gg_graph over an inputs.Workload whose graph and local features are on a CUDA device."""
     mb = max_batch or max(len(b) for b in w.batches)
     return Graph(w.indptr, w.indices, w.part_offsets, w.local_part, w.feat_parts, seed=w.seed,
                  n_hot=n_hot, carry_over=carry_over, max_layers=len(w.fanouts), max_window=max_window,
-                 max_batch=mb, max_cache_rows=max_cache_rows, staging_mode=staging_mode,
+                 max_batch=mb, max_cache_rows=max_cache_rows, max_input_nodes=max_input_nodes, staging_mode=staging_mode,
                  host_threads=host_threads, max_live_windows=max_live_windows, cache_buffers=cache_buffers)
 
 
@@ -61,7 +62,7 @@ def run_epoch(g: Graph, batches: Sequence[np.ndarray], fanouts: Sequence[int], W
                 on_batch(k, j, bi, r)
         if on_window is not None:
             on_window(wid + k, win)
-        g.window_release(wid + k)
+        g.window_release(wid + k, stream)      # the arena is recycled only behind on_batch's work on `stream`
     return n
 
 

@@ -18,7 +18,7 @@ def oracle_parts(w):
 
 def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, max_cache_rows=0,
                 check_features=True, cache_samples=64, host_threads=0, oracle_threads=1, host_graph=None,
-                parts=None, cache_buffers=0, lookahead=2):
+                parts=None, cache_buffers=0, lookahead=2, graph=None, first_window_id=0):
     """Runs one epoch on the GPU and on the oracle; asserts bit-exact agreement everywhere.
     Returns a small summary dict."""
     batches = w.batches if max_batches is None else w.batches[:max_batches]
@@ -33,10 +33,12 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
     if parts is None and check_features:
         parts = oracle_parts(w)
 
-    g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=carry_over, max_window=max(W, 1),
-                               staging_mode=staging_mode, max_cache_rows=max_cache_rows,
-                               host_threads=host_threads, cache_buffers=cache_buffers,
-                               max_live_windows=lookahead + 1)
+    # graph: an existing handle (its cache must be empty: the oracle starts from C_0 = {}); it is
+    # left open for the caller
+    g = graph if graph is not None else ep.graph_from_workload(
+        w, n_hot=n_hot, carry_over=carry_over, max_window=max(W, 1), staging_mode=staging_mode,
+        max_cache_rows=max_cache_rows, host_threads=host_threads, cache_buffers=cache_buffers,
+        max_live_windows=lookahead + 1)
     obatches = {}
     owin = {}
     stats = dict(batches=0, misses=0, windows=0, rows=0, edges=0)
@@ -87,7 +89,7 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
         stats["rows"] += r["n_input"]
 
     def on_window(wid, win):
-        k = wid
+        k = wid - first_window_id
         ow = owin[k]
         t = g.trace(wid, len(win))
         assert np.array_equal(g.window_export(wid, "uniq"), ow.uniq), "U_k"
@@ -113,7 +115,9 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
             assert np.array_equal(got, want), "cache rows"
         stats["windows"] += 1
 
-    ep.run_epoch(g, batches, w.fanouts, W, features, on_batch=on_batch, on_window=on_window, lookahead=lookahead)
+    ep.run_epoch(g, batches, w.fanouts, W, features, on_batch=on_batch, on_window=on_window, lookahead=lookahead,
+                 first_window_id=first_window_id)
     torch.cuda.synchronize()
-    g.close()
+    if graph is None:
+        g.close()
     return stats

@@ -234,8 +234,13 @@ def _stress(w, dev, n_cfg, epochs, max_window, ws, seed, budgets=(-1, 0, 3000, 2
     feats = torch.empty(min(w.num_nodes, 600_000), w.dim, dtype=w.dtype, device=dev)
 
     def on_batch(k, j, bi, r):
-        x = r["features"].contiguous().view(torch.int32)
-        h = (int(x.to(torch.int64).sum().item()), int(r["input_nodes"].to(torch.int64).sum().item()), r["n_input"])
+        # position-weighted sums (mod 2^64, wrapping int64): a permutation of the rows or of the
+        # words inside a row, or two compensating errors, change the value
+        x = r["features"].contiguous().view(torch.int32).reshape(-1).to(torch.int64)
+        wx = torch.arange(1, x.numel() + 1, dtype=torch.int64, device=x.device) * 0x9E3779B1 + 0x7F4A7C15
+        nd = r["input_nodes"].to(torch.int64)
+        wn = torch.arange(1, nd.numel() + 1, dtype=torch.int64, device=nd.device) * 0x85EBCA6B + 0xC2B2AE35
+        h = (int((x * wx).sum().item()), int((nd * wn).sum().item()), r["n_input"])
         if bi in ref:
             assert ref[bi] == h, "batch %d differs from the first epoch" % bi
         else:
@@ -318,6 +323,62 @@ def test_error_codes(workload, dev):
     with pytest.raises(binding.GreenGNNError) as e:
         binding.Graph(w.indptr.cpu(), w.indices.cpu(), w.part_offsets, 0, w.feat_parts, seed=1)
     assert e.value.status == binding.GG_ERR_INVALID_ARG
+
+
+def test_frontier_overflow_is_reported_and_leaves_the_graph_clean(workload, dev):
+    """max_input_nodes too small for a full batch: the window reports GG_ERR_CAPACITY, holds no
+    output, and the NEXT windows on the same graph are bit-exact (the per-batch bitmaps and the
+    packed access counters the failed window had touched are reset)."""
+    import dataclasses
+    from paper_2606_02916_b200 import binding, epoch as ep
+    w0 = workload("small", dev)
+    g = ep.graph_from_workload(w0, n_hot=-1, max_window=4, max_input_nodes=3000)
+    for attempt in range(2):
+        g.window_stage(900 + attempt, 0, w0.batches[:3], w0.fanouts)      # 1024 seeds -> tens of thousands of nodes
+        with pytest.raises(binding.GreenGNNError) as e:
+            g.batch_info(900 + attempt, 0)
+        assert e.value.status == binding.GG_ERR_CAPACITY
+        g.window_release(900 + attempt)
+        # small batches fit under the cap: same graph handle, checked against the oracle
+        small = [w0.batches[0][:3], w0.batches[1][:2], w0.batches[2][:4], w0.batches[3][:1], w0.batches[4][:3]]
+        w = dataclasses.replace(w0, batches=small)
+        s = pu.check_epoch(w, W=2, n_hot=-1, graph=g, first_window_id=100 * attempt)
+        assert s["batches"] == 5
+        g.cache_reset()
+    g.close()
+
+
+def test_growing_shared_scratch_needs_no_live_window(workload, dev):
+    """A window with bigger fanouts than any before needs larger shared scratch: STATE while other
+    windows are live (blocking there could deadlock), fine once they are released."""
+    from paper_2606_02916_b200 import binding, epoch as ep
+    w = workload("small", dev)
+    g = ep.graph_from_workload(w, max_window=4, max_live_windows=4)
+    g.window_stage(0, 0, w.batches[:2], [3, 2])
+    with pytest.raises(binding.GreenGNNError) as e:
+        g.window_stage(1, 2, w.batches[2:4], [15, 10])
+    assert e.value.status == binding.GG_ERR_STATE
+    assert g.batch_info(0, 0)["n_input"] > 0
+    g.window_release(0)
+    g.window_stage(1, 2, w.batches[2:4], [15, 10])
+    assert g.batch_info(1, 1)["n_input"] > 0
+    g.window_release(1)
+    g.close()
+
+
+def test_remote_owner_in_device_memory_mode0(workload, dev):
+    """staging_mode 0 with an owner whose store is DEVICE memory (the stand-in for a peer GPU's HBM):
+    host threads cannot pack it, the library serves that owner with the pull kernel; results are
+    the oracle's."""
+    import dataclasses
+    w0 = workload("small", dev)
+    parts = list(w0.feat_parts)
+    parts[2] = parts[2].to(dev)                      # owner 2 on the device, owners 1 and 3 pinned
+    w = dataclasses.replace(w0, feat_parts=parts)
+    pu.check_epoch(w, W=4, n_hot=-1, staging_mode=0)
+    pu.check_epoch(w, W=2, n_hot=7500, staging_mode=0)
+    parts = [p.to(dev) for p in w0.feat_parts]       # every owner on the device
+    pu.check_epoch(dataclasses.replace(w0, feat_parts=parts), W=4, n_hot=7500, staging_mode=0)
 
 
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times ---------------------

@@ -75,6 +75,46 @@ def test_products_mini_three_layers(workload, dev):
     run(workload("products_mini", dev), dev, hidden=16, classes=47, W=4, steps=3, lr=0.03)
 
 
+def test_consumer_without_host_sync_matches_synced_run(workload, dev):
+    """gg_window_release(stream) orders the arena's reuse behind the consumer's work: a run that
+    never synchronises the host between a batch's training step and the release (arenas =
+    lookahead + 1, so the sampler is free to overwrite the arena at once) must give the losses of
+    a run that synchronises after every step.  Before the release took a stream, window k+n's
+    sampling raced the last steps of window k."""
+    from paper_2606_02916_b200 import binding, epoch as ep
+    w = workload("products_mini", dev)
+    L = len(w.fanouts)
+    dims = [w.dim] + [16] * (L - 1) + [47]
+    stream = torch.cuda.Stream(dev)
+    labels = torch.from_numpy(np.random.default_rng(3).integers(0, 47, (len(w.batches), 512)).astype(np.int32)).to(dev)
+    runs = []
+    for sync in (True, False, False):
+        model = binding.Sage(init_params(dims, 5), dev)
+        g = ep.graph_from_workload(w, max_window=2, max_live_windows=3)
+        feats = torch.empty(w.num_nodes, w.dim, dtype=w.dtype, device=dev)
+        losses = []
+
+        def on_batch(k, j, bi, r):
+            n_seed = r["blocks"][0]["n_dst"]
+            loss = model.step(r, labels[bi, :n_seed].contiguous(), 0.03, stream)
+            with torch.cuda.stream(stream):
+                losses.append(loss.clone())
+            if sync:
+                torch.cuda.synchronize()
+
+        with torch.cuda.stream(stream):
+            for e in range(2):
+                ep.run_epoch(g, w.batches, w.fanouts, 2, feats, on_batch=on_batch, stream=stream, lookahead=2,
+                             first_window_id=1000 * e)
+        torch.cuda.synchronize()
+        runs.append(np.array([float(x.cpu()[0]) for x in losses]))
+        model.close()
+        g.close()
+    assert len(runs[0]) == 2 * len(w.batches)
+    for r in runs[1:]:
+        assert np.allclose(r, runs[0], rtol=2e-4, atol=1e-6), float(np.abs(r - runs[0]).max())
+
+
 def test_sage_errors(workload, dev):
     from paper_2606_02916_b200 import binding
     with pytest.raises(binding.GreenGNNError):
