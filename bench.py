@@ -47,6 +47,9 @@ def parse_args():
     ap.add_argument("--no-clocks", action="store_true", help="debug: do not poll nvidia-smi during the timed region")
     ap.add_argument("--no-profile", action="store_true", help="debug: time the headline without the per-kernel event pairs")
     ap.add_argument("--cpu-sample-batches", type=int, default=4)
+    ap.add_argument("--configs", default="products,dense,large",
+                    help="workloads of the `configs` grid (BASELINE.json:configs); '' switches the grid off")
+    ap.add_argument("--configs-budget-s", type=float, default=420.0, help="wall-clock budget of the `configs` grid")
     return ap.parse_args()
 
 
@@ -70,15 +73,16 @@ def ncu_traffic(name):
     return None
 
 
-# Issue slots the key loop of k_select_warp / k_select_thread spends per key (84 SASS
-# instructions per 4 keys: DESIGN.md Sec. 6); the ALU roofline is one warp instruction per clock
-# per SM sub-partition.
-KEY_ISSUE_SLOTS = 21.0
-SM_COUNT, SMSP_PER_SM = 148, 4
+# The sampler's roofline is the key-only micro-kernel measured in the same run (gg_key_peak).  Two
+# derived figures are kept beside it as notes: the issue-slot bound of the product loop (84 SASS
+# instructions per 4 keys = 21 slots per key) and of the hash alone (16 slots per key), both at one
+# warp instruction per clock per SM sub-partition -- a rate this integer mix does not reach.
+KEY_ISSUE_SLOTS, HASH_ISSUE_SLOTS = 21.0, 16.0
+SMSP_PER_SM = 4
 
 
-def alu_peak_gkeys(sm_mhz):
-    return SM_COUNT * SMSP_PER_SM * 32 * sm_mhz * 1e6 / KEY_ISSUE_SLOTS / 1e9
+def derived_alu_peak_gkeys(sm_mhz, sm_count, slots):
+    return sm_count * SMSP_PER_SM * 32 * sm_mhz * 1e6 / slots / 1e9
 
 
 class EnergyMeter:
@@ -161,31 +165,46 @@ def run_reference(args):
     feat = w.host_features()
     po = w.part_offsets
     parts = [np.ascontiguousarray(feat[po[m]:po[m + 1]]) for m in range(len(po) - 1)]
-    S = 1                                   # mini-batches per step (bounded sample of the epoch)
+    # one step = one window of W mini-batches of the epoch (a bounded sample of it: the oracle needs
+    # seconds per mini-batch), windows taken in epoch order with the cache state carried between them;
+    # the batches of a window are sampled and gathered side by side on the host cores, the oracle
+    # itself unchanged
+    from concurrent.futures import ThreadPoolExecutor
+    from paper_2606_02916_b200 import epoch as ep
+    W = args.window
+    wins = ep.windows_of(len(w.batches), W)
+    cores = os.cpu_count() or 1
     st = ggo.State(g.n, po, 0, args.n_hot, 1)
+    done = [0]
 
-    def step(i):
-        bs = [ggo.Batch(g, w.batches[(i * S + j) % len(w.batches)], w.fanouts, w.seed, (i * S + j) % len(w.batches))
-              for j in range(S)]
+    def step(i, ex):
+        win = wins[i % len(wins)]
+        if i % len(wins) == 0:
+            st.reset()
+        bs = list(ex.map(lambda j: ggo.Batch(g, w.batches[j], w.fanouts, w.seed, j), win))
         st.run_window(bs)
-        for b in bs:
-            ggo.gather(b.nodes, po, parts, w.row_bytes)
+        list(ex.map(lambda b: ggo.gather(b.nodes, po, parts, w.row_bytes), bs))
+        done[0] += len(bs)
 
-    for i in range(args.warmup):
-        step(i)
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        step(args.warmup + i)
-    dt = time.perf_counter() - t0
-    v = args.steps * S / dt
-    sample = "%d mini-batch(es) per step as W=%d windows of the same workload (sample + window + gather)" % (S, S)
+    with ThreadPoolExecutor(cores) as ex:
+        for i in range(args.warmup):
+            step(i, ex)
+        done[0] = 0
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            step(args.warmup + i, ex)
+        dt = time.perf_counter() - t0
+    v = done[0] / dt
+    sample = ("one W=%d window of the epoch per step (%d mini-batches in %d steps), sample + window + gather, "
+              "batches side by side on %d threads" % (W, done[0], args.steps, min(cores, W)))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/int32/uint64",
         "data": "synthetic",
-        "config": {"workload": workload_name(args, w), "step": sample},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot, "step": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": min(cores, W), "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model(), "host_cores": cores},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -277,6 +296,7 @@ def run_ours(args):
     torch.cuda.set_stream(stream)
     energy = EnergyMeter(local_rank)
     link_peak = host_link_peak(dev)
+    key_peak_gkeys = binding.key_peak(8, 65536, 5) / 1e9     # measured ALU roofline of a-1, GPU otherwise idle
 
     # size the output buffer from the first window (|N_b| varies little between batches)
     g.window_stage(10 ** 9, 0, batches[:min(W, 4)], w.fanouts)
@@ -455,43 +475,66 @@ def run_ours(args):
         errors['simulator'] = repr(exc)
         g = recover_graph(g)
 
-    # ---- BASELINE.json configs[2]: batch in {1024, 2048, 4096} at the same W -------------------
-    vs_batch = {}
-    try:
-        if not args.no_sweep and world == 1 and args.config == "products":
-            vs_batch[str(args.batch)] = {"mini_batches_per_s": value, "seeds_per_s": value * args.batch}
-            all_seeds = np.concatenate(batches)
-            for Bx in (2048, 4096):
-                if Bx == args.batch:
-                    continue
-                bx = [all_seeds[i:i + Bx] for i in range(0, len(all_seeds), Bx)]
-                g.close()
-                g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=W, staging_mode=args.staging_mode,
-                                           max_live_windows=args.lookahead + 1, max_batch=Bx)
-                fx = torch.empty(int(cap_rows * Bx / args.batch) + 1024, w.dim, dtype=w.dtype, device=dev)
-                def ep_b():
-                    ep.run_epoch(g, bx, w.fanouts, W, fx, stream=stream, first_window_id=0, lookahead=LA)
-                    torch.cuda.synchronize(dev)
-                    g.cache_reset()
-                n_warm = max(2, -(-(LA + 1) // max(1, -(-len(bx) // W))) + 1)      # every window arena used at least once
-                for _ in range(n_warm):
-                    ep_b()
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(stream)
-                for _ in range(3):
-                    ep_b()
-                b.record(stream)
-                torch.cuda.synchronize(dev)
-                v = 3 * len(bx) / (a.elapsed_time(b) * 1e-3)
-                vs_batch[str(Bx)] = {"mini_batches_per_s": v, "seeds_per_s": v * Bx, "mini_batches_per_epoch": len(bx)}
-                del fx
-            g.close()
-            g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
-                                       staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
-                                       host_threads=args.host_threads)
-    except Exception as exc:      # an optional leg must not cost the headline line
-        errors['vs_batch'] = repr(exc)
-        g = recover_graph(g)
+    # ---- BASELINE.json:configs, every sweep, each point with its per-stage roofline fractions ----
+    vs_batch, configs, simulator_budgeted = {}, None, None
+    if not args.no_sweep and world == 1 and args.config == "products" and args.configs:
+        g.close()
+        ctx = dict(dev=dev, stream=stream, LA=LA, hbm_peak=measured_peaks()[0], link_peak=link_peak, key_peak=key_peak_gkeys,
+                   energy=energy, args=args, feats=None, edge_cut_products=None)
+        try:
+            ctx["edge_cut_products"] = edge_cut(w, dev)
+        except Exception as exc:
+            errors["edge_cut"] = repr(exc)
+        configs = configs_grid(ctx, w, batches, errors, args.configs_budget_s)
+        try:
+            for pt in configs.get("products_batch_x_W", {}).get("points", []):
+                if pt["W"] == W:
+                    vs_batch[str(pt["batch"])] = {"mini_batches_per_s": pt["mini_batches_per_s"],
+                                                  "seeds_per_s": pt["mini_batches_per_s"] * pt["batch"],
+                                                  "mini_batches_per_epoch": pt["mini_batches_per_epoch"]}
+        except Exception as exc:
+            errors["vs_batch"] = repr(exc)
+        # NEXT-1 / NEXT-3 where they can fail: the budgeted series (misses > 0, the hit ratio varies with
+        # W, the hot set goes stale), predicted W* against the measured argmin
+        try:
+            pts = configs["products_budget_10pct_x_W"]["points"]
+            n_hot_b = configs["products_budget_10pct_x_W"]["n_hot"]
+            from paper_2606_02916_b200 import profiler
+            cands = [p_["W"] for p_ in pts]
+            gb = ep.graph_from_workload(w, n_hot=n_hot_b, carry_over=1, max_window=max(cands), staging_mode=args.staging_mode,
+                                        max_live_windows=LA + 1, host_threads=args.host_threads)
+            try:
+                model = profiler.measure_energy_model(dev, w.row_bytes, P, local_part=rank % P)
+                model.pop("probes"), model.pop("p_active")
+                sim = gb.simulate(batches, w.fanouts, cands, model)
+            finally:
+                gb.close()
+            pred = [r["e_phy"] for r in sim["results"]]
+            meas_j = [p_["J_per_epoch"] for p_ in pts]
+            meas_t = [p_["ms_per_epoch"] for p_ in pts]
+            simulator_budgeted = {
+                "candidates": cands, "n_hot": n_hot_b, "W_star_predicted": sim["best"], "e_phy_J": pred,
+                "measured_J_per_epoch": meas_j, "measured_ms_per_epoch": meas_t,
+                "z": [{k: r[k] for k in ("rebuild_events", "miss_events", "t_stall", "hit_ratio", "rebuild_rows", "miss_rows")}
+                      for r in sim["results"]],
+                "kendall_tau_vs_measured_ms": kendall_tau(pred, meas_t),
+                "note": "energy per epoch = NVML counter over 5 timed epochs per W; Table III's metrics (PAPER.md:343-345): "
+                        "rank correlation, top-1 hit, and the measured penalty of running the simulator's pick"}
+            if all(x is not None for x in meas_j):
+                bi = int(np.argmin(meas_j))
+                simulator_budgeted.update({
+                    "W_star_measured_J": cands[bi], "top1_hit": cands[bi] == sim["best"],
+                    "penalty_of_predicted_W_J_frac": meas_j[cands.index(sim["best"])] / meas_j[bi] - 1.0,
+                    "kendall_tau_vs_measured_J": kendall_tau(pred, meas_j),
+                    "calibration": calibrate(sim["results"], meas_j)})
+            bt = int(np.argmin(meas_t))
+            simulator_budgeted.update({"W_star_measured_ms": cands[bt],
+                                       "penalty_of_predicted_W_ms_frac": meas_t[cands.index(sim["best"])] / meas_t[bt] - 1.0})
+        except Exception as exc:
+            errors["simulator_budgeted"] = repr(exc)
+        g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
+                                   staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
+                                   host_threads=args.host_threads)
 
     # ---- variant: epochs back to back with the cache carried over (reading S15: the cache
     # persists across epochs; the trace repeats), no reset and no drain between
@@ -601,16 +644,24 @@ def run_ours(args):
                    "note": "live: shares the SMs with the sampler on the side stream; alone it runs at the ncu time in profiles/"}
     ps = main["prof"]["sample"]
     sm_mhz = (main["clocks"] or {}).get("sm_max_mhz") or 1965.0
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     keys = main["sampler"]["keys"]
     gk = keys / (ps["ms"] * 1e-3) / 1e9 if ps["ms"] > 0 else 0.0
-    gk_peak = alu_peak_gkeys(sm_mhz)
-    roof = {"bound": "alu", "kernel": "a-1 sampling (k_sample_count/plan + k_select_thread + k_select_warp per hop)",
+    gk_peak = key_peak_gkeys
+    roof = {"bound": "alu", "kernel": "a-1 sampling (k_sample_count/plan + the selection kernels of every hop)",
             "achieved": gk, "peak": gk_peak, "unit": "Gkey/s", "frac": gk / gk_peak,
-            "traffic": ncu_traffic("r01_sample_ncu_summary.txt"),
-            "peak_source": "derived: %d SMs x %d sub-partitions x 1 warp instruction/clk x 32 lanes x %.0f MHz / %.0f issue "
-                           "slots per key (DESIGN.md Sec. 6)" % (SM_COUNT, SMSP_PER_SM, sm_mhz, KEY_ISSUE_SLOTS),
+            "traffic": ncu_traffic("r02_sample_ncu_summary.txt"),
+            "traffic_note": "dram read+write bytes of all a-1 kernels of one W=16 window (every hop) / 3 hop regions: the same "
+                            "launches avg_launch_us averages; DRAM traffic is ~5x the algorithmic bytes on the last hop (32-byte "
+                            "sectors for scattered 4-byte neighbor ids) and is not the binding resource",
+            "peak_source": "measured: gg_key_peak, key-only micro-kernel (fmix high word per lane from a register-resident state, "
+                           "no stores, no row logic), 8 CTAs of 256 threads per SM, CUDA events, same run, GPU otherwise idle",
+            "derived_peaks_Gkey/s": {"product_loop_21_issue_slots": derived_alu_peak_gkeys(sm_mhz, sm_count, KEY_ISSUE_SLOTS),
+                                     "hash_only_16_issue_slots": derived_alu_peak_gkeys(sm_mhz, sm_count, HASH_ISSUE_SLOTS),
+                                     "note": "one warp instruction per clock per sub-partition; notes only, not the denominator"},
             "launches": ps["regions"], "avg_launch_us": 1e3 * ps["ms"] / max(ps["regions"], 1),
             "algorithmic_keys_per_launch": keys / max(ps["regions"], 1),
+            "algorithmic_bytes_GB/s": ps["bytes"] / (ps["ms"] * 1e-3) / 1e9 if ps["ms"] > 0 else None,
             "keyed_rows_per_step": main["sampler"]["rows"] / args.steps,
             "fallback_rows_per_step": main["sampler"]["fallbacks"] / args.steps,
             "share_of_step": ps["ms"] * 1e-3 / main["sec"]}
@@ -653,7 +704,8 @@ def run_ours(args):
         "epoch_ms": {"median": statistics.median(main["per_epoch_ms"]), "min": min(main["per_epoch_ms"]),
                      "max": max(main["per_epoch_ms"]), "note": "host clock around each epoch incl. its final synchronise and cache reset"},
         "roofline": roof, "roofline_gather": roof_gather, "kernels_alone": serial, "stages": stages, "vs_W": vs_w,
-        "J_per_epoch_vs_W": j_w, "vs_batch_at_W": vs_batch, "simulator": simulator, "variants": variants,
+        "J_per_epoch_vs_W": j_w, "vs_batch_at_W": vs_batch, "configs": configs, "simulator": simulator,
+        "simulator_budgeted": simulator_budgeted, "variants": variants,
         "errors": errors,
         "gpu_stall_ms_per_step": (main["prof"]["wait"]["ms"] / args.steps) if "wait" in main["prof"] else None,
         "energy": {"J_per_step": (main["joules"] / args.steps) if main["joules"] is not None else None,
@@ -670,6 +722,204 @@ def run_ours(args):
     }
     print(json.dumps(out))
     g.close()
+
+
+def edge_cut(w, dev):
+    """Measured fraction of CSR entries whose two endpoints lie in different owner ranges."""
+    po = torch.as_tensor(np.asarray(w.part_offsets[1:-1], dtype=np.int32), device=dev)
+    N, cut, step = w.num_nodes, 0, 1 << 22
+    for r0 in range(0, N, step):
+        r1 = min(N, r0 + step)
+        ip = w.indptr[r0:r1 + 1]
+        e0, e1 = int(ip[0]), int(ip[-1])
+        if e1 == e0:
+            continue
+        own_row = torch.bucketize(torch.arange(r0, r1, device=dev, dtype=torch.int32), po, right=True, out_int32=True)
+        own_e = torch.repeat_interleave(own_row.to(torch.int8), ip[1:] - ip[:-1])
+        own_n = torch.bucketize(w.indices[e0:e1], po, right=True, out_int32=True).to(torch.int8)
+        cut += int((own_e != own_n).sum())
+    return cut / max(1, w.indices.numel())
+
+
+def measure_point(ctx, w, batches, W, n_hot, K=2, warm=1, max_batch=None, g=None, max_window=32):
+    """One (workload, batch list, W, n_hot) point of the `configs` grid: `warm` untimed + K timed epochs
+    with the library's per-stage event pairs on (so the rates below are LIVE rates, all streams
+    running), then one traced epoch for the byte counts.  Returns the per-stage numbers with their
+    roofline fractions.  ctx: dict(dev, stream, LA, hbm_peak, link_peak, key_peak, energy, args)."""
+    from paper_2606_02916_b200 import epoch as ep, binding
+    dev, stream, LA, args = ctx["dev"], ctx["stream"], ctx["LA"], ctx["args"]
+    own = g is None
+    if own:
+        g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=1, max_window=max_window, staging_mode=args.staging_mode,
+                                   max_live_windows=LA + 1, host_threads=args.host_threads,
+                                   max_batch=max_batch or max(len(b) for b in batches))
+    n_b = len(batches)
+    try:
+        nb0 = min(W, 4, n_b)
+        g.window_stage(10 ** 9, 0, batches[:nb0], w.fanouts)
+        cap_rows = int(max(g.batch_info(10 ** 9, j)["n_input"] for j in range(nb0)) * 1.25) + 1024
+        g.window_release(10 ** 9)
+        g.cache_reset()
+        feats = ctx.get("feats")
+        if feats is None or feats.shape[0] < cap_rows or feats.shape[1] != w.dim or feats.dtype != w.dtype:
+            ctx["feats"] = None
+            feats = torch.empty(cap_rows, w.dim, dtype=w.dtype, device=dev)
+            ctx["feats"] = feats
+
+        def one_epoch(wid0, on_window=None):
+            ep.run_epoch(g, batches, w.fanouts, W, feats, stream=stream, first_window_id=wid0, lookahead=LA,
+                         on_window=on_window)
+            torch.cuda.synchronize(dev)
+            g.cache_reset()
+
+        for e in range(warm):
+            one_epoch(1000 * e)
+        g.profile_enable(True)
+        s0 = binding.sampler_stats()
+        mj0 = ctx["energy"].read_mj()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for e in range(K):
+            one_epoch(1000 * (warm + e))
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        mj1 = ctx["energy"].read_mj()
+        sec = a.elapsed_time(b) * 1e-3
+        prof = g.profile_get()
+        keys = binding.sampler_stats()["keys"] - s0["keys"]
+        g.profile_enable(False)
+        tr = dict(bulk=0, copies=0, n_in=0, local=0, hit=0, miss=0, hot=0, uniq_remote=0)
+
+        def on_window(wid, win):
+            t = g.trace(wid, len(win))
+            tr["bulk"] += sum(t["bulk_bytes"])
+            tr["copies"] += t["bulk_copies"]
+            tr["n_in"] += int(t["n_input"].sum())
+            tr["local"] += int(t["hit_local"].sum())
+            tr["hit"] += int(t["hit_cache"].sum())
+            tr["miss"] += int(t["miss"].sum())
+            tr["hot"] += t["n_hot"]
+            tr["uniq_remote"] += t["n_unique_remote"]
+
+        one_epoch(5 * 10 ** 6, on_window)
+    finally:
+        if own:
+            g.close()
+    rb = w.row_bytes
+
+    def rate(kind, per_byte=1.0):
+        v = prof[kind]
+        return (v["bytes"] * per_byte / (v["ms"] * 1e-3) / 1e9) if v["ms"] > 0 and v["bytes"] else None
+
+    gat, h2d, samp = rate("gather"), rate("stage_copy"), prof["sample"]
+    gk = keys / (samp["ms"] * 1e-3) / 1e9 if samp["ms"] > 0 else None
+    miss_link = rate("miss", 0.5)        # bytes = rows * 2 rb (link read + HBM write); the link carries rows * rb
+    remote = tr["n_in"] - tr["local"]
+    out = {
+        "W": W, "batch": max(len(x) for x in batches), "n_hot": n_hot, "mini_batches_per_epoch": n_b,
+        "mini_batches_per_s": K * n_b / sec, "ms_per_epoch": 1e3 * sec / K,
+        "gather_GB/s": gat, "gather_frac_of_hbm_peak": gat / ctx["hbm_peak"] if gat else None,
+        "gather_vec_bytes": 16 if rb % 16 == 0 else (8 if rb % 8 == 0 else 4),
+        "sample_Gkey/s": gk, "sample_frac_of_key_peak": gk / ctx["key_peak"] if gk else None,
+        "h2d_GB/s": h2d, "h2d_frac_of_link_peak": h2d / ctx["link_peak"] if h2d else None,
+        "host_link_MB_per_epoch": tr["bulk"] / 1e6, "bulk_copies_per_epoch": tr["copies"],
+        "miss_rows_per_epoch": tr["miss"], "miss_fill_link_GB/s": miss_link,
+        "miss_fill_frac_of_link_peak": miss_link / ctx["link_peak"] if miss_link else None,
+        "miss_ms_per_epoch": prof["miss"]["ms"] / K,
+        "cache_hit_ratio_of_remote_accesses": (tr["hit"] / remote) if remote else None,
+        "remote_frac_of_N_b": remote / max(tr["n_in"], 1),
+        "gpu_stall_ms_per_epoch": prof["wait"]["ms"] / K,
+        "J_per_epoch": ((mj1 - mj0) / 1e3 / K) if (mj0 is not None and mj1 is not None) else None,
+    }
+    return out
+
+
+def configs_grid(ctx, w_products, batches_products, errors, t_budget_s):
+    """BASELINE.json:configs, every sweep: products B x W (unlimited budget), products with the paper's
+    10 % budget x W (exercises the miss path, Alg. 1 l.13-14), dense W in {1,4,16}, large
+    W in {4,16}.  Every point: measure_point().  A leg that fails or would overrun the time budget is
+    recorded in `errors` and skipped; the headline line never depends on it."""
+    from paper_2606_02916_b200 import inputs, epoch as ep
+    dev, args = ctx["dev"], ctx["args"]
+    t_start = time.perf_counter()
+    out = {}
+
+    def left():
+        return t_budget_s - (time.perf_counter() - t_start)
+
+    # ---- products: batch x W, unlimited budget ------------------------------------------------
+    w = w_products
+    try:
+        all_seeds = np.concatenate(batches_products)
+        n_remote_nodes = w.num_nodes - int(w.part_offsets[w.local_part + 1] - w.part_offsets[w.local_part])
+        pts = []
+        for Bx in (1024, 2048, 4096):
+            bx = batches_products if Bx == args.batch else [all_seeds[i:i + Bx] for i in range(0, len(all_seeds), Bx)]
+            g = ep.graph_from_workload(w, n_hot=-1, carry_over=1, max_window=32, staging_mode=args.staging_mode,
+                                       max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, max_batch=Bx)
+            try:
+                for Wx in w.cfg["windows"]:
+                    pts.append(measure_point(ctx, w, bx, Wx, -1, K=2, warm=1, g=g))
+            finally:
+                g.close()
+        out["products_batch_x_W"] = {"edge_cut_measured": ctx["edge_cut_products"], "n_hot": "unlimited", "points": pts}
+    except Exception as exc:
+        errors["configs.products_batch_x_W"] = repr(exc)
+    # ---- products: the paper's 10 % budget -----------------------------------------------------
+    try:
+        n_hot = -(-n_remote_nodes // 10)
+        pts = []
+        g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=1, max_window=32, staging_mode=args.staging_mode,
+                                   max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, max_batch=args.batch)
+        try:
+            for Wx in w.cfg["windows"]:
+                pts.append(measure_point(ctx, w, batches_products, Wx, n_hot, K=5, warm=1, g=g))
+        finally:
+            g.close()
+        out["products_budget_10pct_x_W"] = {"n_hot": n_hot, "n_hot_rule": "ceil(0.10 x remote nodes) (PAPER.md:32)", "points": pts}
+    except Exception as exc:
+        errors["configs.products_budget_10pct_x_W"] = repr(exc)
+    ctx["feats"] = None
+    # ---- dense and large --------------------------------------------------------------------------
+    for name in ("dense", "large"):
+        if name not in args.configs.split(","):
+            continue
+        try:
+            if left() < (60 if name == "dense" else 150):
+                raise RuntimeError("skipped: %.0f s left of the bench's time budget" % left())
+            if name == "large":
+                free_b, _ = torch.cuda.mem_get_info()
+                host_gb = os.sysconf("SC_PHYS_PAGES") * os.sysconf("SC_PAGE_SIZE") / 1e9
+                if free_b < 100e9 or host_gb < 80:
+                    raise RuntimeError("skipped: needs ~100 GB of HBM and ~80 GB of host memory")
+            t0 = time.perf_counter()
+            wx = inputs.make_workload(name, device=dev, local_part=w.local_part)
+            t_gen = time.perf_counter() - t0
+            cut = edge_cut(wx, dev)
+            n_rem = wx.num_nodes - int(wx.part_offsets[wx.local_part + 1] - wx.part_offsets[wx.local_part])
+            pts = []
+            for n_hot in (-1, -(-n_rem // 10)):
+                g = ep.graph_from_workload(wx, n_hot=n_hot, carry_over=1, max_window=max(wx.cfg["windows"]),
+                                           staging_mode=args.staging_mode, max_live_windows=ctx["LA"] + 1,
+                                           host_threads=args.host_threads)
+                try:
+                    for Wx in wx.cfg["windows"]:
+                        if n_hot >= 0 and Wx != max(wx.cfg["windows"]):
+                            continue
+                        pts.append(measure_point(ctx, wx, wx.batches, Wx, n_hot, K=1 if name == "large" else 2, warm=1, g=g,
+                                                 max_window=max(wx.cfg["windows"])))
+                finally:
+                    g.close()
+            out[name] = {"workload": workload_name(argparse.Namespace(config=name, batch=wx.cfg["batch"]), wx),
+                         "edge_cut_measured": cut, "generation_s": t_gen, "points": pts}
+            del wx
+            ctx["feats"] = None
+            torch.cuda.empty_cache()
+        except Exception as exc:
+            errors["configs." + name] = repr(exc)
+            ctx["feats"] = None
+            torch.cuda.empty_cache()
+    return out
 
 
 def calibrate(results, meas_j):
@@ -713,24 +963,52 @@ def host_link_peak(dev, nbytes=1 << 30, reps=10):
     return best
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(args, w, batches):
-    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload: one core
+    (first 4 mini-batches as one window), and every host core with the trivially parallel
+    decomposition only (the batches of a full window sampled side by side, their gathers side by
+    side, the window step itself on one thread; results unchanged)."""
+    from concurrent.futures import ThreadPoolExecutor
     from oracle import ggo
-    S = min(args.cpu_sample_batches, len(batches), args.window)
     g = ggo.Graph(*w.host_graph())
     feat = w.host_features()
     po = w.part_offsets
     parts = [np.ascontiguousarray(feat[po[m]:po[m + 1]]) for m in range(len(po) - 1)]
+    S = min(args.cpu_sample_batches, len(batches), args.window)
     st = ggo.State(g.n, po, w.local_part, args.n_hot, 1)
     t0 = time.perf_counter()
     bs = [ggo.Batch(g, batches[j], w.fanouts, w.seed, j) for j in range(S)]
     st.run_window(bs)
     for b in bs:
         ggo.gather(b.nodes, po, parts, w.row_bytes)
-    dt = time.perf_counter() - t0
-    return {"value": S / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "first %d mini-batches of the epoch as one W=%d window (sample + window + gather), %.1f s"
-                      % (S, S, dt)}
+    dt1 = time.perf_counter() - t0
+    del bs
+    cores = os.cpu_count() or 1
+    Wn = min(args.window, len(batches))
+    st = ggo.State(g.n, po, w.local_part, args.n_hot, 1)
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(cores) as ex:                      # ctypes calls release the GIL
+        bs = list(ex.map(lambda j: ggo.Batch(g, batches[j], w.fanouts, w.seed, j), range(Wn)))
+        st.run_window(bs)
+        list(ex.map(lambda b: ggo.gather(b.nodes, po, parts, w.row_bytes), bs))
+    dtn = time.perf_counter() - t0
+    return {"value": Wn / dtn, "unit": UNIT, "cores": min(cores, Wn), "kind": "oracle",
+            "sample": "first %d mini-batches of the epoch as one W=%d window (sample + window + gather), batches sampled and "
+                      "gathered on %d threads, %.1f s" % (Wn, Wn, min(cores, Wn), dtn),
+            "cpu_model": cpu_model(), "host_cores": cores,
+            "one_core": {"value": S / dt1, "unit": UNIT, "cores": 1,
+                         "sample": "first %d mini-batches of the epoch as one W=%d window (sample + window + gather), %.1f s"
+                                   % (S, S, dt1)}}
 
 
 if __name__ == "__main__":

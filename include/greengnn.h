@@ -252,7 +252,8 @@ uint64_t gg_key(uint64_t seed, uint64_t batch, uint64_t layer, uint64_t dst, uin
  *   GATHER  one k_gather launch per region (one launch in four is bracketed when W >= 4, so that
  *           the timing events do not serialise the caller's stream); bytes = |N_b| * (2*row_bytes + 8)
  *           of the bracketed launches
- *   MISS    miss compaction + fill;          bytes = misses * 2*row_bytes   (counted at gg_trace time: 0 here)
+ *   MISS    miss compaction + fill;          bytes = misses * 2*row_bytes   (row over the host link + row written;
+ *           the row count is accumulated on the device by the compaction kernel since the last gg_profile_enable)
  *   SAMPLE  count + scan + select of a hop;  bytes = 24*n_dst + 8*n_edge
  *   FRONTIER mark + word scan + emit + relabel of a hop; bytes = 8*n_edge + 4*n_new
  *   UNIQUE  counter compaction;              bytes = 4*n_access + 8*n_unique
@@ -287,6 +288,22 @@ uint64_t gg_launch_count(void);
  *             kernel, plus warp kernel -> exact ballot/bisection path.
  * Any pointer may be NULL. */
 gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);
+
+/* The measured integer-ALU roofline of a-1 ("keys/s vs the peak of
+ * a key-only micro-kernel measured on the same GPU").  Launches a kernel in which every lane
+ * evaluates keys_per_lane (rounded down to a multiple of 32) consecutive SplitMix64 keys of reading
+ * S1 from a register-resident state -- the high word of fmix, which is all the selection test
+ * reads -- and folds them into one word: no candidate lists, no row logic, no memory traffic.
+ * Grid = ctas_per_sm x SM count CTAs of 256 threads, `reps` timed launches after one warm-up, CUDA
+ * events on the default stream; two formulations of the same arithmetic are timed and
+ * *keys_per_s receives the faster one.  Lane t of CTA c starts launch i (i = 0..reps-1) from the
+ * state 0x9E37 + i + (256 c + t + 1) * 0x632BE59BD9B4E019 and evaluates the states x + gamma * k,
+ * k = 0..keys_per_lane-1; *fold (host, may be NULL) receives the xor over all of them of the high
+ * 32 bits of fmix before its last xor-shift (tests/test_gpu_parity.py recomputes it on the host).
+ * Synchronous.  Errors: INVALID_ARG (null, ctas_per_sm outside [1,8], keys_per_lane < 32);
+ * GG_ERR_CUDA also when the two formulations disagree. */
+gg_status gg_key_peak(int32_t ctas_per_sm, int32_t keys_per_lane, int32_t reps, double* keys_per_s,
+                      uint32_t* fold);
 
 /* Test knobs for the fallback logic of the selection kernel (tests/test_gpu_parity.py); results
  * must stay bit-exact for every setting.  rank_shift in [0,31]: the ranking compares only the

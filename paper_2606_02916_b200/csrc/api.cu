@@ -306,6 +306,7 @@ struct gg_graph {
   DevBuf<uint64_t> tiles64, total64;
   // miss buffers (caller thread, one gather at a time)
   DevBuf<int32_t> miss_tmp_pos, miss_tmp_id, tile_miss, miss_pos, miss_id, n_miss;
+  DevBuf<unsigned long long> miss_total;   // rows the miss path filled since gg_profile_enable
   // pinned
   int32_t* h_small = nullptr;    // phase A readback scratch
   int32_t* h_small_b = nullptr;  // phase B readback scratch
@@ -970,7 +971,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
   g->samp_plan.release(); g->it_hdst.release(); g->it_row0.release(); g->it_deg.release();
   g->it_out.release(); g->it_fb.release();
   g->cnt_tmp.release(); g->miss_tmp_pos.release(); g->miss_tmp_id.release(); g->tile_miss.release();
-  g->miss_pos.release(); g->miss_id.release(); g->n_miss.release();
+  g->miss_pos.release(); g->miss_id.release(); g->n_miss.release(); g->miss_total.release();
   if (g->h_small) cudaFreeHost(g->h_small);
   if (g->h_small_b) cudaFreeHost(g->h_small_b);
   for (int i = 0; i < 2; ++i) {
@@ -1075,6 +1076,8 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   CUC(g->stats.ensure(4)); CUC(g->hist.ensure(256)); CUC(g->owner_cnt.ensure(2 * GG_MAX_PARTS));
   CUC(g->n_delta_dev.ensure(1)); CUC(g->err_flag.ensure(1)); CUC(g->total64.ensure(1)); CUC(g->n_miss.ensure(1));
   CUC(cudaMemset(g->n_miss.p, 0, 4));
+  CUC(g->miss_total.ensure(1));
+  CUC(cudaMemset(g->miss_total.p, 0, sizeof(unsigned long long)));
   CUC(g->seeds_dev.ensure((int64_t)Wmax * cfg->max_batch));
   CUC(g->key_prefix.ensure((int64_t)GG_MAX_LAYERS * Wmax));
   CUC(cudaHostAlloc((void**)&g->h_small, 4096 * sizeof(int32_t), cudaHostAllocDefault));
@@ -1277,6 +1280,7 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   G.miss_tmp_pos = g->miss_tmp_pos.p; G.miss_tmp_id = g->miss_tmp_id.p; G.tile_miss = g->tile_miss.p;
   G.miss_pos = g->miss_pos.p; G.miss_id = g->miss_id.p; G.n_miss = g->n_miss.p;
   G.counters = w->counters.p + (int64_t)b * (2 + GG_MAX_PARTS);
+  G.miss_total = g->miss_total.p;
   // one launch in four is bracketed: a timing event between every pair of back-to-back 50 us
   // kernels costs the step 6 % (the events serialise the stream), a quarter of them 1-2 %
   cudaEvent_t pe = (b & 3) == 1 || w->W < 4 ? g->prof.begin(st) : nullptr;
@@ -1400,6 +1404,7 @@ gg_status gg_profile_enable(gg_graph* g, int32_t on) {
   if (!g) return fail(GG_ERR_INVALID_ARG, "null graph");
   CU(cudaDeviceSynchronize());
   g->prof.clear();
+  CU(cudaMemset(g->miss_total.p, 0, sizeof(unsigned long long)));
   std::lock_guard<std::mutex> l(g->prof.m);
   g->prof.on = on != 0;
   return GG_OK;
@@ -1409,7 +1414,11 @@ gg_status gg_profile_get(gg_graph* g, gg_profile* out) {
   if (!g || !out) return fail(GG_ERR_INVALID_ARG, "null argument");
   CU(cudaDeviceSynchronize());
   g->prof.resolve();
+  // a-8 moves a device-side number of rows per batch: the kernels add them up, 2 * rb bytes per row
+  unsigned long long miss_rows = 0;
+  CU(cudaMemcpy(&miss_rows, g->miss_total.p, sizeof miss_rows, cudaMemcpyDeviceToHost));
   std::lock_guard<std::mutex> l(g->prof.m);
+  g->prof.bytes[GG_PROF_MISS] = (int64_t)miss_rows * 2 * g->rb;
   for (int k = 0; k < GG_PROF_KINDS; ++k) {
     out->ms[k] = g->prof.ms[k];
     out->regions[k] = g->prof.regions[k];
@@ -1435,6 +1444,14 @@ gg_status gg_debug_sampler(int32_t rank_shift, float want_add) {
   if (rank_shift < 0 || rank_shift > 31) return fail(GG_ERR_INVALID_ARG, "rank_shift must be in [0, 31]");
   CU(cudaDeviceSynchronize());
   CU(sampler_debug(rank_shift, want_add));
+  return GG_OK;
+}
+
+gg_status gg_key_peak(int32_t ctas_per_sm, int32_t keys_per_lane, int32_t reps, double* keys_per_s, uint32_t* fold) {
+  if (!keys_per_s) return fail(GG_ERR_INVALID_ARG, "null argument");
+  if (ctas_per_sm < 1 || ctas_per_sm > 8 || keys_per_lane < 32 || reps < 1 || reps > 1000)
+    return fail(GG_ERR_INVALID_ARG, "ctas_per_sm in [1,8], keys_per_lane >= 32, reps in [1,1000]");
+  CU(key_peak(nullptr, ctas_per_sm, keys_per_lane / 32, reps, keys_per_s, fold));
   return GG_OK;
 }
 

@@ -228,7 +228,8 @@ __global__ void __launch_bounds__(kRows) k_gather_tma(GatherArgs A) {
 __global__ void __launch_bounds__(1024)
 k_miss_compact(const int32_t* __restrict__ tile_miss, int tiles, const int32_t* __restrict__ tmp_pos,
                const int32_t* __restrict__ tmp_id, int32_t* __restrict__ miss_pos,
-               int32_t* __restrict__ miss_id, int32_t* __restrict__ n_miss) {
+               int32_t* __restrict__ miss_id, int32_t* __restrict__ n_miss,
+               unsigned long long* __restrict__ miss_total) {
   __shared__ int32_t sm[33];
   __shared__ int32_t carry_s;
   if (threadIdx.x == 0) carry_s = 0;
@@ -247,7 +248,10 @@ k_miss_compact(const int32_t* __restrict__ tile_miss, int tiles, const int32_t* 
     if (threadIdx.x == 0) carry_s = carry + tot;
     __syncthreads();
   }
-  if (threadIdx.x == 0) *n_miss = carry_s;
+  if (threadIdx.x == 0) {
+    *n_miss = carry_s;
+    if (miss_total && carry_s) atomicAdd(miss_total, (unsigned long long)carry_s);   // rows of a-8, for gg_profile_get
+  }
 }
 
 struct RowsArgs {
@@ -346,7 +350,7 @@ void launch_miss_path(cudaStream_t st, const GatherLaunch& G) {
   const int tiles = (G.n + kRows - 1) / kRows;
   count_launches(2);
   k_miss_compact<<<1, 1024, 0, st>>>(G.tile_miss, tiles, G.miss_tmp_pos, G.miss_tmp_id, G.miss_pos,
-                                     G.miss_id, G.n_miss);
+                                     G.miss_id, G.n_miss, G.miss_total);
   // a-8: fill the missed rows straight from the owners' pinned stores (zero-copy reads)
   RowsArgs Rw = {};
   Rw.n = 0; Rw.n_dev = G.n_miss; Rw.src_idx = G.miss_id; Rw.store = G.store; Rw.R = G.R;

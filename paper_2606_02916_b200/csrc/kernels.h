@@ -48,6 +48,8 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
                        int32_t* edge_off_out, int32_t* src_global, const SampleWork& wk);
 void sampler_stats(unsigned long long out[4]);           // synchronous read of g_sampler_stat
 cudaError_t sampler_debug(int rank_shift, float want_add);  // test knobs, see sample.cu
+// key-only micro-kernel: the measured integer-ALU roofline of the sampler (keys per second)
+cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, double* keys_per_s, uint32_t* fold_out);
 // shared by a-1 / a-2: one CTA per batch row, exclusive scan of ceil(n_items[b]/items_per_tile) sums
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
                       int items_per_tile, int32_t* totals);
@@ -100,6 +102,7 @@ struct GatherLaunch {
   int32_t* miss_id;
   int32_t* n_miss;        // device scalar
   int32_t* counters;      // [2 + P]
+  unsigned long long* miss_total;  // device scalar: rows filled by a-8 since the profile was last reset (may be null)
 };
 void launch_gather(cudaStream_t st, const GatherLaunch& G);      // a-7: one k_gather launch
 void launch_miss_path(cudaStream_t st, const GatherLaunch& G);   // a-8: compaction + fill (only if may_miss)

@@ -658,6 +658,80 @@ k_select_warp(const int32_t* __restrict__ indices, int fanout, SamplePlan* __res
   }
 }
 
+// ---- the measured ALU roofline of a-1 (include/greengnn.h gg_key_peak) -------------------------
+// Key evaluation and nothing else: every lane walks a register-resident SplitMix state and forms
+// the high word of fmix for each step (all the selection test reads), folded into one word so
+// the work stays alive.  No list stores, no row logic, no memory traffic.  FORM 0 is the
+// formulation of the product loops (key_zhi: mul.hi for the high-half shifts), FORM 1 uses plain
+// shifts; the reported peak is the better of the two.
+template <int FORM>
+__global__ void __launch_bounds__(256) k_key_peak(uint64_t seed, int groups, uint32_t* __restrict__ fold) {
+  uint64_t x = seed + (uint64_t)(blockIdx.x * 256 + threadIdx.x + 1) * 0x632BE59BD9B4E019ull;
+  uint32_t acc = 0;
+  for (int g = 0; g < groups; ++g) {
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      const uint32_t xlo = (uint32_t)x, xhi = (uint32_t)(x >> 32);
+      if (FORM == 0) {
+        acc ^= key_zhi(xlo, xhi);
+      } else {
+        uint32_t lo = xlo ^ __funnelshift_r(xlo, xhi, 30), hi = xhi ^ (xhi >> 30);
+        const uint64_t p = (uint64_t)lo * kC1lo;
+        hi = mad_lo_u32(lo, kC1hi, mad_lo_u32(hi, kC1lo, (uint32_t)(p >> 32)));
+        lo = (uint32_t)p;
+        lo ^= __funnelshift_r(lo, hi, 27);
+        hi ^= hi >> 27;
+        acc ^= mulhi_u32(lo, kC2lo) + hi * kC2lo + lo * kC2hi;
+      }
+      x += kGamma;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) acc ^= __shfl_xor_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0) atomicXor(fold, acc);
+}
+
+// keys per second of the better formulation (CUDA events on `st`, after one warm-up launch each).
+// fold_out = xor of the keys of formulation 0's timed launches (launch i starts from seed
+// 0x9E37 + i); cudaErrorUnknown if the two formulations fold to different words.
+cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, double* keys_per_s, uint32_t* fold_out) {
+  uint32_t* d = nullptr;
+  cudaError_t e = cudaMalloc((void**)&d, 3 * sizeof(uint32_t));
+  if (e != cudaSuccess) return e;
+  cudaMemsetAsync(d, 0, 3 * sizeof(uint32_t), st);
+  cudaEvent_t a, b;
+  cudaEventCreate(&a);
+  cudaEventCreate(&b);
+  const int grid = sm_count() * ctas_per_sm;
+  double best = 0;
+  for (int form = 0; form < 2 && e == cudaSuccess; ++form) {
+    if (form == 0) k_key_peak<0><<<grid, 256, 0, st>>>(1ull, groups, d + 2);   // warm-up
+    else k_key_peak<1><<<grid, 256, 0, st>>>(1ull, groups, d + 2);
+    cudaEventRecord(a, st);
+    for (int i = 0; i < reps; ++i) {
+      if (form == 0) k_key_peak<0><<<grid, 256, 0, st>>>(0x9E37ull + i, groups, d);
+      else k_key_peak<1><<<grid, 256, 0, st>>>(0x9E37ull + i, groups, d + 1);
+    }
+    count_launches(reps + 1);
+    cudaEventRecord(b, st);
+    e = cudaEventSynchronize(b);
+    float ms = 0;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    if (e != cudaSuccess) break;
+    const double rate = (double)grid * 256.0 * groups * 32.0 * reps / (ms * 1e-3);
+    if (rate > best) best = rate;
+  }
+  uint32_t h[3] = {0, 0, 0};
+  if (e == cudaSuccess) e = cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess && h[0] != h[1]) e = cudaErrorUnknown;
+  if (fold_out) *fold_out = h[0];
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(d);
+  *keys_per_s = best;
+  return e;
+}
+
 void sampler_stats(unsigned long long out[4]) {
   cudaMemcpyFromSymbol(out, g_sampler_stat, 4 * sizeof(unsigned long long));
 }

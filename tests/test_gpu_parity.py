@@ -23,6 +23,28 @@ def test_library_key_matches_golden_and_oracle(dev):
         assert binding.gg_key(*args) == ggo.key(*args)
 
 
+def test_key_peak_kernel_evaluates_the_methods_keys(dev):
+    """The key-only micro-kernel behind bench.py's measured ALU roofline (gg_key_peak) folds exactly
+    the keys of reading S1: host recomputation of the xor of every lane's 32 key words, with the
+    oracle's fmix on a sample of the states."""
+    from oracle import ggo
+    from paper_2606_02916_b200 import binding
+    rate, fold = binding.key_peak(ctas_per_sm=1, keys_per_lane=32, reps=1, with_fold=True)
+    assert rate > 0
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    gamma, step = np.uint64(0x9E3779B97F4A7C15), np.uint64(0x632BE59BD9B4E019)
+    with np.errstate(over="ignore"):
+        gid = np.arange(1, sms * 256 + 1, dtype=np.uint64)
+        x = (np.uint64(0x9E37) + gid * step)[:, None] + gamma * np.arange(32, dtype=np.uint64)[None, :]
+        z = (x ^ (x >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+    zhi = (z >> np.uint64(32)).astype(np.uint32)
+    assert fold == int(np.bitwise_xor.reduce(zhi.ravel()))
+    for i, k in [(0, 0), (17, 5), (sms * 256 - 1, 31), (1000, 16)]:
+        f = ggo.fmix(int(x[i, k]))                      # fmix = z ^ (z >> 31): the last step keeps the high word's upper 31 bits
+        assert (f >> 32) == int(zhi[i, k]) ^ (int(zhi[i, k]) >> 31)
+
+
 @pytest.mark.parametrize("n_hot,carry,mode", [(-1, 1, 0), (200, 1, 0), (200, 0, 0), (-1, 1, 1), (0, 1, 0)])
 def test_tiny_one_window(workload, dev, n_hot, carry, mode):
     w = workload("tiny", dev)
@@ -404,6 +426,59 @@ def test_dense_full_size_first_window(workload, dev):
     w = workload("dense", dev)
     s = pu.check_epoch(w, W=4, n_hot=-1, max_batches=4, cache_samples=128)
     assert s["batches"] == 4
+
+
+def _threads():
+    import os
+    return min(16, os.cpu_count() or 1)
+
+
+@pytest.mark.parametrize("B", [2048, 4096])
+def test_products_full_size_larger_batches_first_window_W16(workload, dev, B):
+    """configs[2]'s other batch sizes, which bench.py times (`vs_batch_at_W`, `configs`): the same
+    epoch's seeds cut into batches of 2048 / 4096, first W=16 window at full size (frontier caps x2 /
+    x4, the last hop of B=4096 capped at N), every array against the oracle."""
+    import dataclasses
+    w0 = workload("products", dev)
+    seeds = np.concatenate(w0.batches)
+    w = dataclasses.replace(w0, batches=[seeds[i:i + B] for i in range(0, len(seeds), B)])
+    s = pu.check_epoch(w, W=16, n_hot=-1, max_batches=16, cache_samples=256, lookahead=6, oracle_threads=_threads())
+    assert s["batches"] == 16 and s["misses"] == 0 and s["rows"] > 16 * 300_000 * (B // 1024) // 2
+
+
+def test_products_full_size_three_consecutive_windows_W16(workload, dev):
+    """Delta / carry-over at 5 M-row scale: three consecutive W=16 windows with an unlimited budget
+    (windows 2 and 3 stage only H_k \\ C_{k-1} and carry the rest), request lists,
+    carried lists, cache rows and every batch element-wise."""
+    w = workload("products", dev)
+    s = pu.check_epoch(w, W=16, n_hot=-1, max_batches=48, cache_samples=256, lookahead=6, oracle_threads=_threads())
+    assert s["windows"] == 3 and s["batches"] == 48 and s["misses"] == 0
+
+
+def test_products_full_size_budgeted_W16_two_windows(workload, dev):
+    """The budgeted series bench.py times (n_hot = 10 % of the remote nodes) at W=16:
+    threshold selection with a quota, a stale cache across the boundary and the miss path at the
+    size of the timed runs."""
+    w = workload("products", dev)
+    n_remote = w.num_nodes - int(w.part_offsets[1] - w.part_offsets[0])
+    s = pu.check_epoch(w, W=16, n_hot=-(-n_remote // 10), max_batches=32, cache_samples=256, lookahead=6,
+                       oracle_threads=_threads())
+    assert s["windows"] == 2 and s["misses"] > 0
+
+
+def test_dense_full_size_W16_two_windows_and_W1(workload, dev):
+    """configs[3] at full size across a window boundary: W=16 over two windows (Delta, carry-over and
+    the carried D2D copy with rb = 2408, the 8-byte path), then W=1 (per-batch fetch, three windows)
+    and a budgeted W=4 pair (miss fill at rb = 2408)."""
+    w = workload("dense", dev)
+    thr = _threads()
+    s = pu.check_epoch(w, W=16, n_hot=-1, max_batches=32, cache_samples=128, lookahead=6, oracle_threads=thr)
+    assert s["windows"] == 2 and s["batches"] == 32 and s["misses"] == 0
+    s = pu.check_epoch(w, W=1, n_hot=-1, max_batches=3, cache_samples=64, oracle_threads=thr)
+    assert s["windows"] == 3
+    n_remote = w.num_nodes - int(w.part_offsets[1] - w.part_offsets[0])
+    s = pu.check_epoch(w, W=4, n_hot=-(-n_remote // 10), max_batches=8, cache_samples=64, oracle_threads=thr)
+    assert s["windows"] == 2 and s["misses"] > 0
 
 
 def test_large_full_size_first_windows(dev):
