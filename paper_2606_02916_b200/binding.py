@@ -85,7 +85,7 @@ PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage
 
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
-           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_key_peak", "gg_simulate", "gg_rank_calibrate",
+           "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_sampler_tune", "gg_key_peak", "gg_simulate", "gg_rank_calibrate",
            "gg_sage_create", "gg_sage_destroy", "gg_sage_step", "gg_sage_params"]
 
 _lib = None
@@ -125,6 +125,7 @@ def load_library(path: Optional[str] = None):
     lib.gg_key.restype = u64
     lib.gg_sampler_stats.argtypes = [P(u64), P(u64), P(u64)]
     lib.gg_debug_sampler.argtypes = [i32, C.c_float]
+    lib.gg_sampler_tune.argtypes = [i32, i32]
     lib.gg_key_peak.argtypes = [i32, i32, i32, P(C.c_double), P(C.c_uint32)]
     lib.gg_simulate.argtypes = [vp, vp, vp, i32, u64, vp, i32, vp, i32, P(gg_energy_model), P(gg_sim_result),
                                 P(i32), vp, vp]
@@ -157,6 +158,11 @@ def sampler_stats() -> dict:
     k, r, f = u64(0), u64(0), u64(0)
     _check_global(load_library().gg_sampler_stats(C.byref(k), C.byref(r), C.byref(f)))
     return {"keys": int(k.value), "rows": int(r.value), "fallbacks": int(f.value)}
+
+
+def sampler_tune(single_bins: int = 36, warp_bin: int = 36) -> None:
+    """Degree-bin cut-overs of the selection kernels (include/greengnn.h gg_sampler_tune)."""
+    _check_global(load_library().gg_sampler_tune(single_bins, warp_bin))
 
 
 def key_peak(ctas_per_sm: int = 8, keys_per_lane: int = 65536, reps: int = 5, with_fold: bool = False):

@@ -298,9 +298,10 @@ struct gg_graph {
   DevBuf<uint64_t> it_hdst;
   DevBuf<int64_t> it_row0;
   DevBuf<uint32_t> it_deg;
-  DevBuf<int32_t> it_out, it_fb;
+  DevBuf<int32_t> it_out, it_fb, it_cnt;
+  DevBuf<uint2> it_cand;
   int64_t cnt_words = 0;  // padded words of cnt8
-  int64_t planned_t32 = 0, planned_cnt_tmp = 0, planned_miss = 0, planned_t64 = 0;
+  int64_t planned_t32 = 0, planned_cnt_tmp = 0, planned_miss = 0, planned_t64 = 0, planned_cand = 0;
   // phase B workspaces (stager thread only)
   DevBuf<int32_t> tiles32_b, owner_cnt, n_delta_dev;
   DevBuf<uint64_t> tiles64, total64;
@@ -393,8 +394,9 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
   const int64_t node_pitch = ceil_div(cap_front[L], 4) * 4;
   if ((int64_t)W * node_pitch >= (1ll << 31))
     return fail(GG_ERR_CAPACITY, "W * max_input_nodes = %lld exceeds int32 indexing", (long long)((int64_t)W * node_pitch));
-  int64_t max_tiles = 1;
+  int64_t max_tiles = 1, cand = 1;
   for (int h = 0; h < L; ++h) {
+    cand = std::max<int64_t>(cand, (int64_t)W * cap_front[h] * sample_cand_cap(fanouts[h]));
     const int64_t ecap = (int64_t)W * cap_front[h] * fanouts[h];
     if (ecap >= (1ll << 31))
       return fail(GG_ERR_CAPACITY, "hop %d edge cap %lld exceeds int32 indexing", h, (long long)ecap);
@@ -407,7 +409,7 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
   const int64_t t64 = ceil_div(ucap, 1024) + 1;
   const int64_t mcap = ceil_div(node_pitch, 64) * 64;
   const bool grow = t32 > g->planned_t32 || cnt_tmp > g->planned_cnt_tmp || t64 > g->planned_t64 ||
-                    mcap > g->planned_miss;
+                    mcap > g->planned_miss || cand > g->planned_cand;
   if (!grow) return GG_OK;
   if (need_drain) {
     *need_drain = true;
@@ -421,6 +423,8 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
   ENS(g->it_deg, cnt_tmp);
   ENS(g->it_out, cnt_tmp);
   ENS(g->it_fb, cnt_tmp);
+  ENS(g->it_cnt, cnt_tmp);
+  ENS(g->it_cand, cand);
   ENS(g->tiles64, t64);
   ENS(g->miss_tmp_pos, mcap);
   ENS(g->miss_tmp_id, mcap);
@@ -431,6 +435,7 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
   g->planned_cnt_tmp = std::max(g->planned_cnt_tmp, cnt_tmp);
   g->planned_t64 = std::max(g->planned_t64, t64);
   g->planned_miss = std::max(g->planned_miss, mcap);
+  g->planned_cand = std::max(g->planned_cand, cand);
   // every window arena now, while the pipeline is drained: an arena that met its first (or a
   // larger) window inside an epoch used to cudaMalloc hundreds of MB under the running pipeline
   for (int s = 0; s < g->n_win; ++s) {
@@ -531,6 +536,7 @@ static gg_status stage_a(gg_graph* g, Window* w) {
     wk.plan = g->samp_plan.p;
     wk.items.hdst = g->it_hdst.p; wk.items.row0 = g->it_row0.p; wk.items.deg = g->it_deg.p;
     wk.items.out = g->it_out.p; wk.items.fallback = g->it_fb.p;
+    wk.items.row_cnt = g->it_cnt.p; wk.items.cand = g->it_cand.p;
     cudaEvent_t pe = g->prof.begin(st);
     launch_sample_hop(st, g->indptr, g->indices, w->nodes.p, w->node_pitch, n_dst, dst_off, W, max_nd,
                       w->fanouts[h], g->key_prefix.p + h * Wmax, g->cnt_tmp.p, cnt_pitch, g->tiles32.p,
@@ -969,7 +975,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
   g->hist.release(); g->owner_cnt.release(); g->n_delta_dev.release(); g->err_flag.release();
   g->seeds_dev.release(); g->tiles64.release(); g->total64.release(); g->key_prefix.release();
   g->samp_plan.release(); g->it_hdst.release(); g->it_row0.release(); g->it_deg.release();
-  g->it_out.release(); g->it_fb.release();
+  g->it_out.release(); g->it_fb.release(); g->it_cnt.release(); g->it_cand.release();
   g->cnt_tmp.release(); g->miss_tmp_pos.release(); g->miss_tmp_id.release(); g->tile_miss.release();
   g->miss_pos.release(); g->miss_id.release(); g->n_miss.release(); g->miss_total.release();
   if (g->h_small) cudaFreeHost(g->h_small);
@@ -1444,6 +1450,14 @@ gg_status gg_debug_sampler(int32_t rank_shift, float want_add) {
   if (rank_shift < 0 || rank_shift > 31) return fail(GG_ERR_INVALID_ARG, "rank_shift must be in [0, 31]");
   CU(cudaDeviceSynchronize());
   CU(sampler_debug(rank_shift, want_add));
+  return GG_OK;
+}
+
+gg_status gg_sampler_tune(int32_t single_bins, int32_t warp_bin) {
+  if (single_bins < 28 || single_bins > 128 || warp_bin < 0 || warp_bin > 128)
+    return fail(GG_ERR_INVALID_ARG, "single_bins must be in [28, 128] (rows below degree 128 are one chunk), warp_bin in [0, 128]");
+  CU(cudaDeviceSynchronize());
+  CU(sampler_tune(single_bins, warp_bin));
   return GG_OK;
 }
 

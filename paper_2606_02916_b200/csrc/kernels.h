@@ -33,13 +33,16 @@ struct SampleItems {
   int64_t* row0;      // indptr[dst]
   uint32_t* deg;
   int32_t* out;       // final offset of the row's first kept neighbor in src_global
-  int32_t* fallback;  // item indices handed from the thread kernel to the warp kernel
+  int32_t* fallback;  // item indices handed to the warp kernel
+  int32_t* row_cnt;   // candidates appended to the row's list so far (multi-chunk rows)
+  uint2* cand;        // [item][sample_cand_cap(fanout)] {high key word before the last xor-shift, edge position}
 };
 struct SampleWork {
   void* plan;         // device, sample_plan_bytes()
   SampleItems items;  // each array holds at least the hop's destination count
 };
 size_t sample_plan_bytes();
+int sample_cand_cap(int fanout);   // entries of a row's candidate list in global memory (0: the hop does not use one)
 void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* indices,
                        const int32_t* nodes, int64_t node_pitch, const BatchOffsets& n_dst,
                        const BatchOffsets& dst_off, int W, int max_nd, int fanout,
@@ -48,6 +51,7 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
                        int32_t* edge_off_out, int32_t* src_global, const SampleWork& wk);
 void sampler_stats(unsigned long long out[4]);           // synchronous read of g_sampler_stat
 cudaError_t sampler_debug(int rank_shift, float want_add);  // test knobs, see sample.cu
+cudaError_t sampler_tune(int single_bins, int warp_bin);     // degree-bin cut-overs of the selection kernels
 // key-only micro-kernel: the measured integer-ALU roofline of the sampler (keys per second)
 cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, double* keys_per_s, uint32_t* fold_out);
 // shared by a-1 / a-2: one CTA per batch row, exclusive scan of ceil(n_items[b]/items_per_tile) sums

@@ -6,20 +6,28 @@
 // edge position.  The key depends on (seed, batch, layer, dst, j) only -- never on the
 // neighbor id -- so the adjacency row is not read to select; only the <= f chosen entries are.
 //
-// Five launches per hop (the rows of a power-law graph differ in cost by 1000x, so they are
-// binned by degree and each bin gets the granularity that suits it):
+// Launches per hop (the rows of a power-law frontier differ in cost by 1000x, so the KEY SPACE,
+// not the row list, is what gets divided among the lanes):
 //   k_sample_count   one thread per destination: c = min(deg, f) -> cnt_tmp, per-tile sums,
-//                    histogram of the keyed rows (deg > f) over half-octave degree bins
+//                    histogram of the keyed rows (deg > f) over quarter-octave degree bins
 //   k_tile_scan      one CTA per batch: exclusive scan of that batch's tile sums, batch total;
-//                    CTA 0 also turns the histogram into bin regions (largest degrees first)
+//                    CTA 0 also turns the histogram into bin regions (largest degrees first) and
+//                    into the chunk numbering below
 //   k_sample_plan    one CTA per tile of 256 destinations: in-tile scan -> block indptr and the
 //                    FINAL output offset of every row (no atomics on output order =>
 //                    deterministic); rows with deg <= f are copied; every other row becomes a
 //                    work item {h_dst, row start, deg, output offset} in its bin's region
-//   k_select_thread  bins with deg < kThreadDeg: ONE THREAD PER ROW (32 rows of similar degree
-//                    per warp); rows it cannot prove exact are appended to a fallback list
-//   k_select_warp    bins with deg >= kThreadDeg, then the fallback list: ONE WARP PER ROW,
-//                    largest rows first, dynamic queue
+//   k_select_chunk   ONE LANE PER CHUNK of <= 128 consecutive edge positions.  Every row of a bin is
+//                    cut into the same number n_b of equal chunks (n_b = ceil(bin's largest degree /
+//                    128)), so chunk k of the bin is chunk k % n_b of the bin's row k / n_b -- no chunk
+//                    table -- and the 32 lanes of a warp always run loops of nearly the same length,
+//                    whatever the degree mix.  A row of degree < 128 is one chunk: its lane ranks its
+//                    candidates and emits the row.  A longer row's lanes append their candidates to the
+//                    row's list in global memory (one atomic per lane that found any).
+//   k_select_rank    one thread per multi-chunk row: ranks the row's ~f+2.5 sqrt(f) candidates,
+//                    proves the result (kept == f) and emits it in ascending edge position
+//   k_select_warp    ONE WARP PER ROW for the rows the kernels above could not prove exact (and for
+//                    every keyed row when fanout > kChunkMaxFanout)
 #include "common.cuh"
 #include "kernels.h"
 
@@ -27,7 +35,7 @@ namespace gg {
 
 // cumulative sampler statistics: [0] key evaluations the method asks for (sum of deg over rows
 // with deg > fanout), [1] such rows, [2] rows that took the exact ballot/bisection path,
-// [3] rows the thread-per-row kernel handed to the warp kernel
+// [3] rows the chunk / rank kernels handed to the warp kernel
 __device__ unsigned long long g_sampler_stat[4];
 // test knobs (gg_debug_sampler): compare only the top 32-shift bits when ranking (forces
 // high-word ties), and add to the candidate target (forces list overflow / too few candidates)
@@ -37,26 +45,50 @@ __constant__ float c_want_add = 0.0f;
 constexpr int kTile = 256;      // destinations per CTA tile
 constexpr int kCand = 256;      // candidate buffer per warp
 constexpr int kWarps = 8;
-constexpr int kBins = 64;       // half-octave degree bins: bin = 2*floor(log2 deg) + next bit
-constexpr int kThreadDegLog2 = 9;
-constexpr uint32_t kThreadDeg = 1u << kThreadDegLog2;   // rows below this degree: one thread per row
-constexpr int kThreadMaxFanout = 16;                    // ... when fanout <= this (candidate list in smem)
+constexpr int kBins = 128;      // quarter-octave degree bins: bin = 4*floor(log2 deg) + next two bits
+constexpr int kChunk = 128;     // edge positions per chunk (at most)
+// tunables (gg_sampler_tune): rows in bins below c_single_bins are one chunk each, whatever their
+// degree; rows in bins >= c_warp_bin go to the warp kernel.  Defaults (bin 36 =
+// degree 512): one lane per row below degree 512, one warp per row above; cutting the rows of
+// degree 128..4095 into chunks with the candidates merged through global memory measured slower
+// (products W=16, sampling per epoch alone: 16.5 ms at 36/36 vs 18.8-20.8 ms for 28/48, 36/48,
+// 28/128), so the multi-chunk path is off by default.
+__constant__ int c_single_bins = 36;
+__constant__ int c_warp_bin = 36;
+constexpr int kChunkMaxFanout = 25;   // candidate lists of the chunk path hold <= 64 entries
 
 // device-side plan of one hop (zeroed before k_sample_count)
 struct SamplePlan {
   int32_t bin_count[kBins];    // keyed rows per bin (k_sample_count)
   int32_t bin_start[kBins];    // first item of the bin's region, bins in DESCENDING degree order
   int32_t bin_cursor[kBins];   // items already placed (k_sample_plan)
+  unsigned long long bin_chunk0[kBins + 1];  // [o]: first chunk of the o-th bin in descending order
+                                             // (bin kBins-1-o), each bin padded to a multiple of 32
+  unsigned long long n_chunks;      // = bin_chunk0[kBins]
+  unsigned long long chunk_cursor;  // dynamic queue of the chunk kernel (units of 32 chunks)
   int32_t n_items;             // keyed rows
-  int32_t n_warp_items;        // items [0, n_warp_items) belong to the warp kernel
-  int32_t n_fallback;          // rows the thread kernel handed over
+  int32_t n_multi;             // items [n_warp_items, n_multi) are multi-chunk rows (c_single_bins <= bin < c_warp_bin)
+  int32_t n_warp_items;        // items [0, n_warp_items) belong to the warp kernel (bins >= c_warp_bin; fanout > kChunkMaxFanout: all)
+  int32_t n_fallback;          // rows handed over to the warp kernel
   int32_t warp_cursor;         // dynamic queue of the warp kernel
 };
 
-__device__ __forceinline__ int deg_bin(uint32_t deg) {   // deg >= 2
+__host__ __device__ __forceinline__ int deg_bin(uint32_t deg) {   // deg >= 2; monotone in deg
+#ifdef __CUDA_ARCH__
   const int l = 31 - __clz(deg);
-  return 2 * l + (int)((deg >> (l - 1)) & 1u);
+#else
+  int l = 0;
+  while ((deg >> (l + 1)) != 0) ++l;
+#endif
+  return l >= 2 ? 4 * l + (int)((deg >> (l - 2)) & 3u) : 4 + (int)((deg << 1) & 3u);
 }
+// chunks per row of a bin: 1 below degree kChunk, else ceil(largest degree of the bin / kChunk)
+__host__ __device__ __forceinline__ uint32_t bin_chunks(int bin, int single_bins) {
+  if (bin < single_bins) return 1u;
+  const int l = bin >> 2, k = bin & 3;
+  return ((uint32_t)(5 + k) << (l - 2)) + (kChunk - 2) >> 7;   // largest degree = ((5+k) << (l-2)) - 1
+}
+static_assert(kChunk == 128, "bin_chunks shifts by log2(kChunk) = 7");
 
 __global__ void __launch_bounds__(kTile)
 k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ nodes,
@@ -97,7 +129,7 @@ k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ n
     rows = s_bin[threadIdx.x];
     if (rows) atomicAdd(&plan->bin_count[threadIdx.x], rows);
   }
-  if (threadIdx.x < 64) {
+  if (threadIdx.x < kBins) {
 #pragma unroll
     for (int o = 16; o; o >>= 1) rows += __shfl_xor_sync(0xffffffffu, rows, o);
     if ((threadIdx.x & 31) == 0 && rows) atomicAdd(&g_sampler_stat[1], (unsigned long long)rows);
@@ -108,7 +140,7 @@ k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ n
 // One CTA per batch (row): in-place exclusive scan of row[0..n_tiles[b]) ; totals[b] = sum.
 __global__ void __launch_bounds__(1024)
 k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, int items_per_tile,
-            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int min_warp_bin) {
+            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int all_to_warp) {
   __shared__ int32_t sm[33];
   __shared__ int32_t carry_s;
   const int b = blockIdx.x;
@@ -127,19 +159,47 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
     __syncthreads();
   }
   if (threadIdx.x == 0) totals[b] = carry_s;
-  // bin regions of the hop's work items, largest degrees first (the warp kernel's bins lead)
-  if (plan && b == 0 && threadIdx.x == 0) {
-    int32_t acc = 0, n_warp = 0;
-    for (int k = kBins - 1; k >= 0; --k) {
-      plan->bin_start[k] = acc;
-      plan->bin_cursor[k] = 0;
-      acc += plan->bin_count[k];
-      if (k == min_warp_bin) n_warp = acc;
+  // bin regions of the hop's work items, largest degrees first, and the chunk numbering: bin b's
+  // rows_b * n_b chunks are numbered consecutively (chunk k = chunk k % n_b of row k / n_b), each
+  // bin padded to a multiple of 32 so that a warp's 32 chunks never straddle two bins
+  if (plan && b == 0) {
+    __shared__ int32_t s_cnt[kBins], s_start[kBins];
+    __shared__ unsigned long long s_nc[kBins], s_c0[kBins + 1];
+    const int single_bins = c_single_bins, warp_bin = all_to_warp ? 0 : c_warp_bin;
+    if (threadIdx.x < kBins) {
+      const int k = threadIdx.x;
+      const int32_t n = plan->bin_count[k];
+      s_cnt[k] = n;
+      const unsigned long long nc = k >= warp_bin ? 0ull : (unsigned long long)n * bin_chunks(k, single_bins);
+      s_nc[k] = (nc + 31ull) & ~31ull;
     }
-    plan->n_items = acc;
-    plan->n_warp_items = min_warp_bin <= 0 ? acc : n_warp;
-    plan->n_fallback = 0;
-    plan->warp_cursor = 0;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int32_t acc = 0, n_multi = 0, n_warp = 0;
+      unsigned long long c0 = 0;
+      for (int k = kBins - 1; k >= 0; --k) {
+        s_start[k] = acc;
+        s_c0[kBins - 1 - k] = c0;
+        c0 += s_nc[k];
+        acc += s_cnt[k];
+        if (k == single_bins) n_multi = acc;
+        if (k == warp_bin) n_warp = acc;
+      }
+      s_c0[kBins] = c0;
+      plan->n_chunks = c0;
+      plan->chunk_cursor = 0;
+      plan->n_items = acc;
+      plan->n_warp_items = n_warp;
+      plan->n_multi = n_multi > n_warp ? n_multi : n_warp;
+      plan->n_fallback = 0;
+      plan->warp_cursor = 0;
+    }
+    __syncthreads();
+    if (threadIdx.x < kBins) {
+      plan->bin_start[threadIdx.x] = s_start[threadIdx.x];
+      plan->bin_cursor[threadIdx.x] = 0;
+    }
+    if (threadIdx.x <= kBins) plan->bin_chunk0[threadIdx.x] = s_c0[threadIdx.x];
   }
 }
 
@@ -304,15 +364,18 @@ constexpr uint32_t kC1lo = 0x1CE4E5B9u, kC1hi = 0xBF58476Du, kC2lo = 0x133111EBu
 
 // high word of z = fmix's value before the last xor-shift, from the state x = {xhi, xlo}
 __device__ __forceinline__ uint32_t key_zhi(uint32_t xlo, uint32_t xhi) {
+  // measured on B200 (warp instructions per clock per sub-partition): IMAD 0.49, SHF / LOP3 / IADD3
+  // 0.5, IMAD.HI and IMAD.WIDE 0.25 -- so the high-half shifts are plain shifts (round 1 used
+  // mul.hi for them to unload the ALU pipe: 4 clocks each on the FMA pipe instead of 2 on the ALU pipe)
   uint32_t lo = xlo ^ __funnelshift_r(xlo, xhi, 30);
-  uint32_t hi = xhi ^ mulhi_u32(xhi, 1u << 2);
-  // {hi,lo} * C1 (low 64 bits) in three FMA-pipe instructions: the cross terms accumulate
-  // straight onto the high half of the wide product
+  uint32_t hi = xhi ^ (xhi >> 30);
+  // {hi,lo} * C1 (low 64 bits): the cross terms accumulate straight onto the high half of the
+  // wide product
   const uint64_t p = (uint64_t)lo * kC1lo;
   hi = mad_lo_u32(lo, kC1hi, mad_lo_u32(hi, kC1lo, (uint32_t)(p >> 32)));
   lo = (uint32_t)p;
   lo ^= __funnelshift_r(lo, hi, 27);
-  hi ^= mulhi_u32(hi, 1u << 5);
+  hi ^= hi >> 27;
   return mulhi_u32(lo, kC2lo) + hi * kC2lo + lo * kC2hi;
 }
 __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
@@ -323,13 +386,16 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
   return v;
 }
+__device__ __forceinline__ void sts_v2(uint32_t addr, uint32_t a, uint32_t b) {
+  asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
+}
+// entry s of lane l: {z_hi, x_lo} at s*256 + l*8 -- one predicated 64-bit store, conflict-free
 __device__ __forceinline__ void fast_step(uint64_t x, uint32_t M, uint32_t& a) {
   const uint32_t xlo = (uint32_t)x;
   const uint32_t z = key_zhi(xlo, (uint32_t)(x >> 32));
   if (z <= M) {
-    sts_u32(a, z);
-    sts_u32(a + kLaneCap * 128, xlo);
-    a += 128;
+    sts_v2(a, z, xlo);
+    a += 256;
   }
 }
 
@@ -357,9 +423,9 @@ __device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row
   } else {
     const uint32_t M = (uint32_t)fminf(__fdividef(wantf, (float)deg) * 4294967296.0f, 4294967040.0f) | 1u;
     const uint32_t K = deg >> 5;
-    const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(scratch) + lane * 4;
+    const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(scratch) + lane * 8;
     uint32_t a = a0;
-    const uint32_t a_lim4 = a0 + (kLaneCap - 4) * 128, a_lim1 = a0 + (kLaneCap - 1) * 128;
+    const uint32_t a_lim4 = a0 + (kLaneCap - 4) * 256, a_lim1 = a0 + (kLaneCap - 1) * 256;
     uint64_t x = hdst + (uint64_t)(lane * K + 1u) * kGamma;
     uint32_t n4 = K >> 2;
     // The ALU pipe (IADD3 / SHF / LOP3 / ISETP, one warp instruction per 2 clocks) carries half
@@ -391,7 +457,7 @@ __device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row
       pt = zt <= M;
     }
     const unsigned tmask = __ballot_sync(0xffffffffu, pt);
-    const int c = (int)((a - a0) >> 7);
+    const int c = (int)((a - a0) >> 8);
     const int total_main = __reduce_add_sync(0xffffffffu, c);
     total = total_main + __popc(tmask);
     if (__any_sync(0xffffffffu, ovf) || total < f || total > kFastCand) return false;
@@ -404,8 +470,8 @@ __device__ __forceinline__ bool warp_select_fast(const int32_t* __restrict__ row
     const int off = incl - c;
     const uint32_t hlo = (uint32_t)hdst;
     for (int s = 0; s < c; ++s) {
-      const uint32_t z = lds_u32(a0 + s * 128);
-      const uint32_t xl = lds_u32(a0 + s * 128 + kLaneCap * 128);
+      const uint32_t z = lds_u32(a0 + s * 256);
+      const uint32_t xl = lds_u32(a0 + s * 256 + 4);
       c_hi[off + s] = (z ^ (z >> 31)) >> rshift;
       c_pos[off + s] = (xl - hlo) * kGammaLoInv - 1u;
     }
@@ -509,128 +575,238 @@ k_sample_plan(const int64_t* __restrict__ indptr, const int32_t* __restrict__ in
     items.row0[q] = r0;
     items.deg[q] = deg;
     items.out[q] = out;
+    if (bin >= c_single_bins) items.row_cnt[q] = 0;   // candidates the chunk kernel will append
   }
 }
 
-// ---- one thread per row (deg < kThreadDeg, fanout <= kThreadMaxFanout) -------------------------
-// Same selection as warp_select_fast, serial in one thread: positions are visited in ascending
-// order, a position whose z_hi passes the odd threshold M appends (z_hi, x_lo) to the thread's
-// own list in shared memory (entry s of thread t: z at s*768 + t*4, the low half of x_lo at
-// s*768 + 512 + t*2: no bank conflicts), the c candidates are ranked on the high key word (c^2 compares, c ~ 12-27), and
-// `kept == fanout` proves the result.  Anything else goes to the warp kernel's fallback list.
-constexpr int kTThreads = 128;
-constexpr uint32_t kTSlot = kTThreads * 6;   // bytes per list entry across the CTA (z u32 | x u16)
+// ---- one lane per chunk ---------------------------------------------------------------------------
+// The lane walks its chunk's positions in ascending order; a position whose z_hi passes the row's
+// odd threshold M appends {z_hi, low word of the SplitMix state} to the lane's own list in shared
+// memory with ONE predicated 64-bit store (entry s of thread t at s*1024 + t*8: conflict-free) and
+// one predicated add -- no ballot, no branch in the loop.  The position comes back from the state's
+// low word: (x - h) * gamma^-1 - 1 (mod 2^32).
+//   single-chunk row (degree < 128): the lane ranks its c candidates on the high key word (the
+//     fanout-th smallest DISTINCT value, one round per rank), keeps those at or below it, and
+//     `kept == fanout` proves the result (DESIGN.md Sec. 6 (iv)); it then emits the row;
+//   longer row: the lane reserves c slots of the row's candidate list in global memory with one
+//     atomicAdd and writes {z_hi, position}; k_select_rank finishes the row.
+// Anything that cannot be proved (list overflow, too few candidates, a high-word tie at the
+// boundary) goes to the warp kernel's fallback list.
+constexpr int kCThreads = 128;
+constexpr uint32_t kCSlot = kCThreads * 8;   // bytes per list entry across the CTA
 
-__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
-  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
-}
-__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
-  unsigned short v;
-  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
-  return v;
-}
-// a: address of the thread's next z slot, ax: of its next x slot (low 16 bits of the state's low
-// word are enough to recover a position < 65536)
-__device__ __forceinline__ void thread_step(uint64_t x, uint32_t M, uint32_t& a, uint32_t& ax) {
+__device__ __forceinline__ void chunk_step(uint64_t x, uint32_t M, uint32_t& a) {
   const uint32_t xlo = (uint32_t)x;
   const uint32_t z = key_zhi(xlo, (uint32_t)(x >> 32));
   if (z <= M) {
-    sts_u32(a, z);
-    sts_u16(ax, xlo);
-    a += kTSlot;
-    ax += kTSlot;
+    sts_v2(a, z, xlo);
+    a += kCSlot;
   }
 }
+// candidate list capacity (per lane in shared memory, per row in global memory): the target count
+// plus 3.5 sigma of a Poisson count, a multiple of 4, at most 64 (keep flags are one 64-bit word)
+__host__ __device__ __forceinline__ int cand_cap(int fanout) {
+  const float want = (float)fanout + 2.0f + 2.5f * sqrtf((float)fanout);
+  const int cap = ((int)ceilf(want + 3.5f * sqrtf(want)) + 3) & ~3;
+  return cap > 64 ? 64 : cap;
+}
+__device__ __forceinline__ uint32_t row_threshold(float wantf, uint32_t deg) {
+  const float fdeg = (float)deg;
+  return fdeg <= wantf ? 0xffffffffu
+                       : ((uint32_t)fminf(__fdividef(wantf, fdeg) * 4294967296.0f, 4294967040.0f) | 1u);
+}
 
-__global__ void __launch_bounds__(kTThreads)
-k_select_thread(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
-                SampleItems items, int32_t* __restrict__ src_global) {
-  extern __shared__ __align__(16) uint32_t s_list[];   // [cap]{z u32[kTThreads], x u16[kTThreads]}
-  const int n_items = plan->n_items, first = plan->n_warp_items;
+// Ranks the c candidates of the calling thread's list (entry s: key word at a0 + s*kCSlot, already
+// final and shifted) and returns the keep flags; *kept = their count.  c <= 64, c >= fanout.
+__device__ __forceinline__ unsigned long long rank_list(uint32_t a0, int c, int fanout, int* kept) {
+  const int c4 = (c + 3) & ~3;
+  for (int s = c; s < c4; ++s) sts_u32(a0 + s * kCSlot, 0xffffffffu);   // the list holds c4 <= cap entries
+  // the fanout-th smallest DISTINCT value, one round per rank: each round takes the minimum of
+  // (v - last - 1) mod 2^32, which orders the values above `last` before everything else
+  uint32_t lastp1 = 0, thr = 0;
+  bool wrapped = false;
+  for (int r = 0; r < fanout; ++r) {
+    wrapped = wrapped || (r > 0 && lastp1 == 0);
+    uint32_t best = 0xffffffffu;
+    for (int s = 0; s < c4; s += 4) {
+      const uint32_t w0 = lds_u32(a0 + s * kCSlot) - lastp1;
+      const uint32_t w1 = lds_u32(a0 + (s + 1) * kCSlot) - lastp1;
+      const uint32_t w2 = lds_u32(a0 + (s + 2) * kCSlot) - lastp1;
+      const uint32_t w3 = lds_u32(a0 + (s + 3) * kCSlot) - lastp1;
+      best = min(min(best, w0), min(w1, min(w2, w3)));
+    }
+    thr = best + lastp1;
+    lastp1 = thr + 1u;
+  }
+  // fewer than `fanout` distinct values or a tie at or below the threshold gives kept != fanout
+  unsigned long long keep = 0;
+  for (int i = 0; i < c; ++i) keep |= (unsigned long long)(lds_u32(a0 + i * kCSlot) <= thr) << i;
+  if (wrapped) keep = 0;
+  *kept = __popcll(keep);
+  return keep;
+}
+
+__global__ void __launch_bounds__(kCThreads)
+k_select_chunk(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
+               SampleItems items, int32_t* __restrict__ src_global) {
+  extern __shared__ __align__(16) uint32_t s_list[];   // [cap][kCThreads]{z, x}
+  __shared__ unsigned long long s_c0[kBins + 1];
+  for (int i = threadIdx.x; i <= kBins; i += kCThreads) s_c0[i] = plan->bin_chunk0[i];
+  __syncthreads();
+  const unsigned long long n_chunks = s_c0[kBins];
   const float wantf = want_candidates(fanout);
-  const int rshift = c_rank_shift;
-  const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(s_list) + threadIdx.x * 4;
-  const uint32_t ax0 = (uint32_t)__cvta_generic_to_shared(s_list) + kTThreads * 4 + threadIdx.x * 2;
-  const uint32_t a_lim4 = a0 + (uint32_t)(cap - 4) * kTSlot, a_lim1 = a0 + (uint32_t)(cap - 1) * kTSlot;
-  for (int q = first + blockIdx.x * kTThreads + threadIdx.x; q < n_items; q += gridDim.x * kTThreads) {
+  const int rshift = c_rank_shift, single_bins = c_single_bins;
+  const int lane = threadIdx.x & 31;
+  const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(s_list) + threadIdx.x * 8;
+  const uint32_t a_lim4 = a0 + (uint32_t)(cap - 4) * kCSlot, a_lim1 = a0 + (uint32_t)(cap - 1) * kCSlot;
+  for (;;) {
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(&plan->chunk_cursor, 32ull);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (base >= n_chunks) break;
+    // the bin of these 32 chunks (bins are padded to multiples of 32): largest o with s_c0[o] <= base
+    int lo = 0, hi = kBins;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (s_c0[mid] <= base) lo = mid; else hi = mid;
+    }
+    const int bin = kBins - 1 - lo;
+    const uint32_t nb = bin_chunks(bin, single_bins);
+    const uint32_t k = (uint32_t)(base - s_c0[lo]) + lane;      // chunk number inside the bin
+    const uint32_t r = k / nb, idx = k - r * nb;
+    if (r >= (uint32_t)plan->bin_count[bin]) continue;          // the bin's padding
+    const int q = plan->bin_start[bin] + (int)r;
     const uint64_t hdst = items.hdst[q];
     const uint32_t deg = items.deg[q];
-    const float fdeg = (float)deg;
-    const uint32_t M = fdeg <= wantf
-                           ? 0xffffffffu
-                           : ((uint32_t)fminf(__fdividef(wantf, fdeg) * 4294967296.0f, 4294967040.0f) | 1u);
-    uint32_t a = a0, ax = ax0;
-    uint64_t x = hdst + kGamma;
-    uint32_t n4 = deg >> 2;
-    while (n4 != 0 && a <= a_lim4) {
-      thread_step(x, M, a, ax);
-      thread_step(x + kGamma, M, a, ax);
-      thread_step(x + 2 * kGamma, M, a, ax);
-      thread_step(x + 3 * kGamma, M, a, ax);
-      x += 4 * kGamma;
-      --n4;
+    const uint32_t len = nb == 1 ? deg : ((deg + nb - 1) / nb + 3u) & ~3u;
+    const uint32_t j0 = idx * len;
+    const uint32_t j1 = min(j0 + len, deg);
+    const uint32_t M = row_threshold(wantf, deg);
+    uint32_t a = a0;
+    uint32_t rem = 0;
+    if (j0 < j1) {
+      uint64_t x = hdst + (uint64_t)(j0 + 1u) * kGamma;
+      uint32_t n4 = (j1 - j0) >> 2;
+      while (n4 != 0 && a <= a_lim4) {
+        chunk_step(x, M, a);
+        chunk_step(x + kGamma, M, a);
+        chunk_step(x + 2 * kGamma, M, a);
+        chunk_step(x + 3 * kGamma, M, a);
+        x += 4 * kGamma;
+        --n4;
+      }
+      rem = ((j1 - j0) & 3u) + 4u * n4;
+      while (rem != 0 && a <= a_lim1) {
+        chunk_step(x, M, a);
+        x += kGamma;
+        --rem;
+      }
     }
-    uint32_t rem = (deg & 3u) + 4u * n4;
-    while (rem != 0 && a <= a_lim1) {
-      thread_step(x, M, a, ax);
-      x += kGamma;
-      --rem;
+    const int c = (int)((a - a0) / kCSlot);
+    const uint32_t hlo = (uint32_t)hdst;
+    if (nb > 1) {
+      // one chunk of a longer row: hand the candidates to the row's list
+      int32_t* cnt = items.row_cnt + q;
+      if (rem != 0) {
+        atomicOr(cnt, 0x40000000);                     // lane list overflow: the row cannot be proved
+      } else if (c > 0) {
+        const int slot = atomicAdd(cnt, c);
+        uint2* dst = items.cand + (int64_t)q * cap;
+        for (int s = 0; s < c; ++s) {
+          if (slot + s >= cap) break;                  // the rank kernel sees the count and hands the row on
+          const uint32_t z = lds_u32(a0 + s * kCSlot);
+          dst[slot + s] = make_uint2(z, (lds_u32(a0 + s * kCSlot + 4) - hlo) * kGammaLoInv - 1u);
+        }
+      }
+      continue;
     }
-    const int c = (int)((a - a0) / kTSlot);
+    // a whole row: rank and emit
     int kept = -1;
     if (rem == 0 && c >= fanout) {
-      // final key word of every candidate; pad to a multiple of 4 with all-ones (cap is one)
       for (int s = 0; s < c; ++s) {
-        const uint32_t z = lds_u32(a0 + s * kTSlot);
-        sts_u32(a0 + s * kTSlot, (z ^ (z >> 31)) >> rshift);
+        const uint32_t z = lds_u32(a0 + s * kCSlot);
+        sts_u32(a0 + s * kCSlot, (z ^ (z >> 31)) >> rshift);
       }
-      const int c4 = (c + 3) & ~3;
-      for (int s = c; s < c4; ++s) sts_u32(a0 + s * kTSlot, 0xffffffffu);
-      // the fanout-th smallest DISTINCT value, one round per rank: each round takes the minimum
-      // of (v - last - 1) mod 2^32, which orders the values above `last` before everything else
-      uint32_t lastp1 = 0, thr = 0;
-      bool wrapped = false;
-      for (int r = 0; r < fanout; ++r) {
-        wrapped = wrapped || (r > 0 && lastp1 == 0);
-        uint32_t best = 0xffffffffu;
-        for (int s = 0; s < c4; s += 4) {
-          const uint32_t w0 = lds_u32(a0 + s * kTSlot) - lastp1;
-          const uint32_t w1 = lds_u32(a0 + (s + 1) * kTSlot) - lastp1;
-          const uint32_t w2 = lds_u32(a0 + (s + 2) * kTSlot) - lastp1;
-          const uint32_t w3 = lds_u32(a0 + (s + 3) * kTSlot) - lastp1;
-          best = min(min(best, w0), min(w1, min(w2, w3)));
-        }
-        thr = best + lastp1;
-        lastp1 = thr + 1u;
-      }
-      // keep flags (one bit per candidate, cap <= 64): fewer than `fanout` distinct values or a
-      // tie at or below the threshold gives kept != fanout
-      unsigned long long keep = 0;
-      for (int i = 0; i < c; ++i) keep |= (unsigned long long)(lds_u32(a0 + i * kTSlot) <= thr) << i;
-      if (wrapped) keep = 0;
-      kept = __popcll(keep);
+      unsigned long long keep = rank_list(a0, c, fanout, &kept);
       if (kept == fanout) {
-        const uint32_t hlo = (uint32_t)hdst;
         const int32_t* row = indices + items.row0[q];
         int32_t* out = src_global + items.out[q];
         for (int e = 0; e < fanout; ++e) {
           const int i = __ffsll((long long)keep) - 1;
           keep &= keep - 1;
-          const uint32_t pos = ((lds_u16(ax0 + i * kTSlot) - hlo) * kGammaLoInv - 1u) & 0xffffu;
+          const uint32_t pos = (lds_u32(a0 + i * kCSlot + 4) - hlo) * kGammaLoInv - 1u;
           out[e] = __ldg(row + pos);
         }
       }
     }
     if (kept != fanout) {
-      // list overflow, too few candidates under the threshold guess, or a high-word tie at the
-      // boundary: the warp kernel redoes the row (and overwrites whatever was written above)
       items.fallback[atomicAdd(&plan->n_fallback, 1)] = q;
       atomicAdd(&g_sampler_stat[3], 1ull);
     }
   }
 }
 
-// ---- one warp per row: bins with deg >= kThreadDeg (largest first), then the fallback list ----
+// ---- one thread per multi-chunk row: rank the row's candidate list, prove, emit ----------------
+// The list (<= cap entries of 8 bytes, written by the chunk kernel) is read straight from global
+// memory in every round: a thread's 100-odd bytes stay in L1 after the first touch, and without a
+// shared-memory copy the kernel runs at full occupancy, which is what hides the first touch.
+__global__ void __launch_bounds__(kCThreads)
+k_select_rank(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
+              SampleItems items, int32_t* __restrict__ src_global) {
+  const int n_multi = plan->n_multi;
+  const int rshift = c_rank_shift;
+  for (int q = plan->n_warp_items + blockIdx.x * kCThreads + threadIdx.x; q < n_multi; q += gridDim.x * kCThreads) {
+    const int c = items.row_cnt[q];
+    int kept = -1;
+    if (c >= fanout && c <= cap) {
+      const uint2* __restrict__ src = items.cand + (int64_t)q * cap;
+      // the fanout-th smallest DISTINCT key word (see rank_list)
+      uint32_t lastp1 = 0, thr = 0;
+      bool wrapped = false;
+      for (int r = 0; r < fanout; ++r) {
+        wrapped = wrapped || (r > 0 && lastp1 == 0);
+        uint32_t best = 0xffffffffu;
+        for (int s = 0; s < c; ++s) {
+          const uint32_t z = __ldg(&src[s].x);
+          best = min(best, ((z ^ (z >> 31)) >> rshift) - lastp1);
+        }
+        thr = best + lastp1;
+        lastp1 = thr + 1u;
+      }
+      unsigned long long keep = 0;
+      for (int i = 0; i < c; ++i) {
+        const uint32_t z = __ldg(&src[i].x);
+        keep |= (unsigned long long)(((z ^ (z >> 31)) >> rshift) <= thr) << i;
+      }
+      if (wrapped) keep = 0;
+      kept = __popcll(keep);
+      if (kept == fanout) {
+        // the lanes of a row append in any order: emit the kept positions ascending
+        const int32_t* row = indices + items.row0[q];
+        int32_t* out = src_global + items.out[q];
+        uint32_t lastq = 0;
+        for (int e = 0; e < fanout; ++e) {
+          uint32_t best = 0xffffffffu;
+          unsigned long long m = keep;
+          while (m) {
+            const int i = __ffsll((long long)m) - 1;
+            m &= m - 1;
+            const uint32_t p = __ldg(&src[i].y);
+            if (p >= lastq && p < best) best = p;
+          }
+          out[e] = __ldg(row + best);
+          lastq = best + 1u;
+        }
+      }
+    }
+    if (kept != fanout) {
+      items.fallback[atomicAdd(&plan->n_fallback, 1)] = q;
+      atomicAdd(&g_sampler_stat[3], 1ull);
+    }
+  }
+}
+
+// ---- one warp per row: the fallback list (and every keyed row when fanout > kChunkMaxFanout) ----
 __global__ void __launch_bounds__(kWarps * 32)
 k_select_warp(const int32_t* __restrict__ indices, int fanout, SamplePlan* __restrict__ plan,
               SampleItems items, int32_t* __restrict__ src_global) {
@@ -662,8 +838,8 @@ k_select_warp(const int32_t* __restrict__ indices, int fanout, SamplePlan* __res
 // Key evaluation and nothing else: every lane walks a register-resident SplitMix state and forms
 // the high word of fmix for each step (all the selection test reads), folded into one word so
 // the work stays alive.  No list stores, no row logic, no memory traffic.  FORM 0 is the
-// formulation of the product loops (key_zhi: mul.hi for the high-half shifts), FORM 1 uses plain
-// shifts; the reported peak is the better of the two.
+// formulation of the product loops (key_zhi), FORM 1 forms the high-half shifts with mul.hi; the
+// reported peak is the better of the two.
 template <int FORM>
 __global__ void __launch_bounds__(256) k_key_peak(uint64_t seed, int groups, uint32_t* __restrict__ fold) {
   uint64_t x = seed + (uint64_t)(blockIdx.x * 256 + threadIdx.x + 1) * 0x632BE59BD9B4E019ull;
@@ -675,12 +851,13 @@ __global__ void __launch_bounds__(256) k_key_peak(uint64_t seed, int groups, uin
       if (FORM == 0) {
         acc ^= key_zhi(xlo, xhi);
       } else {
-        uint32_t lo = xlo ^ __funnelshift_r(xlo, xhi, 30), hi = xhi ^ (xhi >> 30);
+        // round 1's formulation: the high-half shifts as mul.hi (FMA pipe)
+        uint32_t lo = xlo ^ __funnelshift_r(xlo, xhi, 30), hi = xhi ^ mulhi_u32(xhi, 1u << 2);
         const uint64_t p = (uint64_t)lo * kC1lo;
         hi = mad_lo_u32(lo, kC1hi, mad_lo_u32(hi, kC1lo, (uint32_t)(p >> 32)));
         lo = (uint32_t)p;
         lo ^= __funnelshift_r(lo, hi, 27);
-        hi ^= hi >> 27;
+        hi ^= mulhi_u32(hi, 1u << 5);
         acc ^= mulhi_u32(lo, kC2lo) + hi * kC2lo + lo * kC2hi;
       }
       x += kGamma;
@@ -735,6 +912,11 @@ cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, dou
 void sampler_stats(unsigned long long out[4]) {
   cudaMemcpyFromSymbol(out, g_sampler_stat, 4 * sizeof(unsigned long long));
 }
+cudaError_t sampler_tune(int single_bins, int warp_bin) {
+  cudaError_t e = cudaMemcpyToSymbol(c_single_bins, &single_bins, sizeof(int));
+  if (e != cudaSuccess) return e;
+  return cudaMemcpyToSymbol(c_warp_bin, &warp_bin, sizeof(int));
+}
 cudaError_t sampler_debug(int rank_shift, float want_add) {
   cudaError_t e = cudaMemcpyToSymbol(c_rank_shift, &rank_shift, sizeof(int));
   if (e != cudaSuccess) return e;
@@ -758,32 +940,32 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
   const int tiles = (max_nd + kTile - 1) / kTile;
   dim3 grid(tiles, W);
   SamplePlan* plan = static_cast<SamplePlan*>(wk.plan);
-  const bool thread_path = fanout <= kThreadMaxFanout;
-  const int min_warp_bin = thread_path ? 2 * kThreadDegLog2 : 0;
+  const bool chunk_path = fanout <= kChunkMaxFanout;
   cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
-  count_launches(thread_path ? 5 : 4);
+  count_launches(chunk_path ? 6 : 4);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
                                          cnt_tmp, cnt_pitch, tile_sums, plan);
-  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, min_warp_bin);
+  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, chunk_path ? 0 : 1);
   k_sample_plan<<<grid, kTile, 0, st>>>(indptr, indices, nodes, node_pitch, n_dst, dst_off, W,
                                         fanout, max_tiles, key_prefix_b, cnt_tmp, cnt_pitch,
                                         tile_sums, totals, blk_indptr, edge_off_out, src_global,
                                         plan, wk.items);
-  if (thread_path) {
-    // candidate list capacity: target + 4.5 sigma of a Poisson count, multiple of 4
-    const float want = (float)fanout + 2.0f + 2.5f * sqrtf((float)fanout);
-    const int cap = ((int)ceilf(want + 4.5f * sqrtf(want)) + 3) & ~3;
-    const size_t smem = (size_t)cap * kTSlot;
+  if (chunk_path) {
+    const int cap = cand_cap(fanout);
+    const size_t smem = (size_t)cap * kCSlot;
     static bool attr_set = false;
     if (!attr_set) {
-      cudaFuncSetAttribute(k_select_thread, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+      cudaFuncSetAttribute(k_select_chunk, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * (int)kCSlot);
       attr_set = true;
     }
-    int per_sm = (int)((220 * 1024) / (smem + 1024));
+    int per_sm = (int)((220 * 1024) / (smem + 2048));
     per_sm = per_sm < 1 ? 1 : (per_sm > 12 ? 12 : per_sm);
-    k_select_thread<<<sm_count() * per_sm, kTThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
+    k_select_chunk<<<sm_count() * per_sm, kCThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
+    k_select_rank<<<sm_count() * 16, kCThreads, 0, st>>>(indices, fanout, cap, plan, wk.items, src_global);
   }
   k_select_warp<<<sm_count() * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
 }
+
+int sample_cand_cap(int fanout) { return fanout <= kChunkMaxFanout ? cand_cap(fanout) : 0; }
 
 }  // namespace gg
