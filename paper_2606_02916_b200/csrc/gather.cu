@@ -38,29 +38,59 @@ __device__ __forceinline__ void st_stream(uint8_t* p, typename VecT<VEC>::type v
 }
 
 // Copies the tile's rows.  s_src[r] == nullptr means "skip row r".  If DENSE_DST the tile's
-// destination is one contiguous run starting at dst0.
+// destination is one contiguous run starting at dst0 (row pitch = rb).
+// One (sub-)warp per row: lane l of the row's group moves chunk l, l + lpr, ... of the row, so a row
+// costs one load and one store instruction per 32 chunks and no index arithmetic beyond the row
+// pointer -- round 1's flat chunk numbering spent ~50 warp instructions per row on a division per
+// chunk, which is what made the gather lose 40 % of its bandwidth beside the (issue-bound) sampler.
+// Rows narrower than 17 chunks share a warp (lpr = 16, 8, ...: two, four, ... rows per instruction).
+// UNROLL rows (or UNROLL chunks of a wide row) are in flight per lane before the first store.
 template <int VEC, bool DENSE_DST, int UNROLL = kUnroll>
 __device__ __forceinline__ void copy_tile(const uint8_t* const* s_src, uint8_t* const* s_dst,
-                                          uint8_t* dst0, int rows, int cpr /*chunks per row*/) {
-  const int total = rows * cpr;
-  for (int c0 = threadIdx.x; c0 < total; c0 += kThreads * UNROLL) {
-    typename VecT<VEC>::type v[UNROLL];
-    int row[UNROLL], col[UNROLL];
-    bool ok[UNROLL];
+                                          uint8_t* dst0, int rows, int rb) {
+  using V = typename VecT<VEC>::type;
+  const int cpr = rb / VEC;                       // chunks per row
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  constexpr int kWarpsPerCta = kThreads / 32;
+  if (cpr <= 32) {
+    int lpr = 32;                                 // lanes per row: smallest power of two >= cpr
+    while ((lpr >> 1) >= cpr) lpr >>= 1;
+    const int rpi = 32 / lpr;                     // rows per warp instruction
+    const int sub = lane / lpr, l = lane - sub * lpr;
+    const bool lane_on = l < cpr;
+    const int step = kWarpsPerCta * rpi;
+    for (int r0 = wid * rpi + sub; r0 < rows; r0 += step * UNROLL) {
+      V v[UNROLL];
+      bool ok[UNROLL];
 #pragma unroll
-    for (int k = 0; k < UNROLL; ++k) {
-      const int c = c0 + k * kThreads;
-      row[k] = c / cpr;
-      col[k] = c - row[k] * cpr;
-      ok[k] = c < total && s_src[row[k] < rows ? row[k] : 0] != nullptr;
-      if (ok[k]) v[k] = ld_stream<VEC>(s_src[row[k]] + (int64_t)col[k] * VEC);
+      for (int k = 0; k < UNROLL; ++k) {
+        const int r = r0 + k * step;
+        const uint8_t* src = r < rows ? s_src[r] : nullptr;
+        ok[k] = lane_on && src != nullptr;
+        if (ok[k]) v[k] = ld_stream<VEC>(src + (int64_t)l * VEC);
+      }
+#pragma unroll
+      for (int k = 0; k < UNROLL; ++k) {
+        if (ok[k]) {
+          const int r = r0 + k * step;
+          uint8_t* d = DENSE_DST ? dst0 + (int64_t)r * rb : s_dst[r];
+          st_stream<VEC>(d + (int64_t)l * VEC, v[k]);
+        }
+      }
     }
+  } else {
+    for (int r = wid; r < rows; r += kWarpsPerCta) {
+      const uint8_t* src = s_src[r];
+      if (src == nullptr) continue;
+      uint8_t* d = DENSE_DST ? dst0 + (int64_t)r * rb : s_dst[r];
+      for (int c0 = lane; c0 < cpr; c0 += 32 * UNROLL) {
+        V v[UNROLL];
 #pragma unroll
-    for (int k = 0; k < UNROLL; ++k) {
-      if (ok[k]) {
-        uint8_t* d = DENSE_DST ? dst0 + (int64_t)(c0 + k * kThreads) * VEC
-                               : s_dst[row[k]] + (int64_t)col[k] * VEC;
-        st_stream<VEC>(d, v[k]);
+        for (int k = 0; k < UNROLL; ++k)
+          if (c0 + 32 * k < cpr) v[k] = ld_stream<VEC>(src + (int64_t)(c0 + 32 * k) * VEC);
+#pragma unroll
+        for (int k = 0; k < UNROLL; ++k)
+          if (c0 + 32 * k < cpr) st_stream<VEC>(d + (int64_t)(c0 + 32 * k) * VEC, v[k]);
       }
     }
   }
@@ -135,7 +165,7 @@ __global__ void __launch_bounds__(kThreads) k_gather(GatherArgs A) {
     if (threadIdx.x == 32 && A.tile_miss) A.tile_miss[t] = s_w0miss + __popc(mm);
   }
   __syncthreads();
-  copy_tile<VEC, true>(s_src, nullptr, A.out + (int64_t)r0 * A.rb, rows, A.rb / VEC);
+  copy_tile<VEC, true>(s_src, nullptr, A.out + (int64_t)r0 * A.rb, rows, A.rb);
   if (threadIdx.x < 2 + A.R.P && s_cnt[threadIdx.x]) atomicAdd(A.counters + threadIdx.x, s_cnt[threadIdx.x]);
 }
 
@@ -303,7 +333,7 @@ __global__ void __launch_bounds__(kThreads) k_rows(RowsArgs A) {
     __syncthreads();
     // rows that come over the host link (MODE 1) keep twice as many loads in flight per thread:
     // a few CTAs then saturate PCIe and the rest of the GPU stays with the sampler
-    copy_tile<VEC, false, MODE == 1 ? 2 * kUnroll : kUnroll>(s_src, s_dst, nullptr, rows, A.rb / VEC);
+    copy_tile<VEC, false, MODE == 1 ? 2 * kUnroll : kUnroll>(s_src, s_dst, nullptr, rows, A.rb);
   }
 }
 

@@ -28,6 +28,8 @@
 //                    proves the result (kept == f) and emits it in ascending edge position
 //   k_select_warp    ONE WARP PER ROW for the rows the kernels above could not prove exact (and for
 //                    every keyed row when fanout > kChunkMaxFanout)
+#include <cstdlib>
+
 #include "common.cuh"
 #include "kernels.h"
 
@@ -960,10 +962,13 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
     }
     int per_sm = (int)((220 * 1024) / (smem + 2048));
     per_sm = per_sm < 1 ? 1 : (per_sm > 12 ? 12 : per_sm);
+    static int cap_chunk = getenv("GG_SAMP_CTAS_CHUNK") ? atoi(getenv("GG_SAMP_CTAS_CHUNK")) : 0;
+    if (cap_chunk > 0 && per_sm > cap_chunk) per_sm = cap_chunk;
     k_select_chunk<<<sm_count() * per_sm, kCThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
     k_select_rank<<<sm_count() * 16, kCThreads, 0, st>>>(indices, fanout, cap, plan, wk.items, src_global);
   }
-  k_select_warp<<<sm_count() * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
+  static int ctas_warp = getenv("GG_SAMP_CTAS_WARP") ? atoi(getenv("GG_SAMP_CTAS_WARP")) : 6;
+  k_select_warp<<<sm_count() * ctas_warp, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
 }
 
 int sample_cand_cap(int fanout) { return fanout <= kChunkMaxFanout ? cand_cap(fanout) : 0; }
