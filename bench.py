@@ -41,6 +41,7 @@ def parse_args():
                     help="windows staged ahead of the one being served (sampling runs that far ahead; "
                          "the cache is always built one window ahead)")
     ap.add_argument("--host-threads", type=int, default=0)
+    ap.add_argument("--cache-buffers", type=int, default=4, help="HBM cache buffers in rotation (gg_config.cache_buffers)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the W sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -288,7 +289,7 @@ def run_ours(args):
     sweep_ws = [] if args.no_sweep or world > 1 else [x for x in w.cfg["windows"] if x != W]
     g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
                                staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
-                               host_threads=args.host_threads)
+                               host_threads=args.host_threads, cache_buffers=args.cache_buffers)
     LA = args.lookahead
     # gathers run on a high-priority stream so their CTAs are scheduled ahead of the library's
     # (long-running, ALU-bound) sampling kernels whenever an SM has room for both
@@ -371,7 +372,7 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         return ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
                                       staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
-                                      host_threads=args.host_threads)
+                                      host_threads=args.host_threads, cache_buffers=args.cache_buffers)
 
     # ---- headline: device-resident inputs --------------------------------------------------
     if args.no_profile:
@@ -502,7 +503,7 @@ def run_ours(args):
             from paper_2606_02916_b200 import profiler
             cands = [p_["W"] for p_ in pts]
             gb = ep.graph_from_workload(w, n_hot=n_hot_b, carry_over=1, max_window=max(cands), staging_mode=args.staging_mode,
-                                        max_live_windows=LA + 1, host_threads=args.host_threads)
+                                        max_live_windows=LA + 1, host_threads=args.host_threads, cache_buffers=args.cache_buffers)
             try:
                 model = profiler.measure_energy_model(dev, w.row_bytes, P, local_part=rank % P)
                 model.pop("probes"), model.pop("p_active")
@@ -534,7 +535,7 @@ def run_ours(args):
             errors["simulator_budgeted"] = repr(exc)
         g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
                                    staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
-                                   host_threads=args.host_threads)
+                                   host_threads=args.host_threads, cache_buffers=args.cache_buffers)
 
     # ---- variant: epochs back to back with the cache carried over (reading S15: the cache
     # persists across epochs; the trace repeats), no reset and no drain between
@@ -576,41 +577,8 @@ def run_ours(args):
     # ---- NEXT-4: the same epoch with the paper's consumer behind every gather (Alg. 1 l.15): a
     # GraphSAGE-mean model, one layer per hop, 16 hidden units, 47 synthetic classes
     try:
-        if not args.no_sweep and world == 1 and w.dtype == torch.float32 and w.dim <= 128:
-            Lm = len(w.fanouts)
-            dims = [w.dim] + [16] * (Lm - 1) + [47]
-            rng = np.random.default_rng(7)
-            p0 = [dict(W_self=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
-                       W_neigh=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
-                       b=np.zeros(dims[l + 1], np.float32)) for l in range(Lm)]
-            model = binding.Sage(p0, dev)
-            labels = torch.randint(0, 47, (n_b, args.batch), dtype=torch.int32, device=dev)
-            losses = []
-
-            def train(k, j, bi, r):
-                model.step(r, labels[bi, :r["blocks"][0]["n_dst"]].contiguous(), 0.003, stream)
-
-            def epoch_c(wid0):
-                ep.run_epoch(g, batches, w.fanouts, W, feats, on_batch=train, stream=stream, first_window_id=wid0, lookahead=LA)
-                torch.cuda.synchronize(dev)
-                losses.append(float(model.loss.cpu()[0]))
-                g.cache_reset()
-            epoch_c(11 * 10 ** 6)
-            g.profile_enable(True)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            for e in range(3):
-                epoch_c(11 * 10 ** 6 + 1000 * (e + 1))
-            b.record(stream)
-            torch.cuda.synchronize(dev)
-            stall_c = g.profile_get()["wait"]["ms"] / 3
-            g.profile_enable(False)
-            variants["with_graphsage_consumer"] = {
-                "value": 3 * n_b / (a.elapsed_time(b) * 1e-3), "unit": UNIT, "model": "GraphSAGE-mean, dims %s, SGD lr 0.003" % dims,
-                "gpu_stall_ms_per_epoch": stall_c,
-                "last_batch_loss_per_epoch": losses,
-                "note": "forward + loss + backward + update of every mini-batch on the caller's stream right behind its gather"}
-            model.close()
+        if not args.no_sweep and world == 1 and w.dtype == torch.float32 and w.dim <= 1024:
+            variants["with_graphsage_consumer"] = consumer_leg(g, w, batches, W, feats, stream, dev, LA, args.batch)
     except Exception as exc:      # an optional leg must not cost the headline line
         errors['consumer'] = repr(exc)
         g = recover_graph(g)
@@ -724,6 +692,49 @@ def run_ours(args):
     g.close()
 
 
+def consumer_leg(g, w, batches, W, feats, stream, dev, LA, batch):
+    """One warm + three timed epochs with forward + loss + backward + SGD of every mini-batch on the
+    caller's stream right behind its gather (gg_sage_step)."""
+    from paper_2606_02916_b200 import epoch as ep, binding
+    n_b = len(batches)
+    Lm = len(w.fanouts)
+    dims = [w.dim] + [16] * (Lm - 1) + [47]
+    rng = np.random.default_rng(7)
+    p0 = [dict(W_self=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
+               W_neigh=(rng.uniform(-1, 1, (dims[l], dims[l + 1])) / np.sqrt(dims[l])).astype(np.float32),
+               b=np.zeros(dims[l + 1], np.float32)) for l in range(Lm)]
+    model = binding.Sage(p0, dev)
+    labels = torch.randint(0, 47, (n_b, batch), dtype=torch.int32, device=dev)
+    losses = []
+
+    def train(k, j, bi, r):
+        model.step(r, labels[bi, :r["blocks"][0]["n_dst"]].contiguous(), 0.003, stream)
+
+    def epoch_c(wid0):
+        ep.run_epoch(g, batches, w.fanouts, W, feats, on_batch=train, stream=stream, first_window_id=wid0, lookahead=LA)
+        torch.cuda.synchronize(dev)
+        losses.append(float(model.loss.cpu()[0]))
+        g.cache_reset()
+
+    try:
+        epoch_c(11 * 10 ** 6)
+        g.profile_enable(True)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for e in range(3):
+            epoch_c(11 * 10 ** 6 + 1000 * (e + 1))
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        stall_c = g.profile_get()["wait"]["ms"] / 3
+        g.profile_enable(False)
+    finally:
+        model.close()
+    return {"value": 3 * n_b / (a.elapsed_time(b) * 1e-3), "unit": UNIT, "W": W,
+            "model": "GraphSAGE-mean, dims %s, SGD lr 0.003" % dims, "gpu_stall_ms_per_epoch": stall_c,
+            "last_batch_loss_per_epoch": losses,
+            "note": "forward + loss + backward + update of every mini-batch on the caller's stream right behind its gather"}
+
+
 def edge_cut(w, dev):
     """Measured fraction of CSR entries whose two endpoints lie in different owner ranges."""
     po = torch.as_tensor(np.asarray(w.part_offsets[1:-1], dtype=np.int32), device=dev)
@@ -751,7 +762,7 @@ def measure_point(ctx, w, batches, W, n_hot, K=2, warm=1, max_batch=None, g=None
     own = g is None
     if own:
         g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=1, max_window=max_window, staging_mode=args.staging_mode,
-                                   max_live_windows=LA + 1, host_threads=args.host_threads,
+                                   max_live_windows=LA + 1, host_threads=args.host_threads, cache_buffers=args.cache_buffers,
                                    max_batch=max_batch or max(len(b) for b in batches))
     n_b = len(batches)
     try:
@@ -864,7 +875,7 @@ def configs_grid(ctx, w_products, batches_products, errors, t_budget_s):
         for Bx in (1024, 2048, 4096):
             bx = batches_products if Bx == args.batch else [all_seeds[i:i + Bx] for i in range(0, len(all_seeds), Bx)]
             g = ep.graph_from_workload(w, n_hot=-1, carry_over=1, max_window=32, staging_mode=args.staging_mode,
-                                       max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, max_batch=Bx)
+                                       max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, max_batch=Bx, cache_buffers=args.cache_buffers)
             try:
                 for Wx in w.cfg["windows"]:
                     pts.append(measure_point(ctx, w, bx, Wx, -1, K=2, warm=1, g=g))
@@ -878,7 +889,7 @@ def configs_grid(ctx, w_products, batches_products, errors, t_budget_s):
         n_hot = -(-n_remote_nodes // 10)
         pts = []
         g = ep.graph_from_workload(w, n_hot=n_hot, carry_over=1, max_window=32, staging_mode=args.staging_mode,
-                                   max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, max_batch=args.batch)
+                                   max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, max_batch=args.batch, cache_buffers=args.cache_buffers)
         try:
             for Wx in w.cfg["windows"]:
                 pts.append(measure_point(ctx, w, batches_products, Wx, n_hot, K=5, warm=1, g=g))
@@ -909,7 +920,7 @@ def configs_grid(ctx, w_products, batches_products, errors, t_budget_s):
             for n_hot in (-1, -(-n_rem // 10)):
                 g = ep.graph_from_workload(wx, n_hot=n_hot, carry_over=1, max_window=max(wx.cfg["windows"]),
                                            staging_mode=args.staging_mode, max_live_windows=ctx["LA"] + 1,
-                                           host_threads=args.host_threads)
+                                           host_threads=args.host_threads, cache_buffers=args.cache_buffers)
                 try:
                     for Wx in wx.cfg["windows"]:
                         if n_hot >= 0 and Wx != max(wx.cfg["windows"]):
@@ -920,6 +931,20 @@ def configs_grid(ctx, w_products, batches_products, errors, t_budget_s):
                     g.close()
             out[name] = {"workload": workload_name(argparse.Namespace(config=name, batch=wx.cfg["batch"]), wx),
                          "edge_cut_measured": cut, "generation_s": t_gen, "points": pts}
+            if name == "dense":
+                # the paper's own model shape on its Reddit-shaped workload: 2 layers, 16 hidden
+                # units, fanout {25,10}, 602-wide features, trained behind every gather
+                try:
+                    Wc = max(wx.cfg["windows"])
+                    g = ep.graph_from_workload(wx, n_hot=-1, carry_over=1, max_window=Wc, staging_mode=args.staging_mode,
+                                               max_live_windows=ctx["LA"] + 1, host_threads=args.host_threads, cache_buffers=args.cache_buffers)
+                    try:
+                        out[name]["with_graphsage_consumer"] = consumer_leg(g, wx, wx.batches, Wc, ctx["feats"], ctx["stream"], dev,
+                                                                            ctx["LA"], wx.cfg["batch"])
+                    finally:
+                        g.close()
+                except Exception as exc:
+                    errors["configs.dense.consumer"] = repr(exc)
             del wx
             ctx["feats"] = None
             torch.cuda.empty_cache()

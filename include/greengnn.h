@@ -114,7 +114,8 @@ typedef struct {
                              memory (e.g. a peer GPU's HBM) is served by the pull kernel instead,
                              since host threads cannot read it;
                              1 = one GPU-initiated pull kernel per owner reading the pinned store */
-  int32_t host_threads;   /* owner-service pack threads; <= 0 = min(16, hardware threads) */
+  int32_t host_threads;   /* owner-service pack threads; <= 0 = 0.4 x hardware threads (in [2, 16]): the pack shares
+                             the host's DRAM with the DMA reads of the bulk copies, see csrc/api.cu */
   int32_t cache_buffers;  /* HBM cache buffers (+ slot maps) in rotation, window k uses k mod n.  2 = the
                              ping-pong a literal Alg. 1 needs; with 2, window k's hot set can only be
                              selected after window k-2's gathers have finished, and that chain
@@ -384,7 +385,8 @@ gg_status gg_rank_calibrate(const double* z, const double* e_gt, int32_t n, int3
  * layer l consumes block num_layers-1-l (layer 0 reads the feature tensor X_b); the loss is the mean
  * softmax cross-entropy of the seeds against `labels`; parameters move by plain SGD (no dropout:
  * DESIGN.md reading S27).  dims: host [num_layers+1], dims[0] = feature dim (features must be
- * GG_F32), dims[num_layers] = classes; 1 <= dims[l] <= 128 for l < num_layers, dims[l+1] <= 64.
+ * GG_F32), dims[num_layers] = classes; 1 <= dims[l] <= 128 for l < num_layers, dims[l+1] <= 64;
+ * dims[0] may be up to 1024 when dims[1] <= 16 (the paper's 602-wide features into 16 hidden units).
  * w_self / w_neigh / bias: host arrays of num_layers pointers to row-major [dims[l]][dims[l+1]] /
  * [dims[l+1]] initial values (copied). */
 typedef struct gg_sage gg_sage;

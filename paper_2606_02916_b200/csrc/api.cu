@@ -602,16 +602,18 @@ static gg_status stage_a(gg_graph* g, Window* w) {
 
 // Owner-service pack of rows [i0, i1): response row i <- store row of ids[i].  Destination rows
 // are written with non-temporal stores (no read-for-ownership of a buffer the CPU never reads
-// again: the DMA engine is its only consumer) and the next source rows are prefetched, since
-// the requested IDs scatter over the owner's store.
+// again: the DMA engine is its only consumer; plain stores measured 1.7x slower) and the source
+// rows are prefetched into L2 two dozen rows ahead: the requested IDs scatter over the owner's
+// store, a core's ten line-fill buffers hold barely two 400-byte rows, the L2's queue far more
+// (products epoch on the 16-core box: pack 39.9 -> 32.6 ms with 16 threads).
 static void pack_rows(uint8_t* resp, const uint8_t* base, const int32_t* ids, int64_t lo, int64_t stride,
                       int64_t rb, int64_t i0, int64_t i1) {
   const bool nt = (rb % 16 == 0) && (((uintptr_t)resp) % 16 == 0);
-  const int64_t ahead = 6;
+  const int64_t ahead = 24;
   for (int64_t i = i0; i < i1; ++i) {
     if (i + ahead < i1) {
       const uint8_t* nx = base + (ids[i + ahead] - lo) * stride;
-      for (int64_t k = 0; k < rb; k += 64) _mm_prefetch((const char*)(nx + k), _MM_HINT_T0);
+      for (int64_t k = 0; k < rb; k += 64) _mm_prefetch((const char*)(nx + k), _MM_HINT_T1);
     }
     const uint8_t* src = base + (ids[i] - lo) * stride;
     uint8_t* dst = resp + i * rb;
@@ -1119,7 +1121,12 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   }
   CUC(cudaDeviceSynchronize());
 #undef CUC
-  int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(1u, std::thread::hardware_concurrency()));
+  // The pack and the DMA reads of the bulk copies share the host's DRAM: more pack threads finish a
+  // window's pack sooner but slow the copies it overlaps with (products W=16 on the 16-core box,
+  // threads -> copies GB/s / epoch ms: 4 -> 54.4 / 53.2, 6 -> 52.1 / 45.9, 8 -> 47.8 / 46.5, 16 -> 45.8 /
+  // 48.0).  Default: 0.4 x the hardware threads, where pack time and copy time of a window meet.
+  const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+  int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(2u, (hw * 2u + 2u) / 5u));
   g->pool = new Pool(nt > 1 ? nt : 0);
   g->worker_a = std::thread(worker_a_main, g);
   g->worker_b = std::thread(worker_b_main, g);

@@ -25,6 +25,7 @@ namespace gg {
 constexpr int kSageWarps = 8;
 constexpr int kSlotsIn = 4;    // columns per lane, input side  (dims <= 128)
 constexpr int kSlotsOut = 2;   // columns per lane, output side (dims <= 64)
+constexpr int kSageMaxFeatureDim = 1024;   // first layer's input, walked in slabs of 128 columns
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -51,12 +52,13 @@ k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
            const float* __restrict__ w_self, const float* __restrict__ w_neigh,
            const float* __restrict__ bias, float* __restrict__ agg_out, float* __restrict__ h_out) {
   extern __shared__ float s_w[];   // two weight matrices (layout below), then [dout] bias
-  float* ws = s_w;
-  float* wn = s_w + 17 * din + dout * din;   // room for either layout
-  float* sb = wn + 17 * din + dout * din;
   // dout <= 16: rows of 17 floats per input column ([c][17]: odd pitch, lane-consecutive columns hit
   // distinct banks and output o is an immediate offset); otherwise transposed [o][din]
   const bool narrow = dout <= 16;
+  const int wsize = narrow ? 17 * din : dout * din;
+  float* ws = s_w;
+  float* wn = s_w + wsize;
+  float* sb = wn + wsize;
   for (int k = threadIdx.x; k < din * dout; k += blockDim.x) {
     const int c = k / dout, o = k - c * dout;
     const int at = narrow ? c * 17 + o : o * din + c;
@@ -67,56 +69,64 @@ k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   for (int i = blockIdx.x * kSageWarps + wid; i < n_dst; i += gridDim.x * kSageWarps) {
-    float xs[kSlotsIn], ac[kSlotsIn];
-#pragma unroll
-    for (int s = 0; s < kSlotsIn; ++s) {
-      const int c = lane + 32 * s;
-      xs[s] = c < din ? h_in[(int64_t)i * din + c] : 0.0f;
-      ac[s] = 0.0f;
-    }
     const int e0 = indptr[i], e1 = indptr[i + 1];
-    for (int eb = e0; eb < e1; eb += 32) {
-      // 32 neighbor ids at a time, then their rows back to back (independent loads)
-      const int mine = eb + lane < e1 ? __ldg(src_local + eb + lane) : 0;
-      const int cnt = min(32, e1 - eb);
-#pragma unroll 4
-      for (int q = 0; q < cnt; ++q) {
-        const int64_t src = __shfl_sync(0xffffffffu, mine, q);
-#pragma unroll
-        for (int s = 0; s < kSlotsIn; ++s) {
-          const int c = lane + 32 * s;
-          if (c < din) ac[s] += __ldg(h_in + src * din + c);
-        }
-      }
-    }
     const float deg = (float)(e1 - e0);
+    float p[16];
 #pragma unroll
-    for (int s = 0; s < kSlotsIn; ++s) {
-      const int c = lane + 32 * s;
-      ac[s] = (e1 > e0 && c < din) ? ac[s] / deg : 0.0f;
-      if (c < din) agg_out[(int64_t)i * din + c] = ac[s];
-    }
-    if (dout <= 16) {
-      // 16 partial sums per lane, reduced across the warp by a halving butterfly: 8+4+2+1+1
-      // shuffles instead of 16 x 5 (the per-output warp_sum made this kernel shuffle-bound)
-      float p[16];
-      const float* wsp[kSlotsIn];   // column clamped into the row: xs / ac are 0 beyond din, so no predicate is needed
-      const float* wnp[kSlotsIn];
+    for (int o = 0; o < 16; ++o) p[o] = 0.0f;
+    float xs[kSlotsIn], ac[kSlotsIn];
+    // input columns in slabs of 128 (4 per lane); a feature row wider than 128 (the paper's Reddit
+    // shape, 602) walks the row's neighbor list once per slab and keeps the 16 partial outputs
+    for (int c0 = 0; c0 < din; c0 += 32 * kSlotsIn) {
 #pragma unroll
       for (int s = 0; s < kSlotsIn; ++s) {
-        const int cc = min(lane + 32 * s, din - 1);
-        wsp[s] = ws + cc * 17;
-        wnp[s] = wn + cc * 17;
+        const int c = c0 + lane + 32 * s;
+        xs[s] = c < din ? h_in[(int64_t)i * din + c] : 0.0f;
+        ac[s] = 0.0f;
       }
+      for (int eb = e0; eb < e1; eb += 32) {
+        // 32 neighbor ids at a time, then their rows back to back (independent loads)
+        const int mine = eb + lane < e1 ? __ldg(src_local + eb + lane) : 0;
+        const int cnt = min(32, e1 - eb);
+#pragma unroll 4
+        for (int q = 0; q < cnt; ++q) {
+          const int64_t src = __shfl_sync(0xffffffffu, mine, q);
 #pragma unroll
-      for (int o = 0; o < 16; ++o) {
-        float v = 0.0f;
-        if (o < dout) {      // warp-uniform
-#pragma unroll
-          for (int s = 0; s < kSlotsIn; ++s) v = fmaf(xs[s], wsp[s][o], fmaf(ac[s], wnp[s][o], v));
+          for (int s = 0; s < kSlotsIn; ++s) {
+            const int c = c0 + lane + 32 * s;
+            if (c < din) ac[s] += __ldg(h_in + src * din + c);
+          }
         }
-        p[o] = v;
       }
+#pragma unroll
+      for (int s = 0; s < kSlotsIn; ++s) {
+        const int c = c0 + lane + 32 * s;
+        ac[s] = (e1 > e0 && c < din) ? ac[s] / deg : 0.0f;
+        if (c < din) agg_out[(int64_t)i * din + c] = ac[s];
+      }
+      if (narrow) {
+        const float* wsp[kSlotsIn];   // column clamped into the row: xs / ac are 0 beyond din, so no predicate is needed
+        const float* wnp[kSlotsIn];
+#pragma unroll
+        for (int s = 0; s < kSlotsIn; ++s) {
+          const int cc = min(c0 + lane + 32 * s, din - 1);
+          wsp[s] = ws + cc * 17;
+          wnp[s] = wn + cc * 17;
+        }
+#pragma unroll
+        for (int o = 0; o < 16; ++o) {
+          if (o < dout) {      // warp-uniform
+            float v = p[o];
+#pragma unroll
+            for (int s = 0; s < kSlotsIn; ++s) v = fmaf(xs[s], wsp[s][o], fmaf(ac[s], wnp[s][o], v));
+            p[o] = v;
+          }
+        }
+      }
+    }
+    if (narrow) {
+      // 16 partial sums per lane, reduced across the warp by a halving butterfly: 8+4+2+1+1
+      // shuffles instead of 16 x 5 (the per-output warp_sum made this kernel shuffle-bound)
       bfly<8, 16>(p, lane);
       bfly<4, 8>(p, lane);
       bfly<2, 4>(p, lane);
@@ -128,16 +138,17 @@ k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
         h_out[(int64_t)i * dout + o] = RELU ? fmaxf(v, 0.0f) : v;
       }
     } else {
+      // wider outputs: din <= 128 (one slab, checked at create), xs / ac hold the whole row
       float keep[kSlotsOut] = {0.0f, 0.0f};
       for (int o = 0; o < dout; ++o) {
-        float p = 0.0f;
+        float q = 0.0f;
 #pragma unroll
         for (int s = 0; s < kSlotsIn; ++s) {
           const int c = lane + 32 * s;
-          if (c < din) p += xs[s] * ws[o * din + c] + ac[s] * wn[o * din + c];
+          if (c < din) q += xs[s] * ws[o * din + c] + ac[s] * wn[o * din + c];
         }
-        p = warp_sum(p);
-        if (lane == (o & 31)) keep[o >> 5] = p + sb[o];
+        q = warp_sum(q);
+        if (lane == (o & 31)) keep[o >> 5] = q + sb[o];
       }
 #pragma unroll
       for (int t = 0; t < kSlotsOut; ++t) {
@@ -290,7 +301,7 @@ k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, cons
              const float* __restrict__ d_out, int n_dst, int din, int dout, int tile_rows,
              float* __restrict__ part /* [gridDim.x][2*din*dout + dout] per-CTA partial sums */) {
   __shared__ float sg[kWgRows][2 * OH];
-  const int c = threadIdx.x & 127, half = threadIdx.x >> 7;
+  const int c = (threadIdx.x & 127) + 128 * blockIdx.y, half = threadIdx.x >> 7;   // blockIdx.y: slab of 128 input columns
   float a_s[OH], a_n[OH];
 #pragma unroll
   for (int k = 0; k < OH; ++k) a_s[k] = a_n[k] = 0.0f;
@@ -309,7 +320,7 @@ k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, cons
       sg[r][o] = v;
     }
     __syncthreads();
-    if ((int)threadIdx.x < 2 * OH)
+    if ((int)threadIdx.x < 2 * OH && blockIdx.y == 0)
       for (int r = 0; r < rows; ++r) a_b += sg[r][threadIdx.x];
     if (c < din) {
 #pragma unroll 4
@@ -335,7 +346,7 @@ k_sage_wgrad(const float* __restrict__ h_in, const float* __restrict__ agg, cons
       }
     }
   }
-  if ((int)threadIdx.x < 2 * OH && (int)threadIdx.x < dout) mine[2 * din * dout + threadIdx.x] = a_b;
+  if ((int)threadIdx.x < 2 * OH && (int)threadIdx.x < dout && blockIdx.y == 0) mine[2 * din * dout + threadIdx.x] = a_b;
 }
 
 // grads[k] += sum over the CTAs' partials in a fixed order (8 interleaved slices, then the slices
@@ -368,9 +379,10 @@ static void launch_wgrad(cudaStream_t st, const float* h_in, const float* agg, c
   int grid = (n_dst + tile_rows - 1) / tile_rows;
   const int gmax = std::min(kWgMaxGrid, sm_count() * 4);
   grid = grid < 1 ? 1 : (grid > gmax ? gmax : grid);
-  if (dout <= 16) k_sage_wgrad<RELU, 8><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
-  else if (dout <= 48) k_sage_wgrad<RELU, 24><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
-  else k_sage_wgrad<RELU, 32><<<grid, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
+  const dim3 g2(grid, (din + 127) / 128);
+  if (dout <= 16) k_sage_wgrad<RELU, 8><<<g2, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
+  else if (dout <= 48) k_sage_wgrad<RELU, 24><<<g2, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
+  else k_sage_wgrad<RELU, 32><<<g2, 256, 0, st>>>(h_in, agg, h_out, d_out, n_dst, din, dout, tile_rows, part);
   const int P = 2 * din * dout + dout;
   k_sage_wreduce<<<(P + 31) / 32, 256, 0, st>>>(part, grid, P, grads_layer);
 }
@@ -444,9 +456,15 @@ gg_status gg_sage_create(int32_t L, const int32_t* dims, const float* const* w_s
   if (!dims || !w_self || !w_neigh || !bias || !out) return report_error(GG_ERR_INVALID_ARG, "null argument");
   *out = nullptr;
   if (L < 1 || L > GG_MAX_LAYERS) return report_error(GG_ERR_INVALID_ARG, "num_layers out of range");
-  for (int l = 0; l < L; ++l)
-    if (dims[l] < 1 || dims[l] > 32 * kSlotsIn || dims[l + 1] < 1 || dims[l + 1] > 32 * kSlotsOut)
-      return report_error(GG_ERR_INVALID_ARG, "dims: inputs must be in [1,128], outputs in [1,64]");
+  for (int l = 0; l < L; ++l) {
+    if (dims[l] < 1 || dims[l + 1] < 1 || dims[l + 1] > 32 * kSlotsOut)
+      return report_error(GG_ERR_INVALID_ARG, "dims: outputs must be in [1,64]");
+    // a layer's input is walked in slabs of 128 columns when its output is at most 16 wide (the
+    // paper's 16 hidden units); only the first layer (the feature tensor) may be wider than 128
+    const int max_in = (l == 0 && dims[1] <= 16) ? kSageMaxFeatureDim : 32 * kSlotsIn;
+    if (dims[l] > max_in)
+      return report_error(GG_ERR_INVALID_ARG, "dims: layer inputs must be in [1,128] (the feature dim up to 1024 when dims[1] <= 16)");
+  }
   gg_sage* m = new gg_sage();
   m->L = L;
   for (int l = 0; l <= L; ++l) m->dims[l] = dims[l];
@@ -524,7 +542,7 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
   for (int l = 0; l < L; ++l) {
     const gg_block& b = batch->blocks[L - 1 - l];
     const int din = m->dims[l], dout = m->dims[l + 1];
-    const size_t smem = (size_t)(2 * (17 * din + din * dout) + dout) * sizeof(float);
+    const size_t smem = (size_t)(2 * (dout <= 16 ? 17 * din : din * dout) + dout) * sizeof(float);
     if (l < L - 1)
       k_sage_fwd<true><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h, b.indptr, b.src_local, b.n_dst, din, dout,
           p_self(m, l, m->params), p_neigh(m, l, m->params), p_bias(m, l, m->params), m->agg[l].p, m->out[l].p);

@@ -75,6 +75,14 @@ def test_products_mini_three_layers(workload, dev):
     run(workload("products_mini", dev), dev, hidden=16, classes=47, W=4, steps=3, lr=0.03)
 
 
+def test_dense_mini_paper_model_shape_dim_602(workload, dev):
+    """The paper's own model shape: 2 layers, 16 hidden units, fanout {25,10} over
+    602-wide features (the Reddit-shaped config): layer 0 walks the feature row in slabs of 128."""
+    w = workload("dense_mini", dev)
+    assert w.dim == 602 and w.fanouts == [25, 10]
+    run(w, dev, hidden=16, classes=41, W=4, steps=3, lr=0.02)
+
+
 def test_consumer_without_host_sync_matches_synced_run(workload, dev):
     """gg_window_release(stream) orders the arena's reuse behind the consumer's work: a run that
     never synchronises the host between a batch's training step and the release (arenas =
@@ -118,6 +126,10 @@ def test_consumer_without_host_sync_matches_synced_run(workload, dev):
 def test_sage_errors(workload, dev):
     from paper_2606_02916_b200 import binding
     with pytest.raises(binding.GreenGNNError):
-        binding.Sage(init_params([200, 16, 4], 0), dev)          # input dim > 128
+        binding.Sage(init_params([200, 32, 4], 0), dev)          # feature dim > 128 into more than 16 hidden units
+    with pytest.raises(binding.GreenGNNError):
+        binding.Sage(init_params([64, 200, 16, 4], 0), dev)      # a hidden layer's input > 128
+    with pytest.raises(binding.GreenGNNError):
+        binding.Sage(init_params([2000, 16, 4], 0), dev)         # feature dim > 1024
     with pytest.raises(binding.GreenGNNError):
         binding.Sage(init_params([32, 100, 4], 0), dev)          # hidden dim > 64
