@@ -66,7 +66,7 @@ static double now_ms() {
 class Pool {
  public:
   explicit Pool(int n) : stop_(false), gen_(0), pending_(0) {
-    for (int i = 0; i < n; ++i) th_.emplace_back([this] { run(); });
+    for (int i = 0; i < n; ++i) th_.emplace_back([this, i] { run(i); });
   }
   ~Pool() {
     {
@@ -76,10 +76,11 @@ class Pool {
     cv_.notify_all();
     for (auto& t : th_) t.join();
   }
-  // fn(chunk) for chunk in [0, n); returns when all are done
-  void parallel_for(int64_t n, const std::function<void(int64_t)>& fn) {
+  int size() const { return (int)th_.size(); }
+  // fn(chunk) for chunk in [0, n) on at most `limit` of the pool's threads; returns when all are done
+  void parallel_for(int64_t n, const std::function<void(int64_t)>& fn, int limit = 1 << 30) {
     if (n <= 0) return;
-    if (th_.empty() || n == 1) {
+    if (th_.empty() || n == 1 || limit <= 1) {
       for (int64_t i = 0; i < n; ++i) fn(i);
       return;
     }
@@ -87,6 +88,7 @@ class Pool {
       std::lock_guard<std::mutex> l(m_);
       fn_ = &fn;
       n_ = n;
+      limit_ = limit;
       next_.store(0);
       pending_ = (int)th_.size();
       ++gen_;
@@ -97,7 +99,7 @@ class Pool {
   }
 
  private:
-  void run() {
+  void run(int index) {
     uint64_t seen = 0;
     for (;;) {
       const std::function<void(int64_t)>* fn;
@@ -108,9 +110,9 @@ class Pool {
         if (stop_) return;
         seen = gen_;
         fn = fn_;
-        n = n_;
+        n = index < limit_ ? n_ : 0;      // threads beyond the call's limit sit this one out
       }
-      for (;;) {
+      while (n > 0) {
         const int64_t i = next_.fetch_add(1);
         if (i >= n) break;
         (*fn)(i);
@@ -125,6 +127,7 @@ class Pool {
   bool stop_;
   uint64_t gen_;
   int pending_;
+  int limit_ = 1 << 30;
   const std::function<void(int64_t)>* fn_ = nullptr;
   int64_t n_ = 0;
   std::atomic<int64_t> next_{0};
@@ -335,6 +338,10 @@ struct gg_graph {
   int busy = 0;                   // jobs queued or in flight
   bool stop = false;
   Pool* pool = nullptr;
+  int pack_threads_busy = 1;      // pack threads while bulk copies are in flight (they share the host's DRAM)
+  // bulk copies issued on stream C and not yet known to be complete: (end event, bytes), oldest first
+  std::deque<std::pair<cudaEvent_t, int64_t>> link_q;
+  std::vector<cudaEvent_t> link_ev_pool;
 };
 
 namespace gg {
@@ -769,15 +776,35 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
       const int32_t* ids = w->h_req + q0;
       uint8_t* resp = g->h_resp[ri] + q0 * rb;
       const int64_t chunk = 512;
+      // every pool thread while the link is idle (the cold first window: nothing to contend with, and
+      // the first copy cannot start before this pack ends), the tuned few while copies are in flight
+      // Pack threads: the tuned few while the link has more bytes queued than this pack produces (the
+      // copies are what the epoch waits for; fewer threads leave them the host's DRAM), every pool
+      // thread when the link is about to run dry (the cold first window, small windows).
+      while (!g->link_q.empty() && cudaEventQuery(g->link_q.front().first) == cudaSuccess) {
+        g->link_ev_pool.push_back(g->link_q.front().first);
+        g->link_q.pop_front();
+      }
+      cudaGetLastError();
+      int64_t queued = 0;
+      for (auto& e : g->link_q) queued += e.second;
+      const bool link_fed = queued >= nm * rb + nm * rb / 2;
       g->pool->parallel_for(ceil_div(nm, chunk), [&](int64_t c) {
         pack_rows(resp, base, ids, lo, stride, rb, c * chunk, std::min(nm, (c + 1) * chunk));
-      });
+      }, link_fed ? g->pack_threads_busy : g->pool->size());
       w->ms_pack += (float)(now_ms() - p0);
       tl("pack_done", w->id, now_ms() - p0);
       cudaEvent_t pe = g->prof.begin(sc);
       CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies], sc));
       CU(cudaMemcpyAsync(cs->cache + q0 * rb, resp, (size_t)(nm * rb), cudaMemcpyHostToDevice, sc));
       CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies + 1], sc));
+      {
+        cudaEvent_t le = nullptr;
+        if (!g->link_ev_pool.empty()) { le = g->link_ev_pool.back(); g->link_ev_pool.pop_back(); }
+        else CU(cudaEventCreateWithFlags(&le, cudaEventDisableTiming));
+        CU(cudaEventRecord(le, sc));
+        g->link_q.emplace_back(le, nm * rb);
+      }
       g->prof.end(sc, pe, GG_PROF_STAGE_COPY, nm * rb);
       w->bulk_copies += 1;
       q0 += nm;
@@ -986,6 +1013,8 @@ gg_status gg_graph_destroy(gg_graph* g) {
     if (g->h_resp[i]) cudaFreeHost(g->h_resp[i]);
     if (g->resp_free[i]) cudaEventDestroy(g->resp_free[i]);
   }
+  for (auto& e : g->link_q) cudaEventDestroy(e.first);
+  for (auto e : g->link_ev_pool) cudaEventDestroy(e);
   if (g->h_seeds) cudaFreeHost(g->h_seeds);
   if (g->h_kp) cudaFreeHost(g->h_kp);
   if (g->side) cudaStreamDestroy(g->side);
@@ -1126,8 +1155,10 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   // threads -> copies GB/s / epoch ms: 4 -> 54.4 / 53.2, 6 -> 52.1 / 45.9, 8 -> 47.8 / 46.5, 16 -> 45.8 /
   // 48.0).  Default: 0.4 x the hardware threads, where pack time and copy time of a window meet.
   const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
-  int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(2u, (hw * 2u + 2u) / 5u));
-  g->pool = new Pool(nt > 1 ? nt : 0);
+  const int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(2u, (hw * 2u + 2u) / 5u));
+  g->pack_threads_busy = nt;
+  const int n_pool = cfg->host_threads > 0 ? std::max(nt, (int)std::min<unsigned>(16u, hw)) : (int)std::min<unsigned>(16u, hw);
+  g->pool = new Pool(n_pool > 1 ? n_pool : 0);
   g->worker_a = std::thread(worker_a_main, g);
   g->worker_b = std::thread(worker_b_main, g);
   g->worker_c = std::thread(worker_c_main, g);
