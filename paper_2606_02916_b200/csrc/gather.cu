@@ -96,6 +96,31 @@ __device__ __forceinline__ void copy_tile(const uint8_t* const* s_src, uint8_t* 
   }
 }
 
+// Flat variant for rows that cross the host link (pull staging, miss fill): the tile is one run of
+// chunks, thread t takes chunks t, t + 256, ... -- every lane carries a load whatever the row
+// width (a 400-byte row fills only 25 lanes of a warp), which is what counts when the transfer is
+// bound by the bytes in flight over PCIe; the division per chunk does not matter at link speed.
+template <int VEC, int UNROLL>
+__device__ __forceinline__ void copy_tile_flat(const uint8_t* const* s_src, uint8_t* const* s_dst, int rows, int rb) {
+  const int cpr = rb / VEC, total = rows * cpr;
+  for (int c0 = threadIdx.x; c0 < total; c0 += kThreads * UNROLL) {
+    typename VecT<VEC>::type v[UNROLL];
+    int row[UNROLL], col[UNROLL];
+    bool ok[UNROLL];
+#pragma unroll
+    for (int k = 0; k < UNROLL; ++k) {
+      const int c = c0 + k * kThreads;
+      row[k] = c / cpr;
+      col[k] = c - row[k] * cpr;
+      ok[k] = c < total && s_src[row[k] < rows ? row[k] : 0] != nullptr;
+      if (ok[k]) v[k] = ld_stream<VEC>(s_src[row[k]] + (int64_t)col[k] * VEC);
+    }
+#pragma unroll
+    for (int k = 0; k < UNROLL; ++k)
+      if (ok[k]) st_stream<VEC>(s_dst[row[k]] + (int64_t)col[k] * VEC, v[k]);
+  }
+}
+
 struct GatherArgs {
   const int32_t* nodes;     // N_b
   int n;
@@ -333,7 +358,8 @@ __global__ void __launch_bounds__(kThreads) k_rows(RowsArgs A) {
     __syncthreads();
     // rows that come over the host link (MODE 1) keep twice as many loads in flight per thread:
     // a few CTAs then saturate PCIe and the rest of the GPU stays with the sampler
-    copy_tile<VEC, false, MODE == 1 ? 2 * kUnroll : kUnroll>(s_src, s_dst, nullptr, rows, A.rb);
+    if (MODE == 1) copy_tile_flat<VEC, 2 * kUnroll>(s_src, s_dst, rows, A.rb);
+    else copy_tile<VEC, false>(s_src, s_dst, nullptr, rows, A.rb);
   }
 }
 
