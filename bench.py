@@ -583,6 +583,47 @@ def run_ours(args):
         errors['consumer'] = repr(exc)
         g = recover_graph(g)
 
+    # ---- why the gather loses bandwidth beside the sampler: the same gathers timed alone and beside the
+    # key-only ALU kernel (gg_key_peak, no memory traffic at all) at 1, 2, 4, 8 resident CTAs per SM
+    try:
+        if not args.no_sweep and world == 1:
+            import threading
+            g.window_stage(13 * 10 ** 6, 0, batches[:min(W, 16)], w.fanouts)
+            nwin = min(W, 16)
+            g.trace(13 * 10 ** 6, nwin)                                    # the window's staging has completed
+
+            def time_gathers(reps=48):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                rows = 0
+                a.record(stream)
+                for i in range(reps):
+                    rows += g.batch_gather(13 * 10 ** 6, i % nwin, feats, stream)["n_input"]
+                b.record(stream)
+                b.synchronize()
+                return rows * (2 * w.row_bytes + 8) / (a.elapsed_time(b) * 1e-3) / 1e9
+
+            time_gathers()
+            probe = {"gather_alone_GB/s": time_gathers(), "beside_key_only_kernel": []}
+            for ctas in (1, 2, 4, 8):
+                res = {}
+                t = threading.Thread(target=lambda: res.update(v=binding.key_peak(ctas, 65536 * 2, 30)))
+                t.start()
+                time.sleep(0.03)
+                gb = time_gathers()
+                t.join()
+                probe["beside_key_only_kernel"].append({"alu_ctas_per_sm": ctas, "alu_warps_per_subpartition": 2 * ctas,
+                                                        "gather_GB/s": gb, "alu_Gkey/s": res["v"] / 1e9})
+            probe["note"] = ("the key-only kernel moves no memory: whatever the gather loses beside it is lost to warp scheduling on the "
+                             "SMs (its warps, mostly waiting on loads, are rarely picked against always-eligible ALU warps), not to HBM or "
+                             "L2 contention; the ALU kernel loses nothing")
+            variants["gather_vs_alu_kernel"] = probe
+            g.window_release(13 * 10 ** 6, stream)
+            torch.cuda.synchronize(dev)
+            g.cache_reset()
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['gather_vs_alu'] = repr(exc)
+        g = recover_graph(g)
+
     # ---- variant (NEXT-2): GPU-initiated pull staging instead of host pack + cudaMemcpyAsync ----
     try:
         if not args.no_sweep and world == 1 and args.staging_mode == 0:

@@ -28,8 +28,6 @@
 //                    proves the result (kept == f) and emits it in ascending edge position
 //   k_select_warp    ONE WARP PER ROW for the rows the kernels above could not prove exact (and for
 //                    every keyed row when fanout > kChunkMaxFanout)
-#include <cstdlib>
-
 #include "common.cuh"
 #include "kernels.h"
 
@@ -49,14 +47,15 @@ constexpr int kCand = 256;      // candidate buffer per warp
 constexpr int kWarps = 8;
 constexpr int kBins = 128;      // quarter-octave degree bins: bin = 4*floor(log2 deg) + next two bits
 constexpr int kChunk = 128;     // edge positions per chunk (at most)
-// tunables (gg_sampler_tune): rows in bins below c_single_bins are one chunk each, whatever their
-// degree; rows in bins >= c_warp_bin go to the warp kernel.  Defaults (bin 36 =
+// tunables (gg_sampler_tune; passed to the kernels of a hop): rows in bins below single_bins are one
+// chunk each, whatever their degree; rows in bins >= warp_bin go to the warp kernel.  Defaults (bin 36 =
 // degree 512): one lane per row below degree 512, one warp per row above; cutting the rows of
 // degree 128..4095 into chunks with the candidates merged through global memory measured slower
 // (products W=16, sampling per epoch alone: 16.5 ms at 36/36 vs 18.8-20.8 ms for 28/48, 36/48,
 // 28/128), so the multi-chunk path is off by default.
-__constant__ int c_single_bins = 36;
-__constant__ int c_warp_bin = 36;
+static int h_single_bins = 36, h_warp_bin = 36;
+constexpr int kSmallHopRows = 1 << 16;   // destinations of a hop below which the lane kernel stops at ...
+constexpr int kSmallHopBins = 28;        // ... bin 28 = degree 128
 constexpr int kChunkMaxFanout = 25;   // candidate lists of the chunk path hold <= 64 entries
 
 // device-side plan of one hop (zeroed before k_sample_count)
@@ -69,8 +68,8 @@ struct SamplePlan {
   unsigned long long n_chunks;      // = bin_chunk0[kBins]
   unsigned long long chunk_cursor;  // dynamic queue of the chunk kernel (units of 32 chunks)
   int32_t n_items;             // keyed rows
-  int32_t n_multi;             // items [n_warp_items, n_multi) are multi-chunk rows (c_single_bins <= bin < c_warp_bin)
-  int32_t n_warp_items;        // items [0, n_warp_items) belong to the warp kernel (bins >= c_warp_bin; fanout > kChunkMaxFanout: all)
+  int32_t n_multi;             // items [n_warp_items, n_multi) are multi-chunk rows (single_bins <= bin < warp_bin)
+  int32_t n_warp_items;        // items [0, n_warp_items) belong to the warp kernel (bins >= warp_bin; fanout > kChunkMaxFanout: all)
   int32_t n_fallback;          // rows handed over to the warp kernel
   int32_t warp_cursor;         // dynamic queue of the warp kernel
 };
@@ -142,7 +141,7 @@ k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ n
 // One CTA per batch (row): in-place exclusive scan of row[0..n_tiles[b]) ; totals[b] = sum.
 __global__ void __launch_bounds__(1024)
 k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, int items_per_tile,
-            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int all_to_warp) {
+            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int single_bins, int warp_bin) {
   __shared__ int32_t sm[33];
   __shared__ int32_t carry_s;
   const int b = blockIdx.x;
@@ -167,7 +166,6 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
   if (plan && b == 0) {
     __shared__ int32_t s_cnt[kBins], s_start[kBins];
     __shared__ unsigned long long s_nc[kBins], s_c0[kBins + 1];
-    const int single_bins = c_single_bins, warp_bin = all_to_warp ? 0 : c_warp_bin;
     if (threadIdx.x < kBins) {
       const int k = threadIdx.x;
       const int32_t n = plan->bin_count[k];
@@ -515,7 +513,7 @@ k_sample_plan(const int64_t* __restrict__ indptr, const int32_t* __restrict__ in
               int64_t cnt_pitch, const int32_t* __restrict__ tile_sums,
               const int32_t* __restrict__ totals, int32_t* __restrict__ blk_indptr,
               int32_t* __restrict__ edge_off_out, int32_t* __restrict__ src_global,
-              SamplePlan* __restrict__ plan, SampleItems items) {
+              SamplePlan* __restrict__ plan, SampleItems items, int single_bins) {
   __shared__ int32_t sm[33];
   __shared__ int32_t s_edge_base;
   __shared__ int32_t s_bin[kBins], s_base[kBins];
@@ -577,7 +575,7 @@ k_sample_plan(const int64_t* __restrict__ indptr, const int32_t* __restrict__ in
     items.row0[q] = r0;
     items.deg[q] = deg;
     items.out[q] = out;
-    if (bin >= c_single_bins) items.row_cnt[q] = 0;   // candidates the chunk kernel will append
+    if (bin >= single_bins) items.row_cnt[q] = 0;   // candidates the chunk kernel will append
   }
 }
 
@@ -649,15 +647,15 @@ __device__ __forceinline__ unsigned long long rank_list(uint32_t a0, int c, int 
 }
 
 __global__ void __launch_bounds__(kCThreads)
-k_select_chunk(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
-               SampleItems items, int32_t* __restrict__ src_global) {
+k_select_chunk(const int32_t* __restrict__ indices, int fanout, int cap, int single_bins,
+               SamplePlan* __restrict__ plan, SampleItems items, int32_t* __restrict__ src_global) {
   extern __shared__ __align__(16) uint32_t s_list[];   // [cap][kCThreads]{z, x}
   __shared__ unsigned long long s_c0[kBins + 1];
   for (int i = threadIdx.x; i <= kBins; i += kCThreads) s_c0[i] = plan->bin_chunk0[i];
   __syncthreads();
   const unsigned long long n_chunks = s_c0[kBins];
   const float wantf = want_candidates(fanout);
-  const int rshift = c_rank_shift, single_bins = c_single_bins;
+  const int rshift = c_rank_shift;
   const int lane = threadIdx.x & 31;
   const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(s_list) + threadIdx.x * 8;
   const uint32_t a_lim4 = a0 + (uint32_t)(cap - 4) * kCSlot, a_lim1 = a0 + (uint32_t)(cap - 1) * kCSlot;
@@ -915,9 +913,9 @@ void sampler_stats(unsigned long long out[4]) {
   cudaMemcpyFromSymbol(out, g_sampler_stat, 4 * sizeof(unsigned long long));
 }
 cudaError_t sampler_tune(int single_bins, int warp_bin) {
-  cudaError_t e = cudaMemcpyToSymbol(c_single_bins, &single_bins, sizeof(int));
-  if (e != cudaSuccess) return e;
-  return cudaMemcpyToSymbol(c_warp_bin, &warp_bin, sizeof(int));
+  h_single_bins = single_bins;
+  h_warp_bin = warp_bin;
+  return cudaSuccess;
 }
 cudaError_t sampler_debug(int rank_shift, float want_add) {
   cudaError_t e = cudaMemcpyToSymbol(c_rank_shift, &rank_shift, sizeof(int));
@@ -927,7 +925,7 @@ cudaError_t sampler_debug(int rank_shift, float want_add) {
 
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
                       int items_per_tile, int32_t* totals) {
-  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals, nullptr, 0);
+  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals, nullptr, 0, 0);
   count_launches(1);
 }
 
@@ -943,15 +941,25 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
   dim3 grid(tiles, W);
   SamplePlan* plan = static_cast<SamplePlan*>(wk.plan);
   const bool chunk_path = fanout <= kChunkMaxFanout;
+  // cut-overs of this hop.  A hop with few destinations (the hop out of the seeds: W x 1024 rows)
+  // cannot fill the GPU with one lane per row -- its longest rows, alone on their lanes, are the
+  // whole kernel (36 us for 1.6 M warp instructions at W=16) -- so there the lane kernel stops at
+  // degree 128 and everything above takes a warp.
+  int single_bins = h_single_bins, warp_bin = chunk_path ? h_warp_bin : 0;
+  if (chunk_path && dst_off.v[W] < kSmallHopRows) {
+    single_bins = single_bins < kSmallHopBins ? single_bins : kSmallHopBins;
+    warp_bin = warp_bin < kSmallHopBins ? warp_bin : kSmallHopBins;
+  }
+  const bool multi = chunk_path && single_bins < warp_bin;
   cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
-  count_launches(chunk_path ? 6 : 4);
+  count_launches(chunk_path ? (multi ? 6 : 5) : 4);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
                                          cnt_tmp, cnt_pitch, tile_sums, plan);
-  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, chunk_path ? 0 : 1);
+  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, single_bins, warp_bin);
   k_sample_plan<<<grid, kTile, 0, st>>>(indptr, indices, nodes, node_pitch, n_dst, dst_off, W,
                                         fanout, max_tiles, key_prefix_b, cnt_tmp, cnt_pitch,
                                         tile_sums, totals, blk_indptr, edge_off_out, src_global,
-                                        plan, wk.items);
+                                        plan, wk.items, single_bins);
   if (chunk_path) {
     const int cap = cand_cap(fanout);
     const size_t smem = (size_t)cap * kCSlot;
@@ -962,13 +970,12 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
     }
     int per_sm = (int)((220 * 1024) / (smem + 2048));
     per_sm = per_sm < 1 ? 1 : (per_sm > 12 ? 12 : per_sm);
-    static int cap_chunk = getenv("GG_SAMP_CTAS_CHUNK") ? atoi(getenv("GG_SAMP_CTAS_CHUNK")) : 0;
-    if (cap_chunk > 0 && per_sm > cap_chunk) per_sm = cap_chunk;
-    k_select_chunk<<<sm_count() * per_sm, kCThreads, smem, st>>>(indices, fanout, cap, plan, wk.items, src_global);
-    k_select_rank<<<sm_count() * 16, kCThreads, 0, st>>>(indices, fanout, cap, plan, wk.items, src_global);
+    k_select_chunk<<<sm_count() * per_sm, kCThreads, smem, st>>>(indices, fanout, cap, single_bins, plan, wk.items,
+                                                                 src_global);
+    if (multi)      // there are multi-chunk bins: their rows' candidate lists are ranked here
+      k_select_rank<<<sm_count() * 16, kCThreads, 0, st>>>(indices, fanout, cap, plan, wk.items, src_global);
   }
-  static int ctas_warp = getenv("GG_SAMP_CTAS_WARP") ? atoi(getenv("GG_SAMP_CTAS_WARP")) : 6;
-  k_select_warp<<<sm_count() * ctas_warp, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
+  k_select_warp<<<sm_count() * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
 }
 
 int sample_cand_cap(int fanout) { return fanout <= kChunkMaxFanout ? cand_cap(fanout) : 0; }

@@ -51,9 +51,11 @@ def sum_over_ranks(x: float, device="cpu") -> float:
 
 
 def shard_plan(rank: int, world: int, num_parts: int, n_batches: int) -> Tuple[int, List[int]]:
-    """(local partition, batch indices) of a rank.  Weak scaling: every rank serves a full
-    epoch's worth of batches -- the epoch order rotated by rank so ranks see different
-    windows -- and is the trainer of partition rank % P."""
+    """(local partition, batch indices) of a rank.  Replicated work, weak scaling: every rank is
+    an independent trainer (of partition rank % P) that serves a full epoch's worth of batches in
+    its OWN epoch order -- the generator's order rotated by the rank, so ranks see different
+    windows.  The batch index that enters the sampling key (reading S7) is the position in that
+    rank's order; with one rank the rotation is the identity.  This does not divide one epoch by N."""
     local_part = rank % num_parts
     shift = (rank * n_batches) // max(world, 1)
     order = [(i + shift) % n_batches for i in range(n_batches)]
