@@ -753,9 +753,23 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
       g->h_resp[bi] = (uint8_t*)pp;
       if (rc != GG_OK) return rc;
     }
-    int64_t q0 = 0;
-    for (int m = 0; m < g->R.P; ++m) {
+    // Owners are served smallest request first: nothing can cross the link before the first pack
+    // ends, so the shortest pack goes first (each owner keeps its slot range, owners ascending).
+    int64_t q0_of[GG_MAX_PARTS];
+    int order[GG_MAX_PARTS];
+    {
+      int64_t acc = 0;
+      for (int m = 0; m < g->R.P; ++m) {
+        q0_of[m] = acc;
+        acc += w->bulk[m];
+        order[m] = m;
+      }
+      std::stable_sort(order, order + g->R.P, [&](int a, int b) { return w->bulk[a] < w->bulk[b]; });
+    }
+    for (int oi = 0; oi < g->R.P; ++oi) {
+      const int m = order[oi];
       const int64_t nm = w->bulk[m];
+      const int64_t q0 = q0_of[m];
       if (nm == 0) continue;
       if (g->store_on_device[m]) {
         // this owner's store is device memory (e.g. a peer's HBM): host threads cannot read it, so
@@ -766,7 +780,6 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
         CU(cudaEventRecord(w->ev_copy[2 * w->bulk_copies + 1], sc));
         g->prof.end(sc, pd, GG_PROF_STAGE_COPY, nm * rb);
         w->bulk_copies += 1;
-        q0 += nm;
         continue;
       }
       // owner service: gather owner m's requested rows into a contiguous response
@@ -807,7 +820,6 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
       }
       g->prof.end(sc, pe, GG_PROF_STAGE_COPY, nm * rb);
       w->bulk_copies += 1;
-      q0 += nm;
     }
     CU(cudaEventRecord(g->resp_free[ri], sc));
     g->resp_used[ri] = true;

@@ -46,7 +46,7 @@ __device__ __forceinline__ void bfly(float (&p)[16], int lane) {
 }
 
 template <bool RELU>
-__global__ void __launch_bounds__(kSageWarps * 32, 4)
+__global__ void __launch_bounds__(2 * kSageWarps * 32, 2)   // 8 warps per CTA, 16 when the weights fill the SM's shared memory
 k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
            const int32_t* __restrict__ src_local, int n_dst, int din, int dout,
            const float* __restrict__ w_self, const float* __restrict__ w_neigh,
@@ -67,8 +67,8 @@ k_sage_fwd(const float* __restrict__ h_in, const int32_t* __restrict__ indptr,
   }
   for (int k = threadIdx.x; k < dout; k += blockDim.x) sb[k] = bias[k];
   __syncthreads();
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int i = blockIdx.x * kSageWarps + wid; i < n_dst; i += gridDim.x * kSageWarps) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int i = blockIdx.x * nw + wid; i < n_dst; i += gridDim.x * nw) {
     const int e0 = indptr[i], e1 = indptr[i + 1];
     const float deg = (float)(e1 - e0);
     float p[16];
@@ -543,11 +543,16 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
     const gg_block& b = batch->blocks[L - 1 - l];
     const int din = m->dims[l], dout = m->dims[l + 1];
     const size_t smem = (size_t)(2 * (dout <= 16 ? 17 * din : din * dout) + dout) * sizeof(float);
+    // wide feature rows: the weights take 82 KB per CTA at 602 columns (two CTAs per SM), so each CTA
+    // brings 16 warps instead of 8 to keep the row loads of 32 warps per SM in flight
+    const int nw = smem > 48 * 1024 ? 2 * kSageWarps : kSageWarps;
+    int gf = (b.n_dst + nw - 1) / nw;
+    gf = gf < 1 ? 1 : (gf > gcap ? gcap : gf);
     if (l < L - 1)
-      k_sage_fwd<true><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h, b.indptr, b.src_local, b.n_dst, din, dout,
+      k_sage_fwd<true><<<gf, nw * 32, smem, st>>>(h, b.indptr, b.src_local, b.n_dst, din, dout,
           p_self(m, l, m->params), p_neigh(m, l, m->params), p_bias(m, l, m->params), m->agg[l].p, m->out[l].p);
     else
-      k_sage_fwd<false><<<grid_for(b.n_dst), kSageWarps * 32, smem, st>>>(h, b.indptr, b.src_local, b.n_dst, din, dout,
+      k_sage_fwd<false><<<gf, nw * 32, smem, st>>>(h, b.indptr, b.src_local, b.n_dst, din, dout,
           p_self(m, l, m->params), p_neigh(m, l, m->params), p_bias(m, l, m->params), m->agg[l].p, m->out[l].p);
     h = m->out[l].p;
   }
