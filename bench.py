@@ -41,6 +41,7 @@ def parse_args():
                     help="windows staged ahead of the one being served (sampling runs that far ahead; "
                          "the cache is always built one window ahead)")
     ap.add_argument("--host-threads", type=int, default=0)
+    ap.add_argument("--sampler-tune", default="", help="single_bins,warp_bin,hub_bin for gg_sampler_tune (default: the library's)")
     ap.add_argument("--cache-buffers", type=int, default=4, help="HBM cache buffers in rotation (gg_config.cache_buffers)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the W sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -295,6 +296,8 @@ def run_ours(args):
     # (long-running, ALU-bound) sampling kernels whenever an SM has room for both
     stream = torch.cuda.Stream(dev, priority=-1)
     torch.cuda.set_stream(stream)
+    if args.sampler_tune:
+        binding.sampler_tune(*[int(x) for x in args.sampler_tune.split(",")])
     energy = EnergyMeter(local_rank)
     link_peak = host_link_peak(dev)
     key_peak_gkeys = binding.key_peak(8, 65536, 5) / 1e9     # measured ALU roofline of a-1, GPU otherwise idle

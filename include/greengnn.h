@@ -292,13 +292,17 @@ gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);
 
 /* Degree cut-overs of the selection kernels (performance knobs; results are bit-exact for every
  * setting, tests/test_gpu_parity.py).  Keyed rows are binned by degree in quarter octaves, bin =
- * 4*floor(log2 deg) + the next two bits (bin 28 = degree 128, 36 = 512, 48 = 4096).  Rows in bins
- * below single_bins are selected by one lane each; rows in bins >= warp_bin by one warp each; rows
- * in between are cut into chunks of <= 128 edge positions, one lane per chunk, the candidates of a
- * row merged through a list in global memory.  Default (36, 36).  Process-wide; must not be called
- * while a window is being staged.  Errors: INVALID_ARG for single_bins outside [28, 128] (a row below
- * degree 128 is always one chunk) or warp_bin outside [0, 128]. */
-gg_status gg_sampler_tune(int32_t single_bins, int32_t warp_bin);
+ * 4*floor(log2 deg) + the next two bits (bin 28 = degree 128, 36 = 512, 48 = 4096, 60 = 32768).  Rows
+ * in bins below single_bins are selected by one lane each; rows in bins from warp_bin up to hub_bin
+ * by one warp each; rows in bins [single_bins, warp_bin) and the hub rows in bins >= hub_bin are cut
+ * into chunks of <= 128 edge positions, one lane per chunk, the candidates of a row merged through a
+ * list in global memory.  Default (36, 36, 128): one lane per row below degree 512, one warp per row
+ * above, no chunking (measured: chunking moves instructions one for one and adds the rank launch;
+ * Large config with hubs of degree >= 32768 chunked: 290 vs 240 ms of sampling per epoch).
+ * Process-wide; must not be called while a window is being staged.  Errors: INVALID_ARG for
+ * single_bins or hub_bin outside [28, 128] (a row below degree 128 is always one chunk) or warp_bin
+ * outside [0, 128]. */
+gg_status gg_sampler_tune(int32_t single_bins, int32_t warp_bin, int32_t hub_bin);
 
 /* The measured integer-ALU roofline of a-1 ("keys/s vs the peak of
  * a key-only micro-kernel measured on the same GPU").  Launches a kernel in which every lane

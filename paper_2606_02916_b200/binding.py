@@ -125,7 +125,7 @@ def load_library(path: Optional[str] = None):
     lib.gg_key.restype = u64
     lib.gg_sampler_stats.argtypes = [P(u64), P(u64), P(u64)]
     lib.gg_debug_sampler.argtypes = [i32, C.c_float]
-    lib.gg_sampler_tune.argtypes = [i32, i32]
+    lib.gg_sampler_tune.argtypes = [i32, i32, i32]
     lib.gg_key_peak.argtypes = [i32, i32, i32, P(C.c_double), P(C.c_uint32)]
     lib.gg_simulate.argtypes = [vp, vp, vp, i32, u64, vp, i32, vp, i32, P(gg_energy_model), P(gg_sim_result),
                                 P(i32), vp, vp]
@@ -160,9 +160,9 @@ def sampler_stats() -> dict:
     return {"keys": int(k.value), "rows": int(r.value), "fallbacks": int(f.value)}
 
 
-def sampler_tune(single_bins: int = 36, warp_bin: int = 36) -> None:
+def sampler_tune(single_bins: int = 36, warp_bin: int = 36, hub_bin: int = 128) -> None:
     """Degree-bin cut-overs of the selection kernels (include/greengnn.h gg_sampler_tune)."""
-    _check_global(load_library().gg_sampler_tune(single_bins, warp_bin))
+    _check_global(load_library().gg_sampler_tune(single_bins, warp_bin, hub_bin))
 
 
 def key_peak(ctas_per_sm: int = 8, keys_per_lane: int = 65536, reps: int = 5, with_fold: bool = False):

@@ -280,7 +280,7 @@ using namespace gg;
 struct gg_graph {
   Profiler prof;
   // inputs
-  int64_t N = 0, nnz = 0;
+  int64_t N = 0, nnz = 0, max_degree = 0;
   const int64_t* indptr = nullptr;
   const int32_t* indices = nullptr;
   OwnerRanges R;
@@ -544,6 +544,7 @@ static gg_status stage_a(gg_graph* g, Window* w) {
     wk.items.hdst = g->it_hdst.p; wk.items.row0 = g->it_row0.p; wk.items.deg = g->it_deg.p;
     wk.items.out = g->it_out.p; wk.items.fallback = g->it_fb.p;
     wk.items.row_cnt = g->it_cnt.p; wk.items.cand = g->it_cand.p;
+    wk.max_degree = g->max_degree;
     cudaEvent_t pe = g->prof.begin(st);
     launch_sample_hop(st, g->indptr, g->indices, w->nodes.p, w->node_pitch, n_dst, dst_off, W, max_nd,
                       w->fanouts[h], g->key_prefix.p + h * Wmax, g->cnt_tmp.p, cnt_pitch, g->tiles32.p,
@@ -1160,6 +1161,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
     CUC(cudaEventCreateWithFlags(&w.consumer_done, cudaEventDisableTiming));
     for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) CUC(cudaEventCreate(&w.ev_copy[c]));
   }
+  CUC(max_degree(g->indptr, g->N, &g->max_degree));
   CUC(cudaDeviceSynchronize());
 #undef CUC
   // The pack and the DMA reads of the bulk copies share the host's DRAM: more pack threads finish a
@@ -1503,11 +1505,11 @@ gg_status gg_debug_sampler(int32_t rank_shift, float want_add) {
   return GG_OK;
 }
 
-gg_status gg_sampler_tune(int32_t single_bins, int32_t warp_bin) {
-  if (single_bins < 28 || single_bins > 128 || warp_bin < 0 || warp_bin > 128)
-    return fail(GG_ERR_INVALID_ARG, "single_bins must be in [28, 128] (rows below degree 128 are one chunk), warp_bin in [0, 128]");
+gg_status gg_sampler_tune(int32_t single_bins, int32_t warp_bin, int32_t hub_bin) {
+  if (single_bins < 28 || single_bins > 128 || warp_bin < 0 || warp_bin > 128 || hub_bin < 28 || hub_bin > 128)
+    return fail(GG_ERR_INVALID_ARG, "single_bins and hub_bin must be in [28, 128] (rows below degree 128 are one chunk), warp_bin in [0, 128]");
   CU(cudaDeviceSynchronize());
-  CU(sampler_tune(single_bins, warp_bin));
+  CU(sampler_tune(single_bins, warp_bin, hub_bin));
   return GG_OK;
 }
 

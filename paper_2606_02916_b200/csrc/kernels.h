@@ -40,6 +40,7 @@ struct SampleItems {
 struct SampleWork {
   void* plan;         // device, sample_plan_bytes()
   SampleItems items;  // each array holds at least the hop's destination count
+  int64_t max_degree; // longest row of the graph (0 = unknown): hub rows get their own treatment only where they exist
 };
 size_t sample_plan_bytes();
 int sample_cand_cap(int fanout);   // entries of a row's candidate list in global memory (0: the hop does not use one)
@@ -51,7 +52,8 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
                        int32_t* edge_off_out, int32_t* src_global, const SampleWork& wk);
 void sampler_stats(unsigned long long out[4]);           // synchronous read of g_sampler_stat
 cudaError_t sampler_debug(int rank_shift, float want_add);  // test knobs, see sample.cu
-cudaError_t sampler_tune(int single_bins, int warp_bin);     // degree-bin cut-overs of the selection kernels
+cudaError_t sampler_tune(int single_bins, int warp_bin, int hub_bin);   // degree-bin cut-overs of the selection kernels
+cudaError_t max_degree(const int64_t* indptr, int64_t n, int64_t* out);  // synchronous
 // key-only micro-kernel: the measured integer-ALU roofline of the sampler (keys per second)
 cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, double* keys_per_s, uint32_t* fold_out);
 // shared by a-1 / a-2: one CTA per batch row, exclusive scan of ceil(n_items[b]/items_per_tile) sums

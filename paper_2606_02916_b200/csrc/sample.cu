@@ -53,7 +53,7 @@ constexpr int kChunk = 128;     // edge positions per chunk (at most)
 // degree 128..4095 into chunks with the candidates merged through global memory measured slower
 // (products W=16, sampling per epoch alone: 16.5 ms at 36/36 vs 18.8-20.8 ms for 28/48, 36/48,
 // 28/128), so the multi-chunk path is off by default.
-static int h_single_bins = 36, h_warp_bin = 36;
+static int h_single_bins = 36, h_warp_bin = 36, h_hub_bin = 128;   // hub chunking off: see gg_sampler_tune
 constexpr int kSmallHopRows = 1 << 16;   // destinations of a hop below which the lane kernel stops at ...
 constexpr int kSmallHopBins = 28;        // ... bin 28 = degree 128
 constexpr int kChunkMaxFanout = 25;   // candidate lists of the chunk path hold <= 64 entries
@@ -68,8 +68,9 @@ struct SamplePlan {
   unsigned long long n_chunks;      // = bin_chunk0[kBins]
   unsigned long long chunk_cursor;  // dynamic queue of the chunk kernel (units of 32 chunks)
   int32_t n_items;             // keyed rows
+  int32_t n_hub;               // items [0, n_hub): bins >= hub_bin, cut into chunks (a hub row would hold one warp for milliseconds)
+  int32_t n_warp_items;        // items [n_hub, n_warp_items) belong to the warp kernel (warp_bin <= bin < hub_bin; fanout > kChunkMaxFanout: all)
   int32_t n_multi;             // items [n_warp_items, n_multi) are multi-chunk rows (single_bins <= bin < warp_bin)
-  int32_t n_warp_items;        // items [0, n_warp_items) belong to the warp kernel (bins >= warp_bin; fanout > kChunkMaxFanout: all)
   int32_t n_fallback;          // rows handed over to the warp kernel
   int32_t warp_cursor;         // dynamic queue of the warp kernel
 };
@@ -141,7 +142,7 @@ k_sample_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ n
 // One CTA per batch (row): in-place exclusive scan of row[0..n_tiles[b]) ; totals[b] = sum.
 __global__ void __launch_bounds__(1024)
 k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, int items_per_tile,
-            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int single_bins, int warp_bin) {
+            int32_t* __restrict__ totals, SamplePlan* __restrict__ plan, int single_bins, int warp_bin, int hub_bin) {
   __shared__ int32_t sm[33];
   __shared__ int32_t carry_s;
   const int b = blockIdx.x;
@@ -170,12 +171,12 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
       const int k = threadIdx.x;
       const int32_t n = plan->bin_count[k];
       s_cnt[k] = n;
-      const unsigned long long nc = k >= warp_bin ? 0ull : (unsigned long long)n * bin_chunks(k, single_bins);
+      const unsigned long long nc = (k >= warp_bin && k < hub_bin) ? 0ull : (unsigned long long)n * bin_chunks(k, single_bins);
       s_nc[k] = (nc + 31ull) & ~31ull;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-      int32_t acc = 0, n_multi = 0, n_warp = 0;
+      int32_t acc = 0, n_multi = 0, n_warp = 0, n_hub = 0;
       unsigned long long c0 = 0;
       for (int k = kBins - 1; k >= 0; --k) {
         s_start[k] = acc;
@@ -183,12 +184,15 @@ k_tile_scan(int32_t* __restrict__ tiles, int row_pitch, BatchOffsets n_items, in
         c0 += s_nc[k];
         acc += s_cnt[k];
         if (k == single_bins) n_multi = acc;
+        if (k == hub_bin) n_hub = acc;
         if (k == warp_bin) n_warp = acc;
       }
       s_c0[kBins] = c0;
       plan->n_chunks = c0;
       plan->chunk_cursor = 0;
       plan->n_items = acc;
+      n_warp = n_warp > n_hub ? n_warp : n_hub;
+      plan->n_hub = n_hub;
       plan->n_warp_items = n_warp;
       plan->n_multi = n_multi > n_warp ? n_multi : n_warp;
       plan->n_fallback = 0;
@@ -753,9 +757,11 @@ k_select_chunk(const int32_t* __restrict__ indices, int fanout, int cap, int sin
 __global__ void __launch_bounds__(kCThreads)
 k_select_rank(const int32_t* __restrict__ indices, int fanout, int cap, SamplePlan* __restrict__ plan,
               SampleItems items, int32_t* __restrict__ src_global) {
-  const int n_multi = plan->n_multi;
+  const int n_hub = plan->n_hub, n_warp_end = plan->n_warp_items;
+  const int n_rows = n_hub + (plan->n_multi - n_warp_end);     // hub rows, then the mid-range multi-chunk rows
   const int rshift = c_rank_shift;
-  for (int q = plan->n_warp_items + blockIdx.x * kCThreads + threadIdx.x; q < n_multi; q += gridDim.x * kCThreads) {
+  for (int t = blockIdx.x * kCThreads + threadIdx.x; t < n_rows; t += gridDim.x * kCThreads) {
+    const int q = t < n_hub ? t : t - n_hub + n_warp_end;
     const int c = items.row_cnt[q];
     int kept = -1;
     if (c >= fanout && c <= cap) {
@@ -812,14 +818,15 @@ k_select_warp(const int32_t* __restrict__ indices, int fanout, SamplePlan* __res
               SampleItems items, int32_t* __restrict__ src_global) {
   __shared__ __align__(16) uint32_t s_scratch[kWarps][kScratchWords];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int n_warp = plan->n_warp_items, n_total = n_warp + plan->n_fallback;
+  const int n_hub = plan->n_hub;
+  const int n_warp = plan->n_warp_items - n_hub, n_total = n_warp + plan->n_fallback;
   const float wantf = want_candidates(fanout);
   for (;;) {
     int w = 0;
     if (lane == 0) w = atomicAdd(&plan->warp_cursor, 1);
     w = __shfl_sync(0xffffffffu, w, 0);
     if (w >= n_total) break;
-    const int q = w < n_warp ? w : items.fallback[w - n_warp];
+    const int q = w < n_warp ? n_hub + w : items.fallback[w - n_warp];
     const uint64_t hdst = items.hdst[q];
     const uint32_t deg = items.deg[q];
     const int32_t* row = indices + items.row0[q];
@@ -912,10 +919,39 @@ cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, dou
 void sampler_stats(unsigned long long out[4]) {
   cudaMemcpyFromSymbol(out, g_sampler_stat, 4 * sizeof(unsigned long long));
 }
-cudaError_t sampler_tune(int single_bins, int warp_bin) {
+cudaError_t sampler_tune(int single_bins, int warp_bin, int hub_bin) {
   h_single_bins = single_bins;
   h_warp_bin = warp_bin;
+  h_hub_bin = hub_bin;
   return cudaSuccess;
+}
+
+// largest row length of a CSR (one pass over indptr at graph creation)
+__global__ void k_max_degree(const int64_t* __restrict__ indptr, int64_t n, unsigned long long* __restrict__ out) {
+  unsigned long long m = 0;
+  for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < n; v += (int64_t)gridDim.x * blockDim.x) {
+    const unsigned long long d = (unsigned long long)(indptr[v + 1] - indptr[v]);
+    m = d > m ? d : m;
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    const unsigned long long y = __shfl_xor_sync(0xffffffffu, m, o);
+    m = y > m ? y : m;
+  }
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+cudaError_t max_degree(const int64_t* indptr, int64_t n, int64_t* out) {
+  unsigned long long* d = nullptr;
+  cudaError_t e = cudaMalloc((void**)&d, sizeof(unsigned long long));
+  if (e != cudaSuccess) return e;
+  cudaMemset(d, 0, sizeof(unsigned long long));
+  k_max_degree<<<sm_count() * 8, 256>>>(indptr, n, d);
+  count_launches(1);
+  unsigned long long h = 0;
+  e = cudaMemcpy(&h, d, sizeof h, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  *out = (int64_t)h;
+  return e;
 }
 cudaError_t sampler_debug(int rank_shift, float want_add) {
   cudaError_t e = cudaMemcpyToSymbol(c_rank_shift, &rank_shift, sizeof(int));
@@ -925,7 +961,7 @@ cudaError_t sampler_debug(int rank_shift, float want_add) {
 
 void launch_tile_scan(cudaStream_t st, int W, int32_t* tiles, int row_pitch, const BatchOffsets& n_items,
                       int items_per_tile, int32_t* totals) {
-  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals, nullptr, 0, 0);
+  k_tile_scan<<<W, 1024, 0, st>>>(tiles, row_pitch, n_items, items_per_tile, totals, nullptr, 0, 0, 0);
   count_launches(1);
 }
 
@@ -950,12 +986,16 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
     single_bins = single_bins < kSmallHopBins ? single_bins : kSmallHopBins;
     warp_bin = warp_bin < kSmallHopBins ? warp_bin : kSmallHopBins;
   }
-  const bool multi = chunk_path && single_bins < warp_bin;
+  // hub rows (bins >= hub_bin; only graphs that have such rows pay for the extra launch) are cut into
+  // chunks whatever the other cut-overs say
+  int hub_bin = chunk_path ? (h_hub_bin > warp_bin ? h_hub_bin : warp_bin) : kBins;
+  if (wk.max_degree > 0 && deg_bin((uint32_t)(wk.max_degree > 0x7fffffff ? 0x7fffffff : wk.max_degree)) < hub_bin) hub_bin = kBins;
+  const bool multi = chunk_path && (single_bins < warp_bin || hub_bin < kBins);
   cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
   count_launches(chunk_path ? (multi ? 6 : 5) : 4);
   k_sample_count<<<grid, kTile, 0, st>>>(indptr, nodes, node_pitch, n_dst, fanout, max_tiles,
                                          cnt_tmp, cnt_pitch, tile_sums, plan);
-  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, single_bins, warp_bin);
+  k_tile_scan<<<W, 1024, 0, st>>>(tile_sums, max_tiles, n_dst, kTile, totals, plan, single_bins, warp_bin, hub_bin);
   k_sample_plan<<<grid, kTile, 0, st>>>(indptr, indices, nodes, node_pitch, n_dst, dst_off, W,
                                         fanout, max_tiles, key_prefix_b, cnt_tmp, cnt_pitch,
                                         tile_sums, totals, blk_indptr, edge_off_out, src_global,
@@ -973,7 +1013,8 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
     k_select_chunk<<<sm_count() * per_sm, kCThreads, smem, st>>>(indices, fanout, cap, single_bins, plan, wk.items,
                                                                  src_global);
     if (multi)      // there are multi-chunk bins: their rows' candidate lists are ranked here
-      k_select_rank<<<sm_count() * 16, kCThreads, 0, st>>>(indices, fanout, cap, plan, wk.items, src_global);
+      k_select_rank<<<sm_count() * (single_bins < warp_bin ? 16 : 2), kCThreads, 0, st>>>(indices, fanout, cap, plan, wk.items,
+                                                                                            src_global);
   }
   k_select_warp<<<sm_count() * 6, kWarps * 32, 0, st>>>(indices, fanout, plan, wk.items, src_global);
 }

@@ -201,13 +201,14 @@ def test_hub_rows_of_1e5_edges(dev):
     assert binding.sampler_stats()["fallbacks"] > before["fallbacks"]
 
 
-@pytest.mark.parametrize("single_bins,warp_bin", [(28, 48), (28, 128), (36, 48), (28, 28), (128, 128), (40, 64)])
-def test_selection_cut_overs_do_not_change_results(workload, dev, single_bins, warp_bin):
+@pytest.mark.parametrize("single_bins,warp_bin,hub_bin", [(28, 48, 128), (28, 128, 128), (36, 48, 60), (28, 28, 128), (128, 128, 128),
+                                                          (40, 64, 64), (36, 36, 40), (36, 36, 52)])
+def test_selection_cut_overs_do_not_change_results(workload, dev, single_bins, warp_bin, hub_bin):
     """gg_sampler_tune moves rows between the three selection schemes (one lane per row, one lane per
     chunk of 128 positions with the row's candidates merged through global memory, one warp per
     row); the blocks stay the oracle's, also with the fallback knobs on and on hub rows."""
     from paper_2606_02916_b200 import binding
-    binding.sampler_tune(single_bins, warp_bin)
+    binding.sampler_tune(single_bins, warp_bin, hub_bin)
     try:
         pu.check_epoch(workload("dense_mini", dev), W=2, n_hot=-1, max_batches=2, check_features=False)
         pu.check_epoch(workload("products_mini", dev), W=4, n_hot=-1, max_batches=4, check_features=False)
