@@ -285,7 +285,7 @@ uint64_t gg_launch_count(void);
  *   rows      destinations that needed a keyed selection (deg > fanout);
  *   fallbacks of those, hand-overs because a fast selection could not prove its result exact
  *             (candidate list overflow, fewer than fanout candidates under the threshold guess,
- *             or a tie in the high 32 key bits at the boundary): thread-per-row kernel -> warp
+ *             or a tie in the high 32 key bits at the boundary): lane-per-row (or chunk) kernel -> warp
  *             kernel, plus warp kernel -> exact ballot/bisection path.
  * Any pointer may be NULL. */
 gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);

@@ -1,13 +1,15 @@
 // Host orchestration behind the C ABI of include/greengnn.h.
 //
-// Threads and streams (Alg. 1, PAPER.md:166-198):
-//   caller thread   gg_window_stage enqueues a job; gg_batch_gather launches the per-batch kernels
-//                   on the caller's stream after making it wait for the window's cache-ready event
-//   prefetch thread owns the side stream: samples the window, builds U_k / H_k / Delta, runs the
-//                   owner service (host pack) and issues one bulk copy per owner -- all while the
-//                   caller's stream serves the previous window ("Parallel with training", l.8)
-// Two window slots ping-pong (slot = stage counter & 1): each holds the window's blocks, its
-// cache buffer, its ID->slot map and the list of cached IDs (= C_k).
+// Threads and streams (Alg. 1, PAPER.md:166-198; DESIGN.md Sec. 1):
+//   caller thread    gg_window_stage enqueues a job; gg_batch_gather launches the per-batch kernels
+//                    on the caller's stream after making it wait for the window's cache-ready event
+//   sampler thread   stream A: a-1 .. a-3 of a window (sampling, frontiers, unique + count)
+//   selector thread  stream B (high priority): a-4 / a-5, request lists to the host
+//   stager thread    stream C: owner-service pack + one bulk copy per owner, carry-over copy,
+//                    cache-ready event -- all while the caller's stream serves earlier windows
+//                    ("Parallel with training", l.8)
+// n_win window arenas (blocks, N_b, request lists) and n_cs cache buffers (rows, ID->slot map, the
+// list of cached IDs = C_k) rotate: window k uses arena k mod n_win and cache buffer k mod n_cs.
 #include <emmintrin.h>
 #include <xmmintrin.h>
 
