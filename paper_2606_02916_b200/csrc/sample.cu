@@ -626,11 +626,12 @@ __device__ __forceinline__ unsigned long long rank_list(uint32_t a0, int c, int 
   const int c4 = (c + 3) & ~3;
   for (int s = c; s < c4; ++s) sts_u32(a0 + s * kCSlot, 0xffffffffu);   // the list holds c4 <= cap entries
   // the fanout-th smallest DISTINCT value, one round per rank: each round takes the minimum of
-  // (v - last - 1) mod 2^32, which orders the values above `last` before everything else
+  // (v - last - 1) mod 2^32, which orders the values above `last` before everything else.  With
+  // fewer than `fanout` distinct values the rounds wrap around to the small ones again; that needs
+  // no care: whatever thr comes out, {v <= thr} is a set of smallest values, and it is the top
+  // `fanout` exactly when it has `fanout` members, which is the only case the caller accepts.
   uint32_t lastp1 = 0, thr = 0;
-  bool wrapped = false;
   for (int r = 0; r < fanout; ++r) {
-    wrapped = wrapped || (r > 0 && lastp1 == 0);
     uint32_t best = 0xffffffffu;
     for (int s = 0; s < c4; s += 4) {
       const uint32_t w0 = lds_u32(a0 + s * kCSlot) - lastp1;
@@ -642,12 +643,20 @@ __device__ __forceinline__ unsigned long long rank_list(uint32_t a0, int c, int 
     thr = best + lastp1;
     lastp1 = thr + 1u;
   }
-  // fewer than `fanout` distinct values or a tie at or below the threshold gives kept != fanout
-  unsigned long long keep = 0;
-  for (int i = 0; i < c; ++i) keep |= (unsigned long long)(lds_u32(a0 + i * kCSlot) <= thr) << i;
-  if (wrapped) keep = 0;
-  *kept = __popcll(keep);
-  return keep;
+  // keep flags, 32 candidates per word (a 64-bit shift per candidate costs five instructions)
+  uint32_t k0 = 0, k1 = 0, bit = 1u;
+  const int c_lo = c < 32 ? c : 32;
+  for (int i = 0; i < c_lo; ++i) {
+    if (lds_u32(a0 + i * kCSlot) <= thr) k0 |= bit;
+    bit <<= 1;
+  }
+  bit = 1u;
+  for (int i = 32; i < c; ++i) {
+    if (lds_u32(a0 + i * kCSlot) <= thr) k1 |= bit;
+    bit <<= 1;
+  }
+  *kept = __popc(k0) + __popc(k1);
+  return ((unsigned long long)k1 << 32) | k0;
 }
 
 __global__ void __launch_bounds__(kCThreads)
@@ -727,9 +736,13 @@ k_select_chunk(const int32_t* __restrict__ indices, int fanout, int cap, int sin
     // a whole row: rank and emit
     int kept = -1;
     if (rem == 0 && c >= fanout) {
-      for (int s = 0; s < c; ++s) {
-        const uint32_t z = lds_u32(a0 + s * kCSlot);
-        sts_u32(a0 + s * kCSlot, (z ^ (z >> 31)) >> rshift);
+      // the key's high word is z ^ (z >> 31): below 2^31 (every row longer than twice the candidate
+      // target) that is z itself, and the list can be ranked as it stands
+      if (M >= 0x80000000u || rshift != 0) {
+        for (int s = 0; s < c; ++s) {
+          const uint32_t z = lds_u32(a0 + s * kCSlot);
+          sts_u32(a0 + s * kCSlot, (z ^ (z >> 31)) >> rshift);
+        }
       }
       unsigned long long keep = rank_list(a0, c, fanout, &kept);
       if (kept == fanout) {
