@@ -640,6 +640,28 @@ def run_ours(args):
         errors['gpu_pull'] = repr(exc)
         g = recover_graph(g)
 
+    # ---- variant (SURVEY Sec. 8(e)'s single-box stand-in): every owner's store in DEVICE memory, as a
+    # peer GPU's HBM would be over NVLink -- the bulk transfers become device-side row pulls and the
+    # host link drops out: what the GPU side of the path sustains when staging is not link-bound
+    try:
+        if not args.no_sweep and world == 1 and w.num_nodes * w.row_bytes < 8e9:
+            import dataclasses
+            g.close()
+            wd = dataclasses.replace(w, feat_parts=[p_.to(dev) for p_ in w.feat_parts])
+            g = ep.graph_from_workload(wd, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws), staging_mode=0,
+                                       max_live_windows=args.lookahead + 1, cache_buffers=args.cache_buffers)
+            r = timed(W, 3, 2)
+            variants["remote_owners_in_hbm"] = {"value": 3 * n_b / r["sec"], "unit": UNIT,
+                                                "note": "all four feature partitions in device memory (stand-in for peer HBM): one pull "
+                                                        "kernel per owner instead of pack + cudaMemcpyAsync, no host link in the path"}
+            g.close()
+            del wd
+            g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws), staging_mode=args.staging_mode,
+                                       max_live_windows=args.lookahead + 1, host_threads=args.host_threads, cache_buffers=args.cache_buffers)
+    except Exception as exc:      # an optional leg must not cost the headline line
+        errors['remote_owners_in_hbm'] = repr(exc)
+        g = recover_graph(g)
+
     if rank != 0:
         return
     # ---- rooflines: the dominant kernel group (a-1 sampling, ALU-bound) and the gather (HBM) ----
