@@ -171,9 +171,9 @@ struct CacheSlot {
   DevBuf<int32_t> hot;
   int64_t n_cached = 0;        // entries of `hot` currently reflected in slot_map
   Window* tenant = nullptr;    // window whose H_k is in here (may already be released)
-  // last gather that read this buffer / slot map.  Kept per cache slot, not only per window
-  // arena: the arena of a released tenant can be re-staged (and its own flag reset) before the
-  // next stage_b on this slot runs.
+  // the point of the caller's stream behind which every gather that read this buffer / slot map has
+  // completed: recorded by gg_window_release of its tenant.  Kept per cache slot, not per window
+  // arena: the arena of a released tenant can be re-staged before the next stage_b on this slot runs.
   cudaEvent_t gather_done = nullptr;
   bool gather_recorded = false;
 };
@@ -206,8 +206,7 @@ struct Window {
   double t_enqueue = 0;
   // sync
   cudaEvent_t sampled = nullptr;  // phase A complete (stream A)
-  cudaEvent_t ready = nullptr;    // cache ready (stream B)
-  cudaEvent_t gather_done = nullptr;
+  cudaEvent_t ready = nullptr;    // cache ready (stream C)
   cudaEvent_t consumer_done = nullptr;   // recorded by gg_window_release on the caller's stream
   bool consumer_recorded = false;
   cudaEvent_t ev_copy[2 * GG_MAX_PARTS + 2] = {nullptr};  // start/stop per bulk copy, last pair = carry
@@ -216,7 +215,11 @@ struct Window {
   int64_t h_req_cap = 0;
   CacheSlot* prev_cs = nullptr;   // C_{k-1}'s buffer: source of the carry-over copy
   double t_b0 = 0;                // start of phase B on the host
-  bool gather_recorded = false;
+  bool gather_recorded = false;   // a gather of this window has been issued
+  cudaStream_t last_gather_stream = nullptr;
+  cudaStream_t gstreams[4] = {nullptr, nullptr, nullptr, nullptr};   // distinct streams its gathers ran on
+  int n_gstreams = 0;
+  cudaEvent_t ev_join[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // release: one per gather stream + the caller's
   bool enqueued = false;          // phase B finished on the host (or an error was recorded)
   gg_status status = GG_OK;
   std::string error;
@@ -326,6 +329,7 @@ struct gg_graph {
   // streams / threads
   cudaStream_t side = nullptr;    // phase A: sample, frontier, unique
   cudaStream_t side_b = nullptr;  // phase B: select, delta (the stager thread syncs on it)
+  cudaStream_t side_join = nullptr;  // gg_window_release joins the caller's stream and the gather streams here
   cudaStream_t side_c = nullptr;  // phase B: bulk copies, carry-over copy, cache-ready event (never waited on by the stager)
   Window win[GG_MAX_LIVE_WINDOWS];
   int n_win = 3;
@@ -501,7 +505,6 @@ static gg_status stage_a(gg_graph* g, Window* w) {
   // the arena's previous tenant may still be read by gathers already enqueued
   // (and its staging on stream C reads the arena's request / carry lists)
   CU(cudaStreamWaitEvent(st, w->ready, 0));
-  if (w->gather_recorded) CU(cudaStreamWaitEvent(st, w->gather_done, 0));
   w->gather_recorded = false;
   // ... and by the consumer's own kernels / copies behind those gathers (the blocks, N_b): the
   // release recorded the point of the caller's stream after which the arena may be overwritten
@@ -1001,8 +1004,8 @@ gg_status gg_graph_destroy(gg_graph* g) {
     }
     if (w.sampled) cudaEventDestroy(w.sampled);
     if (w.ready) cudaEventDestroy(w.ready);
-    if (w.gather_done) cudaEventDestroy(w.gather_done);
     if (w.consumer_done) cudaEventDestroy(w.consumer_done);
+    for (int c = 0; c < 5; ++c) if (w.ev_join[c]) cudaEventDestroy(w.ev_join[c]);
     if (w.h_req) cudaFreeHost(w.h_req);
     for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) if (w.ev_copy[c]) cudaEventDestroy(w.ev_copy[c]);
   }
@@ -1035,6 +1038,7 @@ gg_status gg_graph_destroy(gg_graph* g) {
   if (g->side) cudaStreamDestroy(g->side);
   if (g->side_b) cudaStreamDestroy(g->side_b);
   if (g->side_c) cudaStreamDestroy(g->side_c);
+  if (g->side_join) cudaStreamDestroy(g->side_join);
   delete g;
   return GG_OK;
 }
@@ -1146,6 +1150,7 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
     CUC(cudaStreamCreateWithPriority(&g->side_b, cudaStreamNonBlocking, hi_pri));
   }
   CUC(cudaStreamCreateWithFlags(&g->side_c, cudaStreamNonBlocking));
+  CUC(cudaStreamCreateWithFlags(&g->side_join, cudaStreamNonBlocking));
   for (int i = 0; i < 2; ++i) CUC(cudaEventCreateWithFlags(&g->resp_free[i], cudaEventDisableTiming));
   for (int s = 0; s < g->n_cs; ++s) {
     CacheSlot& c = g->cslot[s];
@@ -1159,8 +1164,8 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
     Window& w = g->win[s];
     CUC(cudaEventCreateWithFlags(&w.sampled, cudaEventDisableTiming));
     CUC(cudaEventCreateWithFlags(&w.ready, cudaEventDefault));
-    CUC(cudaEventCreateWithFlags(&w.gather_done, cudaEventDisableTiming));
     CUC(cudaEventCreateWithFlags(&w.consumer_done, cudaEventDisableTiming));
+    for (int c = 0; c < 5; ++c) CUC(cudaEventCreateWithFlags(&w.ev_join[c], cudaEventDisableTiming));
     for (int c = 0; c < 2 * GG_MAX_PARTS + 2; ++c) CUC(cudaEventCreate(&w.ev_copy[c]));
   }
   CUC(max_degree(g->indptr, g->N, &g->max_degree));
@@ -1351,10 +1356,19 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
     launch_miss_path(st, G);
     g->prof.end(st, pe, GG_PROF_MISS, 0);
   }
-  CU(cudaEventRecord(w->gather_done, st));
+  // No event behind the gather: two records between every pair of back-to-back 50 us kernels cost
+  // the stream 6-8 us per batch.  What later stages wait for (the arena's next tenant, the cache
+  // buffer's next tenant) is recorded once per window, by gg_window_release on the caller's stream.
   w->gather_recorded = true;
-  CU(cudaEventRecord(w->cs->gather_done, st));
-  w->cs->gather_recorded = true;
+  w->last_gather_stream = st;
+  {
+    int k = 0;
+    while (k < w->n_gstreams && w->gstreams[k] != st) ++k;
+    if (k == w->n_gstreams) {
+      if (k < 4) w->gstreams[w->n_gstreams++] = st;
+      else CU(cudaStreamSynchronize(st));     // a fifth distinct stream: nothing left to remember it by
+    }
+  }
   CU(cudaGetLastError());
   fill_batch_out(w, b, out, g);
   return GG_OK;
@@ -1377,7 +1391,21 @@ gg_status gg_window_release(gg_graph* g, int64_t window_id, void* cuda_stream) {
   // Everything the caller enqueued on `cuda_stream` so far may still read the window's blocks and
   // N_b (a consumer step behind the last gather, a device-to-host copy): the arena's next tenant
   // is sampled only behind this point of that stream.
-  CU(cudaEventRecord(w->consumer_done, (cudaStream_t)cuda_stream));
+  // ... and every gather of the window, on whatever stream it ran.  The join happens on a stream
+  // of the library's own, so no caller stream is made to wait for another.
+  cudaStream_t sj = g->side_join;
+  CU(cudaEventRecord(w->ev_join[4], (cudaStream_t)cuda_stream));
+  CU(cudaStreamWaitEvent(sj, w->ev_join[4], 0));
+  for (int k = 0; k < w->n_gstreams; ++k) {
+    if (w->gstreams[k] == (cudaStream_t)cuda_stream) continue;
+    CU(cudaEventRecord(w->ev_join[k], w->gstreams[k]));
+    CU(cudaStreamWaitEvent(sj, w->ev_join[k], 0));
+  }
+  w->n_gstreams = 0;
+  CU(cudaEventRecord(w->consumer_done, sj));
+  // the cache buffer's next tenant (window seq + n_cs) is built only behind the same point
+  CU(cudaEventRecord(w->cs->gather_done, sj));
+  w->cs->gather_recorded = true;
   {
     std::lock_guard<std::mutex> l(g->mu);
     w->consumer_recorded = true;
@@ -1396,7 +1424,7 @@ gg_status gg_trace(gg_graph* g, int64_t window_id, gg_window_trace* out) {
   if (rc != GG_OK) return rc;
   CU(cudaEventSynchronize(w->ready));
   resolve_timing(w);
-  if (w->gather_recorded) CU(cudaEventSynchronize(w->gather_done));
+  if (w->gather_recorded) CU(cudaStreamSynchronize(w->last_gather_stream));   // the per-batch counters are final
   out->W = w->W; out->num_parts = g->R.P;
   out->n_access = w->n_access; out->n_unique = w->n_unique; out->n_unique_remote = w->n_remote;
   out->n_hot = w->n_hot; out->carried_rows = w->n_carry; out->bulk_copies = w->bulk_copies;
