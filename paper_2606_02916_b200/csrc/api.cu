@@ -795,8 +795,6 @@ static gg_status stage_b2(gg_graph* g, Window* w) {
       const int32_t* ids = w->h_req + q0;
       uint8_t* resp = g->h_resp[ri] + q0 * rb;
       const int64_t chunk = 512;
-      // every pool thread while the link is idle (the cold first window: nothing to contend with, and
-      // the first copy cannot start before this pack ends), the tuned few while copies are in flight
       // Pack threads: the tuned few while the link has more bytes queued than this pack produces (the
       // copies are what the epoch waits for; fewer threads leave them the host's DRAM), every pool
       // thread when the link is about to run dry (the cold first window, small windows).
