@@ -204,7 +204,8 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/int32/uint64",
         "data": "synthetic",
-        "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot, "step": sample},
+        "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot,
+                   "edge_cut_measured": edge_cut_main, "remote_frac_of_N_b": remote_frac_main, "step": sample},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": min(cores, W), "kind": "oracle", "sample": sample,
                          "cpu_model": cpu_model(), "host_cores": cores},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -385,7 +386,7 @@ def run_ours(args):
     main = timed(W, args.steps, args.warmup, profile=True, clocks=None if args.no_clocks else ClockSampler(local_rank))
     value, tmax = gdist.aggregate_throughput(args.steps * n_b, main["sec"], dev)
     # per-window trace of one more epoch (bytes over the host link, stall, timings)
-    tr_acc = dict(bulk_bytes=0, bulk_copies=0, wait_ms=0.0, stage_ms=0.0, pack_ms=0.0, h2d_ms=0.0, n_access=0)
+    tr_acc = dict(bulk_bytes=0, bulk_copies=0, wait_ms=0.0, stage_ms=0.0, pack_ms=0.0, h2d_ms=0.0, n_access=0, hit_local=0)
 
     def on_window(wid, win):
         t = g.trace(wid, len(win))
@@ -396,6 +397,7 @@ def run_ours(args):
         tr_acc["pack_ms"] += t["ms_pack_host"]
         tr_acc["h2d_ms"] += t["ms_h2d"]
         tr_acc["n_access"] += t["n_access"]
+        tr_acc["hit_local"] += int(t["hit_local"].sum())
 
     ep.run_epoch(g, batches, w.fanouts, W, feats, on_window=on_window, stream=stream, first_window_id=5 * 10 ** 6,
                  lookahead=LA)
@@ -664,6 +666,13 @@ def run_ours(args):
 
     if rank != 0:
         return
+    # the owners' measured edge cut and the remote fraction of N_b (what the hot path feels of the split)
+    edge_cut_main, remote_frac_main = None, None
+    try:
+        edge_cut_main = edge_cut(w, dev)
+        remote_frac_main = 1.0 - tr_acc["hit_local"] / max(tr_acc["n_access"], 1)
+    except Exception as exc:
+        errors["edge_cut_main"] = repr(exc)
     # ---- rooflines: the dominant kernel group (a-1 sampling, ALU-bound) and the gather (HBM) ----
     peak, peak_src = measured_peaks()
     pg = main["prof"]["gather"]
@@ -729,6 +738,7 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "u8 rows / int32 ids / uint64 keys",
         "data": "synthetic",
         "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot,
+                   "edge_cut_measured": edge_cut_main, "remote_frac_of_N_b": remote_frac_main,
                    "staging_mode": args.staging_mode, "carry_over": 1, "lookahead_windows": LA,
                    "step": "one epoch = %d mini-batches in %d windows, cache reset per epoch" % (n_b, -(-n_b // W)),
                    "l2": "inputs larger than L2 (feature store %.0f MB, X_b %.0f MB per batch)"
