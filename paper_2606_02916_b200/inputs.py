@@ -416,3 +416,90 @@ def make_workload(name: str, device="cpu", pin: Optional[bool] = None,
                     part_offsets=part_offsets, local_part=local_part, feat_parts=parts, dim=cfg["dim"],
                     dtype=dtype, batches=batches, fanouts=list(cfg["fanouts"]),
                     seed=substream(ms, 400))
+
+
+# --------------------------------------------------------------------------
+# BFS-grown balanced split (BASELINE.json:configs[2] names it; reading S22)
+# --------------------------------------------------------------------------
+
+def bfs_grown_split(indptr: torch.Tensor, indices: torch.Tensor, parts: int, seed: int,
+                    cap_factor: float = 1.02) -> torch.Tensor:
+    """Multi-source BFS growth of `parts` balanced regions: one seeded start node per part, all
+    parts grow level by level, a node reached by several parts in one level goes to the lowest
+    part number, a part stops growing at ceil(N / parts) * cap_factor nodes, whatever is left
+    unreached goes to the parts with room in ID order.  Returns int8 labels [N] on the graph's
+    device.  Input-side only (owner assignment of a synthetic graph): none of the method's
+    arithmetic lives here."""
+    dev = indptr.device
+    n = indptr.numel() - 1
+    cap = int(-(-n // parts) * cap_factor)
+    label = torch.full((n,), -1, dtype=torch.int8, device=dev)
+    size = [0] * parts
+    starts = []
+    k = 0
+    while len(starts) < parts:                     # distinct seeded start nodes
+        s = _mix64_int(seed + 0x9E37 * k) % n
+        k += 1
+        if s not in starts:
+            starts.append(s)
+    frontier = torch.tensor(starts, dtype=torch.int64, device=dev)
+    label[frontier] = torch.arange(parts, dtype=torch.int8, device=dev)
+    for p in range(parts):
+        size[p] = 1
+    big = torch.iinfo(torch.int8).max
+    while frontier.numel() > 0:
+        row0 = indptr[frontier]
+        deg = indptr[frontier + 1] - row0
+        total = int(deg.sum())
+        if total == 0:
+            break
+        first = torch.cumsum(deg, 0) - deg
+        offs = torch.arange(total, device=dev) - torch.repeat_interleave(first, deg) + torch.repeat_interleave(row0, deg)
+        nbr = indices[offs].long()
+        src = torch.repeat_interleave(label[frontier], deg)
+        free = label[nbr] < 0
+        nbr, src = nbr[free], src[free]
+        if nbr.numel() == 0:
+            break
+        cand = torch.full((n,), big, dtype=torch.int8, device=dev)
+        cand.scatter_reduce_(0, nbr, src, reduce="amin")
+        new = torch.nonzero(cand < big).squeeze(1)
+        admitted = []
+        for p in range(parts):
+            room = cap - size[p]
+            if room <= 0:
+                continue
+            idx = new[cand[new] == p][:room]
+            if idx.numel():
+                label[idx] = p
+                size[p] += int(idx.numel())
+                admitted.append(idx)
+        frontier = torch.cat(admitted) if admitted else torch.empty(0, dtype=torch.int64, device=dev)
+    rest = torch.nonzero(label < 0).squeeze(1)
+    pos = 0
+    for p in sorted(range(parts), key=lambda q: size[q]):
+        if pos >= rest.numel():
+            break
+        room = max(0, -(-n // parts) - size[p]) if p != sorted(range(parts), key=lambda q: size[q])[-1] else rest.numel() - pos
+        take = rest[pos:pos + room]
+        label[take] = p
+        size[p] += int(take.numel())
+        pos += int(take.numel())
+    if pos < rest.numel():
+        label[rest[pos:]] = parts - 1
+    return label
+
+
+def edge_cut_of_labels(indptr: torch.Tensor, indices: torch.Tensor, label: torch.Tensor) -> float:
+    """Fraction of CSR entries whose two endpoints carry different labels."""
+    n = indptr.numel() - 1
+    cut, step = 0, 1 << 22
+    for r0 in range(0, n, step):
+        r1 = min(n, r0 + step)
+        ip = indptr[r0:r1 + 1]
+        e0, e1 = int(ip[0]), int(ip[-1])
+        if e1 == e0:
+            continue
+        own_e = torch.repeat_interleave(label[r0:r1], ip[1:] - ip[:-1])
+        cut += int((own_e != label[indices[e0:e1].long()]).sum())
+    return cut / max(1, indices.numel())

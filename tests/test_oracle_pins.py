@@ -358,3 +358,22 @@ def test_generated_configs_have_the_stated_shape(workload):
     cut = (np.searchsorted(w.part_offsets, rows, side="right") !=
            np.searchsorted(w.part_offsets, indices, side="right")).mean()
     assert 0.04 < cut < 0.14, cut                           # planted ~8 % edge-cut
+
+
+def test_bfs_grown_split_is_balanced_and_cuts_more_than_the_planted_owners(workload):
+    """Reading S22: BASELINE.json asks for a BFS-grown balanced 4-way split with ~8 % edge cut; on the
+    planted Chung-Lu graph the BFS growth (hubs reach every community within two levels) is balanced
+    but cuts several times more than the planted communities, which is why those are the owners."""
+    import torch
+    from paper_2606_02916_b200 import inputs
+    w = workload("products_mini")
+    lab = inputs.bfs_grown_split(w.indptr, w.indices, 4, 123)
+    sizes = torch.bincount(lab.long(), minlength=4)
+    assert int(lab.min()) >= 0 and int(sizes.sum()) == w.num_nodes
+    assert int(sizes.max()) <= int(-(-w.num_nodes // 4) * 1.02) + 1
+    po = torch.as_tensor(w.part_offsets)
+    planted = torch.bucketize(torch.arange(w.num_nodes), po[1:-1], right=True).to(torch.int8)
+    cut_planted = inputs.edge_cut_of_labels(w.indptr, w.indices, planted)
+    cut_bfs = inputs.edge_cut_of_labels(w.indptr, w.indices, lab)
+    assert 0.04 <= cut_planted <= 0.14
+    assert cut_bfs > 2 * cut_planted
