@@ -407,6 +407,37 @@ gg_status gg_sage_step(gg_sage* m, const gg_batch_out* batch, const int32_t* lab
 /* Copies layer l's parameters to host arrays (synchronises the device). */
 gg_status gg_sage_params(gg_sage* m, int32_t layer, float* w_self, float* w_neigh, float* bias);
 
+/* ---- window unique + count without any device allocation -------------------------------------------
+ * The same U_k / c_k as step a-3 (the distinct node IDs of the window's trace, ascending,
+ * each with the number of times it is accessed), computed from ID lists the caller already holds on the
+ * device -- for callers that cannot let a library allocate.  Typical cases: the process's own allocator
+ * has taken all free HBM, so a cudaMalloc made here would fail; or the loop has other streams in flight
+ * and must avoid cudaFree, which waits for the whole device.  This call never calls cudaMalloc, cudaFree
+ * or any routine that allocates: its workspace (packed 8-bit counters, one per node ID, plus 512 partial
+ * sums) is a fixed array of 4 MiB + 2 KiB compiled into the library, resident on every GPU that loads
+ * libgreengnn.so until the process exits.  That fixed size is the limit: num_nodes <=
+ * GG_STATIC_MAX_NODES (4,194,304); beyond it the call returns GG_ERR_CAPACITY and touches nothing
+ * (gg_window_stage has no such limit).
+ *   ids       device int32 [n_ids]: the node IDs accessed, in any order (e.g. the N_b lists of the
+ *             window's batches, concatenated).  An ID may occur at most 255 times (N_b holds each node
+ *             once, so this is the W <= GG_MAX_WINDOW rule); more than that corrupts neighbouring counts.
+ *   num_nodes IDs are valid in [0, num_nodes); others are skipped and tallied in stats[1]
+ *   uniq, cnt device int32 [capacity], caller-owned outputs: uniq ascending, cnt[i] = occurrences of uniq[i]
+ *   stats     device int32 [2], caller-owned output: stats[0] = |U| (the number of entries written),
+ *             stats[1] = IDs skipped.  If stats[0] > capacity NOTHING was written to uniq / cnt.
+ *   cuda_stream  a cudaStream_t (NULL = default stream); the call is asynchronous on it.
+ * The workspace is shared by all calls on a device and keeps the previous call's contents; every call
+ * clears what it needs first, so back-to-back calls on one stream are independent.  Calls whose GPU
+ * work can overlap (two streams without an ordering, two threads) race on it: order them yourself.
+ * The first call on each device looks up the workspace's device address (and makes the CUDA runtime
+ * load this module there); make that first call -- n_ids = 0 is enough -- during start-up, before any
+ * stream capture begins.
+ * Errors: INVALID_ARG (null pointer, negative size, num_nodes < 1), CAPACITY (num_nodes too large),
+ * CUDA. */
+#define GG_STATIC_MAX_NODES (1 << 22)
+gg_status gg_unique_count_static(const int32_t* ids, int64_t n_ids, int64_t num_nodes, int32_t* uniq,
+                                 int32_t* cnt, int64_t capacity, int32_t* stats, void* cuda_stream);
+
 const char* gg_last_error(void);
 const char* gg_version(void);
 

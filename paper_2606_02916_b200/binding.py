@@ -18,6 +18,7 @@ import torch
 from . import build as _build
 
 GG_MAX_LAYERS, GG_MAX_PARTS, GG_MAX_FANOUT, GG_MAX_WINDOW = 8, 16, 96, 255
+GG_STATIC_MAX_NODES = 1 << 22
 GG_OK, GG_ERR_INVALID_ARG, GG_ERR_STATE, GG_ERR_CAPACITY, GG_ERR_OOM, GG_ERR_CUDA = range(6)
 _STATUS = {0: "GG_OK", 1: "GG_ERR_INVALID_ARG", 2: "GG_ERR_STATE", 3: "GG_ERR_CAPACITY",
            4: "GG_ERR_OOM", 5: "GG_ERR_CUDA"}
@@ -86,7 +87,7 @@ PROF_KINDS = ["gather", "miss", "sample", "frontier", "unique", "select", "stage
 SYMBOLS = ["gg_profile_enable", "gg_profile_get", "gg_launch_count", "gg_graph_create", "gg_graph_destroy", "gg_window_stage", "gg_batch_info",
            "gg_batch_gather", "gg_window_release", "gg_trace", "gg_window_export", "gg_cache_read",
            "gg_cache_reset", "gg_key", "gg_last_error", "gg_version", "gg_sampler_stats", "gg_debug_sampler", "gg_sampler_tune", "gg_key_peak", "gg_simulate", "gg_rank_calibrate",
-           "gg_sage_create", "gg_sage_destroy", "gg_sage_step", "gg_sage_params"]
+           "gg_sage_create", "gg_sage_destroy", "gg_sage_step", "gg_sage_params", "gg_unique_count_static"]
 
 _lib = None
 
@@ -134,6 +135,7 @@ def load_library(path: Optional[str] = None):
     lib.gg_sage_destroy.argtypes = [vp]
     lib.gg_sage_step.argtypes = [vp, P(gg_batch_out), vp, C.c_float, vp, vp]
     lib.gg_sage_params.argtypes = [vp, i32, vp, vp, vp]
+    lib.gg_unique_count_static.argtypes = [vp, i64, i64, vp, vp, i64, vp, vp]
     lib.gg_last_error.restype = C.c_char_p
     lib.gg_version.restype = C.c_char_p
     for s in SYMBOLS:
@@ -186,6 +188,25 @@ def rank_calibrate(Z: np.ndarray, e_gt: np.ndarray, lam: float, lr: float, iters
     _check_global(load_library().gg_rank_calibrate(Z.ctypes.data, e.ctypes.data, n, F, lam, lr, iters,
                                                    beta.ctypes.data, gamma.ctypes.data, loss.ctypes.data))
     return beta[:F], gamma, float(loss[0])
+
+
+def unique_count_static(ids: torch.Tensor, num_nodes: int, uniq: torch.Tensor, cnt: torch.Tensor,
+                        stats: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """gg_unique_count_static: U_k / c_k of the device ID list `ids` into the caller's device tensors
+    `uniq`, `cnt` (int32, same length = capacity) and `stats` (int32 [2]: |U|, IDs skipped), without
+    any device allocation inside the library -- for callers whose allocator owns all of the HBM or
+    who cannot afford the device-wide wait of a cudaFree.  num_nodes <= GG_STATIC_MAX_NODES.
+    Asynchronous on `stream` (default: torch's current stream); nothing is written to uniq / cnt when
+    stats[0] > len(uniq).  Calls that may overlap on the GPU share one workspace and race."""
+    for t in (ids, uniq, cnt, stats):
+        assert t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()
+    assert uniq.numel() == cnt.numel() and stats.numel() >= 2
+    st = stream if stream is not None else torch.cuda.current_stream(ids.device)
+    with torch.cuda.device(ids.device):
+        _check_global(load_library().gg_unique_count_static(
+            ids.data_ptr() if ids.numel() else None, ids.numel(), num_nodes,
+            uniq.data_ptr() if uniq.numel() else None, cnt.data_ptr() if cnt.numel() else None,
+            uniq.numel(), stats.data_ptr(), st.cuda_stream))
 
 
 class Sage:

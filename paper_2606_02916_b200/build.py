@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgreengnn.so")
-SOURCES = ["sample.cu", "frontier.cu", "window.cu", "gather.cu", "simulate.cu", "sage.cu", "api.cu"]
+SOURCES = ["sample.cu", "frontier.cu", "window.cu", "gather.cu", "simulate.cu", "sage.cu", "noalloc.cu", "api.cu"]
 HEADERS = ["common.cuh", "kernels.h", os.path.join("..", "..", "include", "greengnn.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread"]
