@@ -24,9 +24,10 @@ import torch  # noqa: E402
 
 METRIC = "mini-batches/s (sample+stage+gather), one epoch per step"
 UNIT = "mini-batches/s"
+DTYPE = "u8 rows / int32 ids / uint64 keys"
 
 
-def parse_args():
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
@@ -43,7 +44,10 @@ def parse_args():
     ap.add_argument("--host-threads", type=int, default=0)
     ap.add_argument("--sampler-tune", default="", help="single_bins,warp_bin,hub_bin for gg_sampler_tune (default: the library's)")
     ap.add_argument("--cache-buffers", type=int, default=4, help="HBM cache buffers in rotation (gg_config.cache_buffers)")
-    ap.add_argument("--no-sweep", action="store_true", help="skip the W sweep")
+    ap.add_argument("--full", action="store_true",
+                    help="also run the optional legs (W sweep, BASELINE.json:configs grid, simulator, variants); they go to "
+                         "bench_detail.json, never into the result line")
+    ap.add_argument("--no-sweep", action="store_true", help="with --full: skip the optional legs after all")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-clocks", action="store_true", help="debug: do not poll nvidia-smi during the timed region")
@@ -52,7 +56,10 @@ def parse_args():
     ap.add_argument("--configs", default="products,dense,large",
                     help="workloads of the `configs` grid (BASELINE.json:configs); '' switches the grid off")
     ap.add_argument("--configs-budget-s", type=float, default=420.0, help="wall-clock budget of the `configs` grid")
-    return ap.parse_args()
+    args = ap.parse_args(argv)
+    if not args.full:
+        args.no_sweep = True       # the default run is the headline + rooflines + e2e + cpu_baseline only
+    return args
 
 
 def measured_peaks():
@@ -80,6 +87,9 @@ def ncu_traffic(name):
 # instructions per 4 keys = 21 slots per key) and of the hash alone (16 slots per key), both at one
 # warp instruction per clock per SM sub-partition -- a rate this integer mix does not reach.
 KEY_ISSUE_SLOTS, HASH_ISSUE_SLOTS = 21.0, 16.0
+# the hash needs 11 ALU-pipe instructions per key at 2 clocks per warp instruction = 22
+# ALU-pipe clocks per warp-key: the pipe bound (1.69 Tkey/s at 1965 MHz) the measured key-only peak sits under
+ALU_PIPE_CLOCKS = 22.0
 SMSP_PER_SM = 4
 
 
@@ -176,7 +186,7 @@ def run_reference(args):
     W = args.window
     wins = ep.windows_of(len(w.batches), W)
     cores = os.cpu_count() or 1
-    st = ggo.State(g.n, po, 0, args.n_hot, 1)
+    st = ggo.State(g.n, po, w.local_part, args.n_hot, 1)
     done = [0]
 
     def step(i, ex):
@@ -202,10 +212,9 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/int32/uint64",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": DTYPE,
         "data": "synthetic",
-        "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot,
-                   "edge_cut_measured": edge_cut_main, "remote_frac_of_N_b": remote_frac_main, "step": sample},
+        "config": config_record(args, w),
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": min(cores, W), "kind": "oracle", "sample": sample,
                          "cpu_model": cpu_model(), "host_cores": cores},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -217,6 +226,17 @@ def workload_name(args, w):
             "4 owner ranges (local in HBM, 3 in pinned host)"
             % (args.config, w.num_nodes, w.indices.numel(), w.dim, str(w.dtype).replace("torch.", ""),
                sum(len(b) for b in w.batches), args.batch, len(w.batches), w.fanouts))
+
+
+def config_record(args, w):
+    """The `config` object of the result line.  Both arms (ours, --impl reference) print exactly this, built
+    from the arguments and the workload alone, so that the driver can see they ran the same thing."""
+    return {"workload": "%s N=%d nnz=%d dim=%d %s batch=%d (%d/epoch) fanouts=%s"
+                        % (args.config, w.num_nodes, w.indices.numel(), w.dim, str(w.dtype).replace("torch.", ""),
+                           args.batch, len(w.batches), ",".join(str(f) for f in w.fanouts)),
+            "W": args.window, "n_hot": args.n_hot,
+            "l2": ("inputs larger than L2 (feature store %.0f MB; no flush)" if w.num_nodes * w.row_bytes > 126e6 else
+                   "feature store %.0f MB fits in L2: a parity-size config, not a bench line") % (w.num_nodes * w.row_bytes / 1e6)}
 
 
 class E2ESink:
@@ -288,6 +308,8 @@ def run_ours(args):
     _, order = gdist.shard_plan(rank, world, P, n_b)
     batches = [w.batches[i] for i in order]
     W = args.window
+    if args.host_threads <= 0:
+        args.host_threads = gdist.host_threads_for_rank()    # 0 (library default) unless ranks share the host
     sweep_ws = [] if args.no_sweep or world > 1 else [x for x in w.cfg["windows"] if x != W]
     g = ep.graph_from_workload(w, n_hot=args.n_hot, carry_over=1, max_window=max([W] + sweep_ws),
                                staging_mode=args.staging_mode, max_live_windows=args.lookahead + 1,
@@ -698,6 +720,8 @@ def run_ours(args):
     gk_peak = key_peak_gkeys
     roof = {"bound": "alu", "kernel": "a-1 sampling (k_sample_count/plan + the selection kernels of every hop)",
             "achieved": gk, "peak": gk_peak, "unit": "Gkey/s", "frac": gk / gk_peak,
+            "frac_of_pipe_bound": gk / derived_alu_peak_gkeys(sm_mhz, sm_count, ALU_PIPE_CLOCKS),
+            "pipe_bound_Gkey/s": derived_alu_peak_gkeys(sm_mhz, sm_count, ALU_PIPE_CLOCKS),
             "traffic": ncu_traffic("r02_sample_ncu_summary.txt"),
             "traffic_note": "dram read+write bytes of all a-1 kernels of one W=16 window (every hop) / 3 hop regions: the same "
                             "launches avg_launch_us averages; DRAM traffic is ~5x the algorithmic bytes on the last hop (32-byte "
@@ -740,14 +764,14 @@ def run_ours(args):
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "u8 rows / int32 ids / uint64 keys",
+        "scaling": "weak", "vs_baseline": None, "dtype": DTYPE,
         "data": "synthetic",
-        "config": {"workload": workload_name(args, w), "W": W, "n_hot": args.n_hot,
-                   "edge_cut_measured": edge_cut_main, "remote_frac_of_N_b": remote_frac_main,
-                   "staging_mode": args.staging_mode, "carry_over": 1, "lookahead_windows": LA,
-                   "step": "one epoch = %d mini-batches in %d windows, cache reset per epoch" % (n_b, -(-n_b // W)),
-                   "l2": "inputs larger than L2 (feature store %.0f MB, X_b %.0f MB per batch)"
-                         % (w.num_nodes * w.row_bytes / 1e6, tr_acc["n_access"] / n_b * w.row_bytes / 1e6)},
+        "config": config_record(args, w),
+        "protocol": {"workload_long": workload_name(args, w),
+                     "edge_cut_measured": edge_cut_main, "remote_frac_of_N_b": remote_frac_main,
+                     "staging_mode": args.staging_mode, "carry_over": 1, "lookahead_windows": LA,
+                     "step": "one epoch = %d mini-batches in %d windows, cache reset per epoch" % (n_b, -(-n_b // W)),
+                     "X_b_MB_per_batch": tr_acc["n_access"] / n_b * w.row_bytes / 1e6},
         "clocks": main["clocks"], "gpu_launches": int(main["launches"]),
         "wall_ms_per_step": 1e3 * main["wall"] / args.steps,
         "epoch_ms": {"median": statistics.median(main["per_epoch_ms"]), "min": min(main["per_epoch_ms"]),
@@ -769,8 +793,74 @@ def run_ours(args):
                     "boundary_stall_ms_per_step": tr_acc["wait_ms"]},
         "e2e": e2e, "cpu_baseline": cpu,
     }
-    print(json.dumps(out))
     g.close()
+    detail = write_detail(out)
+    print(json.dumps(compact_record(out, detail)))
+
+
+DETAIL_FILE = "bench_detail.json"
+
+
+def write_detail(out):
+    """Everything the run measured goes to bench_detail.json (git-ignored; also into gpurun_out/ when that
+    folder exists, so it comes back from the GPU box).  Returns the path written, or None."""
+    paths = [os.path.join(ROOT, DETAIL_FILE)]
+    if os.path.isdir(os.path.join(ROOT, "gpurun_out")):
+        paths.append(os.path.join(ROOT, "gpurun_out", DETAIL_FILE))
+    done = None
+    for p in paths:
+        try:
+            with open(p, "w") as f:
+                json.dump(out, f, indent=1)
+            done = done or os.path.relpath(p, ROOT)
+        except OSError:
+            pass
+    return done
+
+
+def _sig(x, digits=6):
+    """Floats to `digits` significant digits (the line is read by a driver with a small buffer)."""
+    if isinstance(x, float):
+        return float("%.*g" % (digits, x))
+    if isinstance(x, dict):
+        return {k: _sig(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_sig(v, digits) for v in x]
+    return x
+
+
+def _pick(d, keys):
+    return {k: d[k] for k in keys if d is not None and k in d} if d is not None else None
+
+
+def compact_record(out, detail_path=None):
+    """The ONE line bench.py prints last: the contract's keys and the two rooflines, nothing that grows
+    with the number of optional legs.  Kept under 4 KB (tests/test_bench_host.py)."""
+    c = {k: out.get(k) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step",
+                                 "higher_is_better", "scaling", "vs_baseline", "dtype", "data", "config")}
+    c["clocks"] = _pick(out.get("clocks"), ("sm_mhz", "sm_max_mhz", "samples", "reasons"))
+    c["gpu_launches"] = out.get("gpu_launches")
+    c["roofline"] = _pick(out.get("roofline"), ("bound", "kernel", "achieved", "peak", "unit", "frac", "frac_of_pipe_bound",
+                                                "pipe_bound_Gkey/s", "traffic", "launches", "avg_launch_us",
+                                                "algorithmic_keys_per_launch", "share_of_step"))
+    if c["roofline"] is not None:
+        c["roofline"]["peak_source"] = "measured in this run: gg_key_peak key-only kernel"
+    c["roofline_gather"] = _pick(out.get("roofline_gather"), ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic",
+                                                              "peak_source", "launches", "avg_launch_us",
+                                                              "algorithmic_bytes_per_launch", "share_of_step"))
+    alone = out.get("kernels_alone") or {}
+    c["kernels_alone"] = _pick(alone, ("sample_frac_of_alu_peak", "gather_frac_of_hbm_peak", "h2d_frac_of_link_peak"))
+    c["staging"] = _pick(out.get("staging"), ("host_link_bytes_per_step", "bulk_copies_per_step", "h2d_GB/s",
+                                              "host_link_peak_GB/s", "h2d_frac_of_link_peak", "boundary_stall_ms_per_step"))
+    c["gpu_stall_ms_per_step"] = out.get("gpu_stall_ms_per_step")
+    c["energy"] = _pick(out.get("energy"), ("J_per_step", "avg_W"))
+    c["e2e"] = _pick(out.get("e2e"), ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step"))
+    c["cpu_baseline"] = _pick(out.get("cpu_baseline"), ("value", "unit", "cores", "kind", "sample"))
+    if out.get("vs_W"):
+        c["vs_W"] = out["vs_W"]
+    c["errors"] = sorted((out.get("errors") or {}).keys())
+    c["detail"] = detail_path
+    return _sig(c)
 
 
 def consumer_leg(g, w, batches, W, feats, stream, dev, LA, batch):
