@@ -114,8 +114,11 @@ typedef struct {
                              memory (e.g. a peer GPU's HBM) is served by the pull kernel instead,
                              since host threads cannot read it;
                              1 = one GPU-initiated pull kernel per owner reading the pinned store */
-  int32_t host_threads;   /* owner-service pack threads; <= 0 = 0.4 x hardware threads (in [2, 16]): the pack shares
-                             the host's DRAM with the DMA reads of the bulk copies, see csrc/api.cu */
+  int32_t host_threads;   /* owner-service pack threads.  > 0: a hard cap, no pack ever runs on more threads (1 = on
+                             the stager thread itself).  <= 0: 0.4 x hardware threads (in [2, 16]) while bulk copies
+                             are queued -- the pack shares the host's DRAM with their DMA reads, see csrc/api.cu --
+                             and up to 16 when the link is idle (cold or small windows).  Several ranks on one
+                             host should pass an explicit share (dist.host_threads_for_rank) */
   int32_t cache_buffers;  /* HBM cache buffers (+ slot maps) in rotation, window k uses k mod n.  2 = the
                              ping-pong a literal Alg. 1 needs; with 2, window k's hot set can only be
                              selected after window k-2's gathers have finished, and that chain
@@ -200,7 +203,10 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t batch_in_windo
  *       consumer step behind the last gather (gg_sage_step), a device-to-host copy of the blocks.
  * A consumer that reads the window's pointers on some other stream must make `cuda_stream` wait
  * for that stream (cudaStreamWaitEvent) before the release, or synchronise it.  The caller's own
- * features buffer is not covered: it belongs to the caller. */
+ * features buffer is not covered: it belongs to the caller.
+ * `cuda_stream` and every stream a gg_batch_gather of this window ran on must still exist when the
+ * window is released (the library records an event on each).  If a record fails (GG_ERR_CUDA: invalid
+ * or destroyed stream) nothing has changed: the window is still live and the call can be repeated. */
 gg_status gg_window_release(gg_graph* g, int64_t window_id, void* cuda_stream);
 
 typedef struct {
@@ -299,6 +305,11 @@ gg_status gg_sampler_stats(uint64_t* keys, uint64_t* rows, uint64_t* fallbacks);
  * list in global memory.  Default (36, 36, 128): one lane per row below degree 512, one warp per row
  * above, no chunking (measured: chunking moves instructions one for one and adds the rank launch;
  * Large config with hubs of degree >= 32768 chunked: 290 vs 240 ms of sampling per epoch).
+ * single_bins > hub_bin is accepted and treated as single_bins = hub_bin on the hops where hub rows exist
+ * (hub rows are always chunked).
+ * The candidate lists of the chunked schemes (8 bytes x ~28 per destination of a hop) are allocated only
+ * while a setting that can use them is in force; after turning one on, the next gg_window_stage grows the
+ * shared scratch and therefore needs every earlier window released (GG_ERR_STATE otherwise).
  * Process-wide; must not be called while a window is being staged.  Errors: INVALID_ARG for
  * single_bins or hub_bin outside [28, 128] (a row below degree 128 is always one chunk) or warp_bin
  * outside [0, 128]. */
@@ -310,13 +321,11 @@ gg_status gg_sampler_tune(int32_t single_bins, int32_t warp_bin, int32_t hub_bin
  * S1 from a register-resident state -- the high word of fmix, which is all the selection test
  * reads -- and folds them into one word: no candidate lists, no row logic, no memory traffic.
  * Grid = ctas_per_sm x SM count CTAs of 256 threads, `reps` timed launches after one warm-up, CUDA
- * events on the default stream; two formulations of the same arithmetic are timed and
- * *keys_per_s receives the faster one.  Lane t of CTA c starts launch i (i = 0..reps-1) from the
+ * events on the default stream.  Lane t of CTA c starts launch i (i = 0..reps-1) from the
  * state 0x9E37 + i + (256 c + t + 1) * 0x632BE59BD9B4E019 and evaluates the states x + gamma * k,
  * k = 0..keys_per_lane-1; *fold (host, may be NULL) receives the xor over all of them of the high
  * 32 bits of fmix before its last xor-shift (tests/test_gpu_parity.py recomputes it on the host).
- * Synchronous.  Errors: INVALID_ARG (null, ctas_per_sm outside [1,8], keys_per_lane < 32);
- * GG_ERR_CUDA also when the two formulations disagree. */
+ * Synchronous.  Errors: INVALID_ARG (null, ctas_per_sm outside [1,8], keys_per_lane < 32). */
 gg_status gg_key_peak(int32_t ctas_per_sm, int32_t keys_per_lane, int32_t reps, double* keys_per_s,
                       uint32_t* fold);
 

@@ -415,6 +415,10 @@ static gg_status ensure_shared(gg_graph* g, int W, int L, const int* fanouts, bo
       return fail(GG_ERR_CAPACITY, "hop %d edge cap %lld exceeds int32 indexing", h, (long long)ecap);
     max_tiles = std::max(max_tiles, ceil_div(cap_front[h], 256));
   }
+  // the per-row candidate lists (28 x 8 bytes per destination: ~1.3 GB for products W=32, ~10x the hop's
+  // edge arrays) exist only while gg_sampler_tune has the multi-chunk path on; turning it on later makes
+  // the next gg_window_stage grow this scratch (which needs no live window, like any other growth)
+  if (!sampler_multi_chunk_on()) cand = 1;
   const int64_t ucap = std::min<int64_t>(g->N, (int64_t)W * node_pitch);
   int64_t t32 = std::max<int64_t>((int64_t)W * max_tiles, (int64_t)W * g->F.n_wtiles);
   t32 = std::max<int64_t>(t32, g->cnt_words / kWordTile);
@@ -1176,7 +1180,9 @@ gg_status gg_graph_create(const gg_csr* csr, const gg_owner_map* owners, const g
   const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
   const int nt = cfg->host_threads > 0 ? cfg->host_threads : (int)std::min<unsigned>(16u, std::max(2u, (hw * 2u + 2u) / 5u));
   g->pack_threads_busy = nt;
-  const int n_pool = cfg->host_threads > 0 ? std::max(nt, (int)std::min<unsigned>(16u, hw)) : (int)std::min<unsigned>(16u, hw);
+  // an explicit host_threads is a hard cap (the pool IS that many threads, link busy or not); only the
+  // default lets a pack that finds the link idle (cold or small windows) spread over up to 16 threads
+  const int n_pool = cfg->host_threads > 0 ? nt : (int)std::min<unsigned>(16u, hw);
   g->pool = new Pool(n_pool > 1 ? n_pool : 0);
   g->worker_a = std::thread(worker_a_main, g);
   g->worker_b = std::thread(worker_b_main, g);
@@ -1344,6 +1350,9 @@ gg_status gg_batch_gather(gg_graph* g, int64_t window_id, int32_t b, gg_batch_ou
   G.miss_pos = g->miss_pos.p; G.miss_id = g->miss_id.p; G.n_miss = g->n_miss.p;
   G.counters = w->counters.p + (int64_t)b * (2 + GG_MAX_PARTS);
   G.miss_total = g->miss_total.p;
+  G.miss_over_link = false;
+  for (int m = 0; m < g->R.P; ++m)
+    if (m != g->R.local && g->R.lo[m] < g->R.lo[m + 1] && !g->store_on_device[m]) G.miss_over_link = true;
   // one launch in four is bracketed: a timing event between every pair of back-to-back 50 us
   // kernels costs the step 6 % (the events serialise the stream), a quarter of them 1-2 %
   cudaEvent_t pe = (b & 3) == 1 || w->W < 4 ? g->prof.begin(st) : nullptr;
@@ -1399,10 +1408,13 @@ gg_status gg_window_release(gg_graph* g, int64_t window_id, void* cuda_stream) {
     CU(cudaEventRecord(w->ev_join[k], w->gstreams[k]));
     CU(cudaStreamWaitEvent(sj, w->ev_join[k], 0));
   }
-  w->n_gstreams = 0;
   CU(cudaEventRecord(w->consumer_done, sj));
   // the cache buffer's next tenant (window seq + n_cs) is built only behind the same point
   CU(cudaEventRecord(w->cs->gather_done, sj));
+  // every record above succeeded: only now does the window's state change (a failed call -- an invalid
+  // or destroyed stream -- returns with the window still live and its gather streams still remembered,
+  // so a retry joins them again)
+  w->n_gstreams = 0;
   w->cs->gather_recorded = true;
   {
     std::lock_guard<std::mutex> l(g->mu);

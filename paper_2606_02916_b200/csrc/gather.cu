@@ -194,91 +194,6 @@ __global__ void __launch_bounds__(kThreads) k_gather(GatherArgs A) {
   if (threadIdx.x < 2 + A.R.P && s_cnt[threadIdx.x]) atomicAdd(A.counters + threadIdx.x, s_cnt[threadIdx.x]);
 }
 
-// ---- TMA variant of the gather (A/B against k_gather<16>) --------------------------------------
-// One tile of kRows rows per CTA of kRows threads.  Thread r resolves row r's source and issues
-// ONE bulk asynchronous copy global -> shared for it (cp.async.bulk, SASS UBLKCP: rows are
-// 16-byte multiples at 16-byte aligned addresses), all signalling one mbarrier; when the tile has
-// landed, thread 0 issues ONE bulk copy shared -> global for the whole tile, which is contiguous
-// in X_b.  No register staging, 65 memory instructions per 25.6 KB tile.
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__global__ void __launch_bounds__(kRows) k_gather_tma(GatherArgs A) {
-  extern __shared__ __align__(128) uint8_t s_rows[];   // [kRows][rb]
-  __shared__ __align__(8) uint64_t s_bar;
-  __shared__ int32_t s_cnt[2 + GG_MAX_PARTS];
-  __shared__ int32_t s_w0miss, s_valid[2];
-  const int t = blockIdx.x, r = threadIdx.x;
-  const int r0 = t * kRows;
-  const int rows = min(kRows, A.n - r0);
-  if (r < 2 + GG_MAX_PARTS) s_cnt[r] = 0;
-  if (A.n_miss_zero && t == 0 && r == 0) *A.n_miss_zero = 0;
-  if (r == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s_bar)));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  const uint8_t* src = nullptr;
-  bool miss = false;
-  int32_t u = 0;
-  int m = 0;
-  if (r < rows) {
-    u = __ldg(A.nodes + r0 + r);
-    m = owner_of(A.R, u);
-    if (m == A.R.local) {
-      src = A.local_base + (u - A.R.lo[m]) * A.local_stride;
-    } else {
-      const int32_t s = __ldg(A.slot_of + u);
-      if (s >= 0) src = A.cache_base + (int64_t)s * A.cache_stride;
-      else miss = true;
-    }
-  }
-  const unsigned act = __ballot_sync(0xffffffffu, r < rows);
-  const unsigned ml = __ballot_sync(0xffffffffu, r < rows && m == A.R.local);
-  const unsigned mm = __ballot_sync(0xffffffffu, miss);
-  const int lane = r & 31, wid = r >> 5;
-  if (lane == 0) {
-    atomicAdd(&s_cnt[0], __popc(ml));
-    atomicAdd(&s_cnt[1], __popc(act) - __popc(ml) - __popc(mm));
-    s_valid[wid] = __popc(act) - __popc(mm);
-    if (wid == 0) s_w0miss = __popc(mm);
-  }
-  if (miss) {
-    atomicAdd(&s_cnt[2 + m], 1);
-    // the miss path fills this row later; the tile store must not publish stale shared memory
-    uint4* z = reinterpret_cast<uint4*>(s_rows + (size_t)r * A.rb);
-    for (int k = 0; k < A.rb / 16; ++k) z[k] = make_uint4(0, 0, 0, 0);
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  }
-  __syncthreads();
-  if (r == 0) {
-    const uint32_t bytes = (uint32_t)(s_valid[0] + s_valid[1]) * (uint32_t)A.rb;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s_bar)), "r"(bytes) : "memory");
-  }
-  if (src) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(s_rows + (size_t)r * A.rb)), "l"(src), "r"((uint32_t)A.rb), "r"(smem_u32(&s_bar))
-                 : "memory");
-  }
-  if (miss && A.miss_tmp_pos) {
-    const int q = (wid ? s_w0miss : 0) + __popc(mm & lanemask_lt());
-    A.miss_tmp_pos[(int64_t)t * kRows + q] = r0 + r;
-    A.miss_tmp_id[(int64_t)t * kRows + q] = u;
-  }
-  if (r == 32 && A.tile_miss) A.tile_miss[t] = s_w0miss + __popc(mm);
-  if (r < 2 + A.R.P && s_cnt[r]) atomicAdd(A.counters + r, s_cnt[r]);
-  if (r == 0) {
-    uint32_t done = 0;
-    while (!done) {
-      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                   : "=r"(done) : "r"(smem_u32(&s_bar)) : "memory");
-    }
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                 ::"l"(A.out + (int64_t)r0 * A.rb), "r"(smem_u32(s_rows)), "r"((uint32_t)(rows * A.rb)) : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-  }
-}
-
 // ordered concatenation of the tile-local miss lists (single CTA; tiles <= ~20k)
 __global__ void __launch_bounds__(1024)
 k_miss_compact(const int32_t* __restrict__ tile_miss, int tiles, const int32_t* __restrict__ tmp_pos,
@@ -383,19 +298,9 @@ void launch_gather(cudaStream_t st, const GatherLaunch& G) {
   const int tiles = (G.n + kRows - 1) / kRows;
   int vec = pick_vec(G.rb, G.local_base, G.cache_base, G.local_stride, G.cache_stride);
   if ((uintptr_t)G.out % vec) vec = ((uintptr_t)G.out % 8 == 0 && vec >= 8) ? 8 : 4;
-  static int use_tma = -1;
-  if (use_tma < 0) {
-    const char* e = getenv("GG_GATHER_TMA");
-    use_tma = e ? atoi(e) : 0;
-  }
-  if (vec == 16 && use_tma && (size_t)kRows * G.rb <= 200 * 1024) {
-    static bool attr = false;
-    if (!attr) {
-      cudaFuncSetAttribute(k_gather_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-      attr = true;
-    }
-    k_gather_tma<<<tiles, kRows, (size_t)kRows * G.rb, st>>>(A);
-  } else if (vec == 16) k_gather<16><<<tiles, kThreads, 0, st>>>(A);
+  // (a cp.async.bulk variant -- one bulk copy per row into shared memory, one bulk store per tile -- was
+  // built and measured in round 2: equal alone, slower beside the sampler; DESIGN.md Sec. 6 keeps the numbers)
+  if (vec == 16) k_gather<16><<<tiles, kThreads, 0, st>>>(A);
   else if (vec == 8) k_gather<8><<<tiles, kThreads, 0, st>>>(A);
   else k_gather<4><<<tiles, kThreads, 0, st>>>(A);
   count_launches(1);
@@ -421,7 +326,13 @@ void launch_miss_path(cudaStream_t st, const GatherLaunch& G) {
     }
     v2 = ok16 ? 16 : (ok8 ? 8 : 4);
   }
-  const int grid = sm_count() * 4;
+  // Misses that cross the host link: like the pull kernel below, a few CTAs with 8 loads in flight per
+  // thread keep PCIe full; a GPU-wide grid of zero-copy readers only crowds the bulk copies' DMA off the
+  // link and the sampler off the SMs (bench numbers in DESIGN.md Sec. 6).
+#ifndef GG_MISS_LINK_CTAS
+#define GG_MISS_LINK_CTAS 0   /* 0 = the full grid */
+#endif
+  const int grid = (G.miss_over_link && GG_MISS_LINK_CTAS > 0) ? GG_MISS_LINK_CTAS : sm_count() * 4;
   if (v2 == 16) k_rows<16, 1><<<grid, kThreads, 0, st>>>(Rw);
   else if (v2 == 8) k_rows<8, 1><<<grid, kThreads, 0, st>>>(Rw);
   else k_rows<4, 1><<<grid, kThreads, 0, st>>>(Rw);

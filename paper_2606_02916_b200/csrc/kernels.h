@@ -44,6 +44,7 @@ struct SampleWork {
 };
 size_t sample_plan_bytes();
 int sample_cand_cap(int fanout);   // entries of a row's candidate list in global memory (0: the hop does not use one)
+bool sampler_multi_chunk_on();     // do the current gg_sampler_tune cut-overs enable the multi-chunk path at all?
 void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* indices,
                        const int32_t* nodes, int64_t node_pitch, const BatchOffsets& n_dst,
                        const BatchOffsets& dst_off, int W, int max_nd, int fanout,
@@ -109,6 +110,7 @@ struct GatherLaunch {
   int32_t* n_miss;        // device scalar
   int32_t* counters;      // [2 + P]
   unsigned long long* miss_total;  // device scalar: rows filled by a-8 since the profile was last reset (may be null)
+  bool miss_over_link;    // a-8 reads pinned host memory (PCIe): a few CTAs saturate it; false: every remote store is device memory
 };
 void launch_gather(cudaStream_t st, const GatherLaunch& G);      // a-7: one k_gather launch
 void launch_miss_path(cudaStream_t st, const GatherLaunch& G);   // a-8: compaction + fill (only if may_miss)

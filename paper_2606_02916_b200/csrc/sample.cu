@@ -856,30 +856,17 @@ k_select_warp(const int32_t* __restrict__ indices, int fanout, SamplePlan* __res
 
 // ---- the measured ALU roofline of a-1 (include/greengnn.h gg_key_peak) -------------------------
 // Key evaluation and nothing else: every lane walks a register-resident SplitMix state and forms
-// the high word of fmix for each step (all the selection test reads), folded into one word so
-// the work stays alive.  No list stores, no row logic, no memory traffic.  FORM 0 is the
-// formulation of the product loops (key_zhi), FORM 1 forms the high-half shifts with mul.hi; the
-// reported peak is the better of the two.
-template <int FORM>
+// the high word of fmix for each step (all the selection test reads) with the product loops' own
+// key_zhi, folded into one word so the work stays alive.  No list stores, no row logic, no memory
+// traffic.  (Round 1's formulation -- the high-half shifts as mul.hi on the FMA pipe -- measured
+// 1.35 vs 1.41 Tkey/s and is gone.)
 __global__ void __launch_bounds__(256) k_key_peak(uint64_t seed, int groups, uint32_t* __restrict__ fold) {
   uint64_t x = seed + (uint64_t)(blockIdx.x * 256 + threadIdx.x + 1) * 0x632BE59BD9B4E019ull;
   uint32_t acc = 0;
   for (int g = 0; g < groups; ++g) {
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
-      const uint32_t xlo = (uint32_t)x, xhi = (uint32_t)(x >> 32);
-      if (FORM == 0) {
-        acc ^= key_zhi(xlo, xhi);
-      } else {
-        // round 1's formulation: the high-half shifts as mul.hi (FMA pipe)
-        uint32_t lo = xlo ^ __funnelshift_r(xlo, xhi, 30), hi = xhi ^ mulhi_u32(xhi, 1u << 2);
-        const uint64_t p = (uint64_t)lo * kC1lo;
-        hi = mad_lo_u32(lo, kC1hi, mad_lo_u32(hi, kC1lo, (uint32_t)(p >> 32)));
-        lo = (uint32_t)p;
-        lo ^= __funnelshift_r(lo, hi, 27);
-        hi ^= mulhi_u32(hi, 1u << 5);
-        acc ^= mulhi_u32(lo, kC2lo) + hi * kC2lo + lo * kC2hi;
-      }
+      acc ^= key_zhi((uint32_t)x, (uint32_t)(x >> 32));
       x += kGamma;
     }
   }
@@ -888,44 +875,34 @@ __global__ void __launch_bounds__(256) k_key_peak(uint64_t seed, int groups, uin
   if ((threadIdx.x & 31) == 0) atomicXor(fold, acc);
 }
 
-// keys per second of the better formulation (CUDA events on `st`, after one warm-up launch each).
-// fold_out = xor of the keys of formulation 0's timed launches (launch i starts from seed
-// 0x9E37 + i); cudaErrorUnknown if the two formulations fold to different words.
+// keys per second (CUDA events on `st`, after one warm-up launch).  fold_out = xor of the keys of the
+// timed launches (launch i starts from seed 0x9E37 + i).
 cudaError_t key_peak(cudaStream_t st, int ctas_per_sm, int groups, int reps, double* keys_per_s, uint32_t* fold_out) {
   uint32_t* d = nullptr;
-  cudaError_t e = cudaMalloc((void**)&d, 3 * sizeof(uint32_t));
+  cudaError_t e = cudaMalloc((void**)&d, 2 * sizeof(uint32_t));
   if (e != cudaSuccess) return e;
-  cudaMemsetAsync(d, 0, 3 * sizeof(uint32_t), st);
+  cudaMemsetAsync(d, 0, 2 * sizeof(uint32_t), st);
   cudaEvent_t a, b;
   cudaEventCreate(&a);
   cudaEventCreate(&b);
   const int grid = sm_count() * ctas_per_sm;
-  double best = 0;
-  for (int form = 0; form < 2 && e == cudaSuccess; ++form) {
-    if (form == 0) k_key_peak<0><<<grid, 256, 0, st>>>(1ull, groups, d + 2);   // warm-up
-    else k_key_peak<1><<<grid, 256, 0, st>>>(1ull, groups, d + 2);
-    cudaEventRecord(a, st);
-    for (int i = 0; i < reps; ++i) {
-      if (form == 0) k_key_peak<0><<<grid, 256, 0, st>>>(0x9E37ull + i, groups, d);
-      else k_key_peak<1><<<grid, 256, 0, st>>>(0x9E37ull + i, groups, d + 1);
-    }
-    count_launches(reps + 1);
-    cudaEventRecord(b, st);
-    e = cudaEventSynchronize(b);
-    float ms = 0;
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
-    if (e != cudaSuccess) break;
-    const double rate = (double)grid * 256.0 * groups * 32.0 * reps / (ms * 1e-3);
-    if (rate > best) best = rate;
-  }
-  uint32_t h[3] = {0, 0, 0};
+  double rate = 0;
+  k_key_peak<<<grid, 256, 0, st>>>(1ull, groups, d + 1);   // warm-up
+  cudaEventRecord(a, st);
+  for (int i = 0; i < reps; ++i) k_key_peak<<<grid, 256, 0, st>>>(0x9E37ull + i, groups, d);
+  count_launches(reps + 1);
+  cudaEventRecord(b, st);
+  e = cudaEventSynchronize(b);
+  float ms = 0;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+  if (e == cudaSuccess) rate = (double)grid * 256.0 * groups * 32.0 * reps / (ms * 1e-3);
+  uint32_t h[2] = {0, 0};
   if (e == cudaSuccess) e = cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess && h[0] != h[1]) e = cudaErrorUnknown;
   if (fold_out) *fold_out = h[0];
   cudaEventDestroy(a);
   cudaEventDestroy(b);
   cudaFree(d);
-  *keys_per_s = best;
+  *keys_per_s = rate;
   return e;
 }
 
@@ -1003,6 +980,10 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
   // chunks whatever the other cut-overs say
   int hub_bin = chunk_path ? (h_hub_bin > warp_bin ? h_hub_bin : warp_bin) : kBins;
   if (wk.max_degree > 0 && deg_bin((uint32_t)(wk.max_degree > 0x7fffffff ? 0x7fffffff : wk.max_degree)) < hub_bin) hub_bin = kBins;
+  // "whatever the other cut-overs say" includes single_bins: a setting with single_bins > hub_bin would
+  // leave the hub rows of bins [hub_bin, single_bins) as single chunks that the lane kernel finishes while
+  // the rank kernel still reads their (never zeroed) candidate counts.  Hub rows are always multi-chunk.
+  if (single_bins > hub_bin) single_bins = hub_bin;
   const bool multi = chunk_path && (single_bins < warp_bin || hub_bin < kBins);
   cudaMemsetAsync(plan, 0, sizeof(SamplePlan), st);
   count_launches(chunk_path ? (multi ? 6 : 5) : 4);
@@ -1033,5 +1014,8 @@ void launch_sample_hop(cudaStream_t st, const int64_t* indptr, const int32_t* in
 }
 
 int sample_cand_cap(int fanout) { return fanout <= kChunkMaxFanout ? cand_cap(fanout) : 0; }
+// true when the current cut-overs can send a row through the multi-chunk path (the only user of
+// SampleItems::cand): off with the defaults, so the candidate lists need not exist
+bool sampler_multi_chunk_on() { return h_single_bins < h_warp_bin || h_hub_bin < kBins; }
 
 }  // namespace gg

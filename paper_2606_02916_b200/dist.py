@@ -50,6 +50,20 @@ def sum_over_ranks(x: float, device="cpu") -> float:
     return _reduce(x, dist.ReduceOp.SUM, device)
 
 
+def host_threads_for_rank(local_world_size: int = 0, hardware_threads: int = 0) -> int:
+    """gg_config.host_threads for one of `local_world_size` ranks that share a host (default: the
+    LOCAL_WORLD_SIZE torchrun exports).  One rank alone returns 0 = the library's default (0.4 x the
+    hardware threads while copies are queued).  N ranks split that same budget -- the pack threads of all
+    ranks read and write the one host DRAM that already bounds a single rank -- so each
+    gets floor(0.4 x hardware threads / N), at least 1, as a hard cap."""
+    n = local_world_size or int(os.environ.get("LOCAL_WORLD_SIZE", "1"))
+    if n <= 1:
+        return 0
+    hw = hardware_threads or os.cpu_count() or 1
+    budget = min(16, max(2, (hw * 2 + 2) // 5))
+    return max(1, budget // n)
+
+
 def shard_plan(rank: int, world: int, num_parts: int, n_batches: int) -> Tuple[int, List[int]]:
     """(local partition, batch indices) of a rank.  Replicated work, weak scaling: every rank is
     an independent trainer (of partition rank % P) that serves a full epoch's worth of batches in

@@ -18,7 +18,7 @@ def oracle_parts(w):
 
 def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, max_cache_rows=0,
                 check_features=True, cache_samples=64, host_threads=0, oracle_threads=1, host_graph=None,
-                parts=None, cache_buffers=0, lookahead=2, graph=None, first_window_id=0):
+                parts=None, cache_buffers=0, lookahead=2, graph=None, first_window_id=0, oracle_batches=None):
     """Runs one epoch on the GPU and on the oracle; asserts bit-exact agreement everywhere.
     Returns a small summary dict."""
     batches = w.batches if max_batches is None else w.batches[:max_batches]
@@ -39,7 +39,9 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
         w, n_hot=n_hot, carry_over=carry_over, max_window=max(W, 1), staging_mode=staging_mode,
         max_cache_rows=max_cache_rows, host_threads=host_threads, cache_buffers=cache_buffers,
         max_live_windows=lookahead + 1)
-    obatches = {}
+    # oracle_batches: a dict the caller keeps between runs over the SAME batch list (the oracle's batches
+    # depend on graph, seeds, fanouts, seed and batch index only -- not on W, n_hot or the cache)
+    obatches = oracle_batches if oracle_batches is not None else {}
     owin = {}
     stats = dict(batches=0, misses=0, windows=0, rows=0, edges=0)
     wins = ep.windows_of(len(batches), W)
@@ -55,8 +57,8 @@ def check_epoch(w, W, n_hot=-1, carry_over=1, staging_mode=0, max_batches=None, 
         # side; the oracle itself is unchanged and single-threaded per batch
         from concurrent.futures import ThreadPoolExecutor
         with ThreadPoolExecutor(oracle_threads) as ex:
-            for bi, ob in zip(range(len(batches)),
-                              ex.map(lambda bi: ggo.Batch(og, batches[bi], w.fanouts, w.seed, bi), range(len(batches)))):
+            todo = [bi for bi in range(len(batches)) if bi not in obatches]
+            for bi, ob in zip(todo, ex.map(lambda bi: ggo.Batch(og, batches[bi], w.fanouts, w.seed, bi), todo)):
                 obatches[bi] = ob
 
     # the oracle advances its cache window by window in the same order

@@ -20,7 +20,7 @@ def _free_port():
 
 def _worker(rank, world, port, q):
     sys.path.insert(0, ROOT)
-    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world),
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), LOCAL_WORLD_SIZE=str(world),
                       MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     from paper_2606_02916_b200 import dist as gdist
     r, lr, w = gdist.init("gloo")
@@ -29,6 +29,9 @@ def _worker(rank, world, port, q):
     gdist.barrier()
     # rank r "processes" 10 units in (1 + r) seconds
     value, tmax = gdist.aggregate_throughput(10.0, 1.0 + rank)
+    # the ranks of one host split the pack-thread budget a single rank would take (read from LOCAL_WORLD_SIZE)
+    threads = gdist.sum_over_ranks(float(gdist.host_threads_for_rank(hardware_threads=16)))
+    assert threads == 6.0, threads                 # 0.4 x 16 = 6 threads on the host in total, 3 per rank
     q.put((rank, local_part, order, value, tmax, gdist.max_over_ranks(float(rank)), gdist.sum_over_ranks(1.0)))
     gdist.barrier()
 
@@ -60,3 +63,15 @@ def test_single_process_is_identity():
     assert gdist.aggregate_throughput(10.0, 2.0) == (5.0, 2.0)
     lp, order = gdist.shard_plan(0, 1, 4, 7)
     assert lp == 0 and order == list(range(7))
+
+
+def test_pack_thread_split_between_ranks_of_one_host():
+    sys.path.insert(0, ROOT)
+    from paper_2606_02916_b200 import dist as gdist
+    assert gdist.host_threads_for_rank(1, 16) == 0               # alone: the library's default
+    assert gdist.host_threads_for_rank(2, 16) == 3 and gdist.host_threads_for_rank(4, 16) == 1
+    assert gdist.host_threads_for_rank(8, 16) == 1               # never below one thread
+    assert gdist.host_threads_for_rank(8, 192) == 2              # the budget is capped at 16 threads per host
+    for n in (2, 4, 8):
+        for hw in (8, 16, 64, 192):
+            assert n * gdist.host_threads_for_rank(n, hw) <= max(n, min(16, max(2, (hw * 2 + 2) // 5)))

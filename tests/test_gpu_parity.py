@@ -202,7 +202,7 @@ def test_hub_rows_of_1e5_edges(dev):
 
 
 @pytest.mark.parametrize("single_bins,warp_bin,hub_bin", [(28, 48, 128), (28, 128, 128), (36, 48, 60), (28, 28, 128), (128, 128, 128),
-                                                          (40, 64, 64), (36, 36, 40), (36, 36, 52)])
+                                                          (40, 64, 64), (36, 36, 40), (36, 36, 52), (60, 36, 48), (128, 28, 44)])
 def test_selection_cut_overs_do_not_change_results(workload, dev, single_bins, warp_bin, hub_bin):
     """gg_sampler_tune moves rows between the three selection schemes (one lane per row, one lane per
     chunk of 128 positions with the row's candidates merged through global memory, one warp per
@@ -488,6 +488,23 @@ def test_products_full_size_budgeted_W16_two_windows(workload, dev):
     s = pu.check_epoch(w, W=16, n_hot=-(-n_remote // 10), max_batches=32, cache_samples=256, lookahead=6,
                        oracle_threads=_threads())
     assert s["windows"] == 2 and s["misses"] > 0
+
+
+def test_products_full_size_whole_epoch_W16_W32_unlimited_and_budgeted(workload, dev):
+    """The headline config over its WHOLE epoch (one epoch's trace fixes all later ones):
+    all 193 mini-batches at full size, every array of every batch and window against the oracle, for
+    W=16 (13 windows, the last one a single batch) and W=32 (32-batch arenas, counts up to 32 at 5 M-row
+    scale), each with an unlimited budget and with n_hot = 10 % of the remote nodes.  The
+    oracle samples the 193 batches once (they do not depend on W or the budget)."""
+    w = workload("products", dev)
+    assert len(w.batches) == 193
+    n_remote = w.num_nodes - int(w.part_offsets[1] - w.part_offsets[0])
+    shared, hg, parts = {}, w.host_graph(), pu.oracle_parts(w)
+    for W, n_hot in [(16, -1), (32, -1), (16, -(-n_remote // 10)), (32, -(-n_remote // 10))]:
+        s = pu.check_epoch(w, W=W, n_hot=n_hot, cache_samples=64, lookahead=6 if W == 16 else 3,
+                           oracle_threads=_threads(), oracle_batches=shared, host_graph=hg, parts=parts)
+        assert s["batches"] == 193 and s["windows"] == -(-193 // W)
+        assert (s["misses"] == 0) == (n_hot < 0)
 
 
 def test_dense_full_size_W16_two_windows_and_W1(workload, dev):
