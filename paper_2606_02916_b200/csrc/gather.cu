@@ -326,13 +326,13 @@ void launch_miss_path(cudaStream_t st, const GatherLaunch& G) {
     }
     v2 = ok16 ? 16 : (ok8 ? 8 : 4);
   }
-  // Misses that cross the host link: like the pull kernel below, a few CTAs with 8 loads in flight per
-  // thread keep PCIe full; a GPU-wide grid of zero-copy readers only crowds the bulk copies' DMA off the
-  // link and the sampler off the SMs (bench numbers in DESIGN.md Sec. 6).
-#ifndef GG_MISS_LINK_CTAS
-#define GG_MISS_LINK_CTAS 0   /* 0 = the full grid */
-#endif
-  const int grid = (G.miss_over_link && GG_MISS_LINK_CTAS > 0) ? GG_MISS_LINK_CTAS : sm_count() * 4;
+  // Misses that cross the host link: like the pull kernel below, a dozen CTAs with 8 loads in flight per
+  // thread keep PCIe as full as zero-copy reads of 400-byte rows can (0.63 of the pinned-copy peak,
+  // whatever the grid: products, n_hot = 10 %, W=16, miss fill 325-330 ms per epoch at 12 / 24 / 48 / 148 /
+  // 592 CTAs), while a GPU-wide grid of readers crowds the bulk copies' DMA off the link (copies at
+  // 0.66 / 0.50 / 0.40 / 0.32 / 0.34 of the link peak) and the sampler off the SMs.
+  constexpr int kMissLinkCtas = 12;
+  const int grid = G.miss_over_link ? kMissLinkCtas : sm_count() * 4;
   if (v2 == 16) k_rows<16, 1><<<grid, kThreads, 0, st>>>(Rw);
   else if (v2 == 8) k_rows<8, 1><<<grid, kThreads, 0, st>>>(Rw);
   else k_rows<4, 1><<<grid, kThreads, 0, st>>>(Rw);
