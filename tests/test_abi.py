@@ -69,3 +69,21 @@ def test_no_cpu_fallback_when_library_missing(tmp_path):
 
 def test_version_string(lib):
     assert b"sm_100a" in lib.gg_version()
+
+
+def test_static_unique_count_rejects_bad_sizes_before_touching_the_gpu(lib):
+    """gg_unique_count_static validates its arguments before its first CUDA call, so the limit of its
+    fixed workspace can be checked here: one node more than GG_STATIC_MAX_NODES is GG_ERR_CAPACITY with
+    a message that names the limit; null outputs and negative sizes are GG_ERR_INVALID_ARG."""
+    from paper_2606_02916_b200 import binding
+    src = open(HEADER).read()
+    m = re.search(r"#define\s+GG_STATIC_MAX_NODES\s+\(1\s*<<\s*(\d+)\)", src)
+    assert m and (1 << int(m.group(1))) == binding.GG_STATIC_MAX_NODES == 4_194_304
+    stats = (C.c_int32 * 2)()
+    f = lib.gg_unique_count_static
+    assert f(None, 0, binding.GG_STATIC_MAX_NODES + 1, None, None, 0, stats, None) == binding.GG_ERR_CAPACITY
+    assert b"GG_STATIC_MAX_NODES" in lib.gg_last_error()
+    assert f(None, 0, 1000, None, None, 0, None, None) == binding.GG_ERR_INVALID_ARG      # no stats
+    assert f(None, 5, 1000, None, None, 0, stats, None) == binding.GG_ERR_INVALID_ARG     # ids missing
+    assert f(None, 0, 0, None, None, 0, stats, None) == binding.GG_ERR_INVALID_ARG        # num_nodes < 1
+    assert f(None, 0, 1000, None, None, 4, stats, None) == binding.GG_ERR_INVALID_ARG     # capacity without outputs
