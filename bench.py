@@ -706,7 +706,7 @@ def run_ours(args):
     ach = pg["bytes"] / (pg["ms"] * 1e-3) / 1e9 if pg["ms"] > 0 else 0.0
     g_scale = args.steps * n_b / max(pg["regions"], 1)      # one launch in four carries an event pair
     roof_gather = {"bound": "hbm", "kernel": "k_gather", "achieved": ach, "peak": peak, "unit": "GB/s",
-                   "frac": ach / peak, "traffic": ncu_traffic("r02_gather_ncu_summary.txt"), "peak_source": peak_src,
+                   "frac": ach / peak, "traffic": ncu_traffic("r03_gather_ncu_summary.txt"), "peak_source": peak_src,
                    "launches": args.steps * n_b, "bracketed_launches": pg["regions"],
                    "avg_launch_us": 1e3 * pg["ms"] / max(pg["regions"], 1),
                    "algorithmic_bytes_per_launch": pg["bytes"] / max(pg["regions"], 1),
